@@ -1,0 +1,226 @@
+/*
+ * lazy_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU statement of what the LazyAttention hot path computes
+ * (arxiv/paper_2606_04302).  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may load this file.  It shares no code,
+ * header, table or constant with the CUDA path under paper_2606_04302_b200/.
+ *
+ * Result definition (PAPER.md: LazyAttention "is mathematically identical to
+ * existing methods that duplicate KV caches for position re-encoding"):
+ *   1. materialise, per request, a RoPE-rotated copy of every visible key at its
+ *      logical position ("deferred encoding", L164-166 rotation
+ *      formula, Fig. 3b "K1/K2 denote the RoPE half-dimensions");
+ *   2. run textbook causal softmax attention softmax(f(Q,m) f(K,n)^T / sqrt(d_k)) V
+ *      (Eq. 4 and its RoPE form) with the GQA head mapping
+ *      hk = hq / (Hq/Hkv).
+ * No tiling, no online softmax, no fusion: every step is the definition written out.
+ * OpenMP only distributes independent output rows over host cores.
+ *
+ * Readings of the paper taken here: half-split pairing
+ * (j, j+D/2); theta_j = theta^(-2j/D); q arrives un-rotated and is rotated by the
+ * position of its own token; causal mask by sequence index (s <= sq), positions feed
+ * only RoPE; scale 1/sqrt(D).
+ *
+ * Pins: tests/test_oracle_pins.py (brute force, closed forms, shift invariance,
+ * SDPA reduction, sharing equivalence, golden worked examples).  No function here is
+ * "parity unpinned".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define DT_F64 0
+#define DT_BF16 1
+
+/* exact bf16 -> double (bf16 is the top 16 bits of an IEEE fp32) */
+static double bf16_to_double(uint16_t b) {
+    uint32_t u = ((uint32_t)b) << 16;
+    float f;
+    memcpy(&f, &u, sizeof f);
+    return (double)f;
+}
+
+static inline double load_elem(const void* base, int dtype, int64_t idx) {
+    if (dtype == DT_BF16) return bf16_to_double(((const uint16_t*)base)[idx]);
+    return ((const double*)base)[idx];
+}
+
+/* RoPE, half-split pairing.  PAPER.md L164-166:
+ *   k1' = k1 cos(D) - k2 sin(D),  k2' = k1 sin(D) + k2 cos(D)
+ * with k1 = x[0:D/2], k2 = x[D/2:D]; angle for pair j is pos * theta^(-2j/D) (RoPE, Su et al.,
+ * cited at PAPER.md L102; stateless, from the absolute index: PAPER.md L455). */
+void lazy_oracle_rope(const double* x, double pos, int D, double theta, double* y) {
+    int half = D / 2;
+    for (int j = 0; j < half; ++j) {
+        double a = pos * pow(theta, -2.0 * (double)j / (double)D);
+        double c = cos(a), s = sin(a);
+        y[j] = x[j] * c - x[j + half] * s;
+        y[j + half] = x[j] * s + x[j + half] * c;
+    }
+}
+
+/* Core: attention of n_q query rows over L keys with explicit positions.
+ *   q      [n_q][Hq][D]   un-rotated queries
+ *   k, v   [L][Hkv][D]    un-rotated keys, values (already gathered)
+ *   pos_q  [n_q], pos_k [L]  logical positions (doubles so tests may pass any value)
+ *   vis    [n_q]          query i sees key indices s <= vis[i]  (index-based causal mask)
+ *   out    [n_q][Hq][D]
+ *   probs  optional [n_q][Hq][L] softmax weights (0 beyond vis); may be NULL
+ *   khat_out optional [L][Hkv][D] the materialised rotated keys; may be NULL
+ *   qhat_out optional [n_q][Hq][D]; may be NULL
+ * Step 1 materialises Khat = R_{pos_k} K (the "duplicate + re-encode" copy),
+ * step 2 is Eq. 4 on (R_{pos_q} q, Khat, V).
+ */
+int lazy_oracle_attend_core(const double* q, const double* k, const double* v,
+                            const double* pos_q, const double* pos_k, const int64_t* vis,
+                            int n_q, int64_t L, int Hq, int Hkv, int D, double theta,
+                            const uint8_t* row_select,
+                            double* out, double* probs, double* khat_out, double* qhat_out) {
+    if (Hq % Hkv != 0 || D % 2 != 0) return -1;
+    int group = Hq / Hkv;
+    double* khat = (double*)malloc(sizeof(double) * (size_t)(L > 0 ? L : 1) * Hkv * D);
+    if (!khat) return -2;
+    /* 1. materialise the rotated copy */
+#pragma omp parallel for schedule(static)
+    for (int64_t s = 0; s < L; ++s)
+        for (int hk = 0; hk < Hkv; ++hk)
+            lazy_oracle_rope(k + ((size_t)s * Hkv + hk) * D, pos_k[s], D, theta,
+                             khat + ((size_t)s * Hkv + hk) * D);
+    if (khat_out) memcpy(khat_out, khat, sizeof(double) * (size_t)L * Hkv * D);
+    /* 2. standard attention, one (query row, head) at a time */
+    int64_t n_rows = (int64_t)n_q * Hq;
+    int err = 0;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t row = 0; row < n_rows; ++row) {
+        int i = (int)(row / Hq), hq = (int)(row % Hq);
+        if (row_select && !row_select[i]) continue;
+        int hk = hq / group;
+        int64_t last = vis[i];               /* keys 0..last visible */
+        if (last >= L) last = L - 1;
+        double* o = out + ((size_t)i * Hq + hq) * D;
+        for (int d = 0; d < D; ++d) o[d] = 0.0;
+        double* qhat = (double*)malloc(sizeof(double) * D);
+        double* sc = (double*)malloc(sizeof(double) * (size_t)(last >= 0 ? last + 1 : 1));
+        if (!qhat || !sc) { err = 1; free(qhat); free(sc); continue; }
+        lazy_oracle_rope(q + ((size_t)i * Hq + hq) * D, pos_q[i], D, theta, qhat);
+        if (qhat_out) memcpy(qhat_out + ((size_t)i * Hq + hq) * D, qhat, sizeof(double) * D);
+        if (probs) for (int64_t s = 0; s < L; ++s) probs[((size_t)i * Hq + hq) * L + s] = 0.0;
+        if (last >= 0) {
+            double m = -INFINITY;
+            for (int64_t s = 0; s <= last; ++s) {
+                const double* kr = khat + ((size_t)s * Hkv + hk) * D;
+                double acc = 0.0;
+                for (int d = 0; d < D; ++d) acc += qhat[d] * kr[d];
+                sc[s] = acc / sqrt((double)D);
+                if (sc[s] > m) m = sc[s];
+            }
+            double l = 0.0;
+            for (int64_t s = 0; s <= last; ++s) { sc[s] = exp(sc[s] - m); l += sc[s]; }
+            for (int64_t s = 0; s <= last; ++s) {
+                double p = sc[s] / l;
+                if (probs) probs[((size_t)i * Hq + hq) * L + s] = p;
+                const double* vr = v + ((size_t)s * Hkv + hk) * D;
+                for (int d = 0; d < D; ++d) o[d] += p * vr[d];
+            }
+        }
+        free(qhat); free(sc);
+    }
+    free(khat);
+    return err ? -2 : 0;
+}
+
+/* Paged wrapper (the three-call boundary's read side; PAPER.md L83-88 problem statement, L173/L182
+ * per-document offsets carried as metadata -- here one logical start per page, north_star).
+ * For request r: sequence index s lives in table slot s/P at in-page offset s%P, physical page
+ * block_table[r][s/P], logical position page_logical_pos[r][s/P] + s%P.  The n_q query tokens are the
+ * last n_q tokens of the sequence (already written to the cache): sq = L - n_q + i.
+ *   q [total_q][Hq][D] (dtype_q), k_pool/v_pool [num_pages][Hkv][P][D] (dtype_kv)
+ *   out [total_q][Hq][D] double.  row_select optional [total_q] (0 = skip row, left untouched).
+ * Rows of requests with seq_len == 0 are written as zeros.
+ */
+int lazy_oracle_attend_paged(const void* q, int dtype_q, const void* k_pool, const void* v_pool, int dtype_kv,
+                             const int32_t* block_table, const int32_t* page_logical_pos, int64_t table_stride,
+                             const int32_t* seq_lens, const int32_t* cu_q_lens, int num_reqs,
+                             int Hq, int Hkv, int D, int P, double theta,
+                             const uint8_t* row_select, double* out) {
+    for (int r = 0; r < num_reqs; ++r) {
+        int64_t L = seq_lens[r];
+        int q0 = cu_q_lens[r], n_q = cu_q_lens[r + 1] - cu_q_lens[r];
+        if (n_q <= 0) continue;
+        if (row_select) {
+            int any = 0;
+            for (int i = 0; i < n_q; ++i) any |= row_select[q0 + i];
+            if (!any) continue;
+        }
+        if (L <= 0) {
+            for (int64_t e = 0; e < (int64_t)n_q * Hq * D; ++e) out[(size_t)q0 * Hq * D + e] = 0.0;
+            continue;
+        }
+        if (n_q > L) return -1;
+        double* kg = (double*)malloc(sizeof(double) * (size_t)L * Hkv * D);
+        double* vg = (double*)malloc(sizeof(double) * (size_t)L * Hkv * D);
+        double* pos = (double*)malloc(sizeof(double) * (size_t)L);
+        double* qd = (double*)malloc(sizeof(double) * (size_t)n_q * Hq * D);
+        double* pos_q = (double*)malloc(sizeof(double) * (size_t)n_q);
+        int64_t* vis = (int64_t*)malloc(sizeof(int64_t) * (size_t)n_q);
+        if (!kg || !vg || !pos || !qd || !pos_q || !vis) return -2;
+        /* gather the request's rows through the block table */
+#pragma omp parallel for schedule(static)
+        for (int64_t s = 0; s < L; ++s) {
+            int64_t slot = s / P, t = s % P;
+            int64_t page = block_table[(size_t)r * table_stride + slot];
+            pos[s] = (double)page_logical_pos[(size_t)r * table_stride + slot] + (double)t;
+            for (int hk = 0; hk < Hkv; ++hk) {
+                int64_t base = (((int64_t)page * Hkv + hk) * P + t) * D;
+                for (int d = 0; d < D; ++d) {
+                    kg[((size_t)s * Hkv + hk) * D + d] = load_elem(k_pool, dtype_kv, base + d);
+                    vg[((size_t)s * Hkv + hk) * D + d] = load_elem(v_pool, dtype_kv, base + d);
+                }
+            }
+        }
+        for (int64_t e = 0; e < (int64_t)n_q * Hq * D; ++e) qd[e] = load_elem(q, dtype_q, (int64_t)q0 * Hq * D + e);
+        for (int i = 0; i < n_q; ++i) {
+            int64_t sq = L - n_q + i;        /* sequence index of this query token */
+            vis[i] = sq;
+            pos_q[i] = pos[sq];
+        }
+        int rc = lazy_oracle_attend_core(qd, kg, vg, pos_q, pos, vis, n_q, L, Hq, Hkv, D, theta,
+                                         row_select ? row_select + q0 : NULL,
+                                         out + (size_t)q0 * Hq * D, NULL, NULL, NULL);
+        free(kg); free(vg); free(pos); free(qd); free(pos_q); free(vis);
+        if (rc) return rc;
+    }
+    return 0;
+}
+
+/* lazy_cache_write oracle: bit copy of un-rotated rows into pages (the cache is
+ * "purely content-based keys and values").  slot = page*P + off; slot < 0 skips the token.
+ *   k_new/v_new [T][Hkv][D] 16-bit words, pools [num_pages][Hkv][P][D] 16-bit words. */
+int lazy_oracle_cache_write(const uint16_t* k_new, const uint16_t* v_new, const int64_t* slot_mapping,
+                            int64_t num_tokens, int Hkv, int D, int P, int64_t num_pages,
+                            uint16_t* k_pool, uint16_t* v_pool) {
+    for (int64_t t = 0; t < num_tokens; ++t) {
+        int64_t slot = slot_mapping[t];
+        if (slot < 0) continue;
+        int64_t page = slot / P, off = slot % P;
+        if (page >= num_pages) return -1;
+        for (int hk = 0; hk < Hkv; ++hk) {
+            int64_t dst = ((page * Hkv + hk) * P + off) * D;
+            int64_t src = (t * Hkv + hk) * D;
+            memcpy(k_pool + dst, k_new + src, sizeof(uint16_t) * D);
+            memcpy(v_pool + dst, v_new + src, sizeof(uint16_t) * D);
+        }
+    }
+    return 0;
+}
+
+int lazy_oracle_num_threads(void) {
+#ifdef _OPENMP
+    extern int omp_get_max_threads(void);
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
