@@ -1,0 +1,472 @@
+#!/usr/bin/env python
+"""bench.py -- LazyAttention hot path on B200: one JSON line per run (see README "Benchmark").
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg3|cfg4|cfg5] [--impl ours|reference]
+
+A step = one pass of the whole hot path over one synthetic Zipf-shared RAG batch: lazy_cache_write of the
+step's new tokens, then the attention call(s) (decode for cfg2/cfg4, prefill for cfg3, prefill + decode for
+cfg5).  Default workload: BASELINE.json configs[1] (decode at the Llama-3-8B layer shape); unless
+--no-secondary, the prefill headline (configs[2]) is measured in the same run and reported under "prefill".
+`--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm=float(d["hbm_gbs"]), tensor=float(d["bf16_tflops"]),
+                    tensor_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])), source="measured")
+    return dict(hbm=6650.0, tensor=1590.0, tensor_sustained=1400.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------------
+def make_batch(workload: str, rank: int, noshare: bool = False):
+    from paper_2606_04302_b200 import workloads as W
+    idx = int(workload[3:])
+    if idx == 5:
+        return W.config5()
+    kw = dict(noshare=True) if noshare else {}
+    b = W.CONFIGS[idx](**kw)
+    if rank:
+        # weak scaling: every rank owns a batch of the same shape drawn from its own seed
+        import dataclasses  # noqa: F401
+        W_SEED = W.SEED0
+        W.SEED0 = W_SEED + 1000 * rank
+        try:
+            b = W.CONFIGS[idx](**kw)
+        finally:
+            W.SEED0 = W_SEED
+    return b
+
+
+def step_work(batch, steps):
+    """Algorithmic work of the timed attention calls."""
+    sh = batch.shape
+    logical = 0          # decode: K and V once per (token, kv head): 2*D*2 B, + q/out
+    flops = 0            # prefill: 4*D FLOPs per visible (query, key) pair per q head
+    q_tokens = dec_tokens = kv_tokens = 0
+    for st in steps:
+        L = st.seq_lens.numpy().astype(np.int64)
+        if st.kind == "decode":
+            logical += int(L.sum()) * sh.num_kv_heads * sh.head_dim * 2 * 2
+            logical += len(L) * sh.num_q_heads * sh.head_dim * 2 * 2
+            dec_tokens += len(L)
+            kv_tokens += int(L.sum())
+        else:
+            nq = (st.cu_q_lens[1:] - st.cu_q_lens[:-1]).numpy().astype(np.int64)
+            pairs = int((nq * (L - nq) + nq * (nq + 1) // 2).sum())
+            flops += 4 * sh.head_dim * sh.num_q_heads * pairs
+            q_tokens += int(nq.sum())
+    return dict(logical_bytes=logical, flops=flops, q_tokens=q_tokens, dec_tokens=dec_tokens, kv_tokens=kv_tokens)
+
+
+def unique_bytes(batch, steps):
+    sh = batch.shape
+    P = sh.page_size
+    pages = set()
+    for st in steps:
+        if st.kind != "decode":
+            continue
+        bt = batch.block_table if st.req_ids is None else batch.block_table[st.req_ids]
+        for r, L in enumerate(st.seq_lens.tolist()):
+            pages.update(bt[r, : (L + P - 1) // P].tolist())
+    return len(pages) * sh.num_kv_heads * P * sh.head_dim * 2 * 2
+
+
+class GpuJob:
+    """Holds the device-resident batch and replays its timed step."""
+
+    def __init__(self, batch, device):
+        from paper_2606_04302_b200.runner import DeviceBatch
+        from paper_2606_04302_b200 import binding as B
+        self.B = B
+        self.batch = batch
+        self.dev = DeviceBatch(batch, device=device)
+        d = self.dev.device
+        self.timed = []
+        for st in batch.steps:
+            if st.kind == "write_only":
+                self.dev.write(st)                     # set-up: question tokens already in the cache
+        # cfg5's follow-up decode (last step) is a correctness-only call: not timed
+        steps = [s for s in batch.steps if s.kind != "write_only"]
+        if batch.name.startswith("cfg5"):
+            steps = steps[:2]
+        for st in steps:
+            bt, pp = self.dev.tables_for(st)
+            rec = dict(step=st, bt=bt, pp=pp, q=st.q.to(d), out=torch.empty_like(st.q, device=d),
+                       sl=st.seq_lens.to(d), k_new=st.k_new.to(d), v_new=st.v_new.to(d),
+                       slots=st.slot_mapping.to(d))
+            if st.kind == "prefill":
+                rec["cu"] = st.cu_q_lens.to(d)
+                rec["max_q"] = int((st.cu_q_lens[1:] - st.cu_q_lens[:-1]).max())
+            self.timed.append(rec)
+        self.flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device=d)
+
+    def flush_l2(self):
+        self.flush_buf.fill_(1)
+
+    def run(self, ev_mid=None):
+        B, dev = self.B, self.dev
+        for rec in self.timed:
+            B.lazy_cache_write(dev.handle, rec["k_new"], rec["v_new"], rec["slots"], dev.k_pool, dev.v_pool)
+        if ev_mid is not None:
+            ev_mid.record()
+        for rec in self.timed:
+            if rec["step"].kind == "decode":
+                B.lazy_attn_decode(dev.handle, rec["q"], dev.k_pool, dev.v_pool, rec["bt"], rec["pp"], rec["sl"],
+                                   rec["out"])
+            else:
+                B.lazy_attn_prefill(dev.handle, rec["q"], dev.k_pool, dev.v_pool, rec["bt"], rec["pp"], rec["sl"],
+                                    rec["cu"], rec["max_q"], rec["out"])
+
+    def time_steps(self, steps, warmup, barrier):
+        for _ in range(warmup):
+            self.flush_l2(); self.run()
+        n0 = self.dev.handle.launch_count()
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(steps)]
+        barrier(); torch.cuda.synchronize()
+        for i in range(steps):
+            self.flush_l2()                          # > L2 (126 MB) written between timed iterations
+            evs[i][0].record()
+            self.run(ev_mid=evs[i][1])
+            evs[i][2].record()
+        torch.cuda.synchronize(); barrier()
+        total = sum(e[0].elapsed_time(e[2]) for e in evs)
+        attn = sum(e[1].elapsed_time(e[2]) for e in evs)
+        return total, attn, self.dev.handle.launch_count() - n0
+
+    # -------- end to end through lazy_host_step (HOST buffers; copies inside the timed region)
+    def prepare_e2e(self):
+        B, dev = self.B, self.dev
+        pin = lambda t: t.contiguous().pin_memory()
+        self.e2e = []
+        for rec in self.timed:
+            st = rec["step"]
+            bt = self.batch.block_table if st.req_ids is None else self.batch.block_table[st.req_ids]
+            pp = self.batch.page_logical_pos if st.req_ids is None else self.batch.page_logical_pos[st.req_ids]
+            R, tq, nn = st.seq_lens.shape[0], st.q.shape[0], st.k_new.shape[0]
+            host = dict(q=pin(st.q), k=pin(st.k_new), v=pin(st.v_new), s=pin(st.slot_mapping), bt=pin(bt), pp=pin(pp),
+                        sl=pin(st.seq_lens), cu=pin(st.cu_q_lens), out=torch.empty_like(st.q).pin_memory())
+            nbytes = B.lazy_host_step_staging_bytes(dev.handle, R, tq, nn)
+            staging = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev.device)
+            base = (staging.data_ptr() + 255) // 256 * 256
+            kind = 0 if st.kind == "decode" else 1
+            args = B.HostStep(kind, R, tq, rec.get("max_q", 1), nn, 0, host["q"].data_ptr(), host["k"].data_ptr(),
+                              host["v"].data_ptr(), host["s"].data_ptr(), host["bt"].data_ptr(),
+                              host["pp"].data_ptr(), host["sl"].data_ptr(), host["cu"].data_ptr(),
+                              host["out"].data_ptr(), dev.k_pool.data_ptr(), dev.v_pool.data_ptr(), base, nbytes)
+            h2d = sum(host[k].numel() * host[k].element_size() for k in ("q", "k", "v", "s", "bt", "pp", "sl"))
+            if kind == 1:
+                h2d += host["cu"].numel() * 4
+            d2h = host["out"].numel() * 2
+            self.e2e.append(dict(args=args, host=host, staging=staging, h2d=h2d, d2h=d2h))
+
+    def run_e2e(self):
+        for e in self.e2e:
+            self.B.lazy_host_step(self.dev.handle, e["args"])
+
+    def time_e2e(self, steps, warmup, barrier):
+        for _ in range(warmup):
+            self.flush_l2(); self.run_e2e()
+        evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(steps)]
+        barrier(); torch.cuda.synchronize()
+        for i in range(steps):
+            self.flush_l2()
+            evs[i][0].record()
+            self.run_e2e()
+            evs[i][1].record()
+        torch.cuda.synchronize(); barrier()
+        return sum(e[0].elapsed_time(e[1]) for e in evs)
+
+
+def headline(workload, work, ms_step):
+    s = ms_step * 1e-3
+    if workload in ("cfg2", "cfg4"):
+        return "decode_attn_logical_GBps", work["logical_bytes"] / s / 1e9, "GB/s"
+    if workload == "cfg3":
+        return "prefill_attn_TFLOPs", work["flops"] / s / 1e12, "TFLOP/s"
+    return "mixed_step_attn_tokens_per_s", (work["q_tokens"] + work["dec_tokens"]) / s, "tokens/s"
+
+
+# ------------------------------------------------------------------------------------------------------
+def oracle_sample(workload, batch, budget_s=20.0):
+    """Times the oracle as it stands on a bounded sample of the workload; returns (value in the headline's
+    unit, seconds, description).  Decode: the first requests; prefill: seeded query rows of request 0."""
+    from oracle import oracle as O
+    O.build()
+    sh = batch.shape
+    steps = [s for s in batch.steps if s.kind != "write_only"]
+    if batch.name.startswith("cfg5"):
+        steps = steps[:2]
+    k_ref, v_ref = batch.k_pool.clone(), batch.v_pool.clone()
+    for st in batch.steps:
+        if st.k_new is not None:
+            O.cache_write(st.k_new, st.v_new, st.slot_mapping.numpy(), k_ref, v_ref, sh.page_size)
+    t_total, logical, flops, toks = 0.0, 0, 0, 0
+    desc = []
+    for st in steps:
+        bt = batch.block_table if st.req_ids is None else batch.block_table[st.req_ids]
+        pp = batch.page_logical_pos if st.req_ids is None else batch.page_logical_pos[st.req_ids]
+        R = st.seq_lens.shape[0]
+        if st.kind == "decode":
+            n = max(1, min(R, 64))
+            sl = st.seq_lens[:n].numpy()
+            t0 = time.perf_counter()
+            O.attend_paged(st.q[:n], k_ref, v_ref, bt[:n].numpy(), pp[:n].numpy(), sl,
+                           np.arange(n + 1, dtype=np.int32), num_q_heads=sh.num_q_heads,
+                           num_kv_heads=sh.num_kv_heads, head_dim=sh.head_dim, page_size=sh.page_size,
+                           theta=sh.rope_theta)
+            t_total += time.perf_counter() - t0
+            logical += int(sl.sum()) * sh.num_kv_heads * sh.head_dim * 4 + n * sh.num_q_heads * sh.head_dim * 4
+            toks += n
+            desc.append(f"decode: first {n} of {R} requests")
+        else:
+            nq = int(st.cu_q_lens[1] - st.cu_q_lens[0])
+            L = int(st.seq_lens[0])
+            rows = min(nq, 16)
+            sel = np.zeros(nq, dtype=np.uint8)
+            pick = np.sort(np.random.default_rng(0).choice(nq, size=rows, replace=False))
+            sel[pick] = 1
+            t0 = time.perf_counter()
+            O.attend_paged(st.q[:nq], k_ref, v_ref, bt[:1].numpy(), pp[:1].numpy(), st.seq_lens[:1].numpy(),
+                           np.array([0, nq], dtype=np.int32), num_q_heads=sh.num_q_heads,
+                           num_kv_heads=sh.num_kv_heads, head_dim=sh.head_dim, page_size=sh.page_size,
+                           theta=sh.rope_theta, row_select=sel)
+            t_total += time.perf_counter() - t0
+            flops += 4 * sh.head_dim * sh.num_q_heads * int(sum(L - nq + i + 1 for i in pick))
+            toks += rows
+            desc.append(f"prefill: {rows} seeded query rows of request 0 of {R} (materialise + attend)")
+    if workload in ("cfg2", "cfg4"):
+        v = logical / t_total / 1e9
+    elif workload == "cfg3":
+        v = flops / t_total / 1e12
+    else:
+        v = toks / t_total
+    return v, t_total, "; ".join(desc), O.num_threads()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--noshare", action="store_true", help="every drawn document distinct (logical == unique bytes)")
+    ap.add_argument("--no-secondary", action="store_true", help="skip the prefill (cfg3) and noshare side measurements")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    peaks = load_peaks()
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        batch = make_batch(args.workload, 0, args.noshare)
+        work = step_work(batch, [s for s in batch.steps if s.kind != "write_only"][:2 if args.workload == "cfg5" else None])
+        vals, secs = [], []
+        sample = ""
+        for i in range(args.warmup + args.steps):
+            v, t, sample, cores = oracle_sample(args.workload, batch)
+            if i >= args.warmup:
+                vals.append(v); secs.append(t)
+        metric, _, unit = headline(args.workload, work, 1.0)
+        value = float(np.mean(vals))
+        print(json.dumps({
+            "impl": "reference", "metric": metric, "value": value, "unit": unit, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": float(np.mean(secs) * 1e3),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.workload + (" noshare" if args.noshare else ""), "batch": batch.name,
+                       "note": "each step is a bounded sample of the workload"},
+            "cpu_baseline": {"value": value, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}))
+        return
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    device = f"cuda:{local_rank}"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(device))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    def max_over_ranks(x: float) -> float:
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    from paper_2606_04302_b200 import build as lazy_build
+    if rank == 0:
+        lazy_build.build()
+    barrier()
+
+    batch = make_batch(args.workload, rank, args.noshare)
+    job = GpuJob(batch, device)
+    work = step_work(batch, [r["step"] for r in job.timed])
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    total_ms, attn_ms, launches = job.time_steps(args.steps, args.warmup, barrier)
+    clocks = sampler.stop()
+    total_ms, attn_ms = max_over_ranks(total_ms), max_over_ranks(attn_ms)
+    ms_step, ms_attn = total_ms / args.steps, attn_ms / args.steps
+    job.prepare_e2e()
+    e2e_ms = max_over_ranks(job.time_e2e(args.steps, args.warmup, barrier)) / args.steps
+
+    metric, value1, unit = headline(args.workload, work, ms_step)
+    _, e2e1, _ = headline(args.workload, work, e2e_ms)
+    value, e2e_value = value1 * world, e2e1 * world           # whole-job aggregate (weak scaling: same work per rank)
+
+    if args.workload in ("cfg2", "cfg4", "cfg5"):
+        ach = work["logical_bytes"] / (ms_attn * 1e-3) / 1e9 if args.workload != "cfg5" else None
+    roof = None
+    if args.workload in ("cfg2", "cfg4"):
+        ub = unique_bytes(batch, [r["step"] for r in job.timed])
+        roof = {"bound": "hbm", "kernel": "lazy_attn_decode (split-KV + combine)", "achieved": ach,
+                "peak": peaks["hbm"], "unit": "GB/s", "frac": ach / peaks["hbm"], "traffic": None,
+                "peak_source": peaks["source"], "algorithmic_bytes_per_launch": work["logical_bytes"],
+                "unique_bytes_per_launch": ub, "achieved_unique": ub / (ms_attn * 1e-3) / 1e9,
+                "kernel_ms": ms_attn}
+    elif args.workload == "cfg3":
+        ach = work["flops"] / (ms_attn * 1e-3) / 1e12
+        roof = {"bound": "tensor", "kernel": "lazy_attn_prefill", "achieved": ach, "peak": peaks["tensor"],
+                "unit": "TFLOP/s", "frac": ach / peaks["tensor"], "traffic": None, "peak_source": peaks["source"],
+                "algorithmic_flops_per_launch": work["flops"], "kernel_ms": ms_attn}
+    else:
+        roof = {"bound": "hbm", "kernel": "mixed step (prefill + decode)", "achieved": None, "peak": peaks["hbm"],
+                "unit": "GB/s", "frac": None, "traffic": None, "kernel_ms": ms_attn}
+
+    out = {
+        "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic",
+        "config": {"workload": args.workload + (" noshare" if args.noshare else ""), "batch": batch.name,
+                   "heads": [batch.shape.num_q_heads, batch.shape.num_kv_heads, batch.shape.head_dim],
+                   "num_reqs": int(sum(len(r["step"].seq_lens) for r in job.timed)),
+                   "distinct_docs": batch.meta.get("distinct_docs"), "l2": "flushed between timed steps (512 MB fill)",
+                   "parallelism": f"request-parallel replicas x{world}, no data-path collective"},
+        "tokens_per_s": {"decode_tokens": work["dec_tokens"] / (ms_step * 1e-3) * world,
+                         "kv_tokens_attended": work["kv_tokens"] / (ms_step * 1e-3) * world,
+                         "prefill_query_tokens": work["q_tokens"] / (ms_step * 1e-3) * world},
+        "roofline": roof,
+        "e2e": {"value": e2e_value, "unit": unit, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": int(sum(e["h2d"] for e in job.e2e)),
+                "d2h_bytes_per_step": int(sum(e["d2h"] for e in job.e2e))},
+        "gpu_launches": int(launches), "clocks": clocks,
+    }
+    job.dev.close()
+    del job
+    torch.cuda.empty_cache()
+
+    if rank == 0 and world == 1 and not args.no_secondary and args.workload == "cfg2":
+        # side measurements in the same run: the prefill headline (configs[2]) and the noshare decode variant
+        side = {}
+        for name, wl, ns in (("decode_noshare", "cfg2", True), ("prefill", "cfg3", False)):
+            try:
+                b2 = make_batch(wl, 0, ns)
+                j2 = GpuJob(b2, device)
+                w2 = step_work(b2, [r["step"] for r in j2.timed])
+                k = max(5, args.steps // 3)
+                t_ms, a_ms, _ = j2.time_steps(k, 3, barrier)
+                a = a_ms / k
+                if wl == "cfg3":
+                    tf = w2["flops"] / (a * 1e-3) / 1e12
+                    side[name] = {"workload": "cfg3", "kernel_ms": a, "ms_per_step": t_ms / k, "TFLOPs": tf,
+                                  "frac_of_bf16_peak": tf / peaks["tensor"],
+                                  "frac_of_bf16_sustained": tf / peaks["tensor_sustained"],
+                                  "query_tokens_per_s": w2["q_tokens"] / (t_ms / k * 1e-3)}
+                else:
+                    gb = w2["logical_bytes"] / (a * 1e-3) / 1e9
+                    side[name] = {"workload": "cfg2 noshare", "kernel_ms": a, "GBps": gb,
+                                  "frac_of_hbm_peak": gb / peaks["hbm"]}
+                j2.dev.close()
+                del j2, b2
+                torch.cuda.empty_cache()
+            except Exception as e:  # a side measurement must not lose the headline
+                side[name] = {"error": repr(e)}
+        out.update(side)
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        v, t, sample, cores = oracle_sample(args.workload, batch)
+        out["cpu_baseline"] = {"value": v, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample,
+                               "seconds": t}
+    if rank == 0:
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

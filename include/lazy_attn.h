@@ -1,0 +1,161 @@
+/*
+ * lazy_attn.h -- C ABI of liblazyattn.so: the LazyAttention hot path on B200 (sm_100a).
+ *
+ * Paged attention over a KV cache that stores keys UN-ROTATED (pre-RoPE).  Every page of a request
+ * carries, next to its physical page id, the logical position of its first token; the kernels apply
+ * RoPE on chip, so one physical copy of a document's KV serves many requests at different positions
+ * with no materialised re-encoding and no writes on the read path.
+ *
+ * What the calls compute is defined by the paper (arxiv/paper_2606_04302, /root/reference/PAPER.md):
+ *   - deferred positional encoding: Q/K/V are produced without positions, RoPE is applied during
+ *     attention after fetching from the cache (section 3.1; Fig. 1b L29-31);
+ *   - attention with RoPE  softmax(f(Q,m) f(K,n)^T / sqrt(d_k)) V  (Eq. 4);
+ *   - half-split rotation  k1' = k1 cos - k2 sin, k2' = k1 sin + k2 cos  (Fig. 3b);
+ *   - one cached copy reused by several requests at different global offsets inside one batch
+ *     (PAPER.md L83-88 problem statement; L173/L182 offsets carried as metadata);
+ *   - the result is exactly what duplicating + re-encoding the KV would give.
+ * Readings taken where the paper is silent are listed in DESIGN.md ("Readings of the paper").
+ *
+ * Conventions common to all calls
+ *   - All tensor pointers are DEVICE pointers owned by the caller, 16-byte aligned, bf16 unless stated.
+ *     `cfg`, `out` handle pointers and the returned strings are HOST pointers.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Every call only
+ *     enqueues work on it: no host synchronisation, no device allocation, no host<->device copies.
+ *   - The library owns nothing on the device except what it places inside the caller's `workspace`.
+ *   - lazy_attn_* never write k_cache / v_cache (read path is read-only).
+ *   - Return value: 0 = OK, <0 = error (lazy_status_string).  Errors are detected on the host from the
+ *     scalar arguments only; the CONTENTS of device tables are trusted (page id >= num_pages or a
+ *     position >= max_position is undefined behaviour).
+ *   - Pool layout (frozen):  k_cache, v_cache : [num_pages][num_kv_heads][page_size][head_dim] bf16.
+ *     K holds the projection output with NO rotary applied; token t of a page sits at logical position
+ *     page_logical_pos + t.
+ *   - Sequence model: request r has seq_lens[r] tokens; token s lives in table slot s / page_size at
+ *     in-page offset s % page_size.  The query tokens of a call are the LAST tokens of the sequence and
+ *     are already in the cache (lazy_cache_write first, same stream).  Causal mask is by sequence index
+ *     (key s visible to the query with index sq iff s <= sq); positions feed RoPE only.
+ *   - GQA: q head hq reads kv head hq / (num_q_heads / num_kv_heads).
+ *   - Scale 1/sqrt(head_dim); theta_j = rope_theta^(-2j/head_dim), j < head_dim/2; pair (j, j+head_dim/2).
+ */
+#ifndef LAZY_ATTN_H_
+#define LAZY_ATTN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lazy_handle lazy_handle;
+
+typedef struct lazy_config {
+  int32_t num_q_heads;       /* Hq                                                              */
+  int32_t num_kv_heads;      /* Hkv; Hq % Hkv == 0, group = Hq/Hkv <= 8; Hkv in {1,2,4} or a multiple of 8 */
+  int32_t head_dim;          /* D in {64, 128}                                                  */
+  int32_t page_size;         /* 16                                                              */
+  int32_t num_pages;         /* physical pool size (pages)                                      */
+  int32_t max_position;      /* logical positions lie in [0, max_position)                      */
+  int32_t max_reqs;          /* upper bound on num_reqs of any call                             */
+  int32_t max_pages_per_req; /* row stride (in entries) of block_table and page_logical_pos     */
+  double  rope_theta;        /* 1e4, 5e5, 1e6 ...                                               */
+  int32_t rope_style;        /* 0 = half-split (the only style)                                 */
+  int32_t dtype;             /* 0 = bf16 (the only dtype)                                       */
+  int32_t flags;             /* LAZY_FLAG_* (0 for production)                                  */
+  int32_t reserved;
+} lazy_config;
+
+/* flags: debugging aids, never set by bench.py */
+#define LAZY_FLAG_ROWWISE_KERNELS 1  /* run the simple one-row-per-CTA CUDA kernels for prefill and decode */
+
+#define LAZY_OK               0
+#define LAZY_ERR_INVALID     -1  /* null / misaligned pointer, negative count, num_reqs > max_reqs ...     */
+#define LAZY_ERR_UNSUPPORTED -2  /* head_dim, page_size, head grouping, dtype or rope_style not supported  */
+#define LAZY_ERR_WORKSPACE   -3  /* workspace too small or misaligned                                      */
+#define LAZY_ERR_CUDA        -4  /* CUDA error at launch (cudaGetLastError)                                */
+
+/* Bytes of device workspace lazy_create needs for `cfg` (RoPE cos/sin table built from fp64 angles --
+ * PAPER.md L138/L173 "loaded from a table", L455 stateless absolute-index rotation -- plus split-KV
+ * partials, PAPER-external: north_star "split-KV flash-decoding ... and a combine pass").
+ * Returns 0 if cfg is NULL or unsupported. */
+size_t lazy_workspace_bytes(const lazy_config* cfg);
+
+/* Creates a handle (host memory) over caller-owned device `workspace` (256-byte aligned, at least
+ * lazy_workspace_bytes(cfg)); enqueues the table build on `stream`.  The workspace must stay alive and
+ * untouched by the caller until lazy_destroy.  One host thread at a time per handle. */
+int lazy_create(const lazy_config* cfg, void* workspace, size_t workspace_bytes, void* stream,
+                lazy_handle** out);
+void lazy_destroy(lazy_handle* h);
+
+/* a0. Store un-rotated K and V rows of new tokens into physical pages ("purely
+ * content-based keys and values"; L188).  Pure data movement, bit exact.
+ *   k_new, v_new : [num_tokens][Hkv][D] bf16     slot_mapping : [num_tokens] int64,
+ *   slot = page*page_size + offset, slot < 0 skips the token.  num_tokens == 0 -> no launch. */
+int lazy_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
+                     int32_t num_tokens, void* k_cache, void* v_cache, void* stream);
+
+/* Prefill: a chunk of n_q[r] = cu_q_lens[r+1]-cu_q_lens[r] query tokens per request (the last n_q[r]
+ * tokens of its sequence) attends to all earlier tokens (shared document pages, at the logical
+ * positions this request gives them) and causally to itself (Fig. 5 phase 2; K rotated
+ * once per tile, L164-173).  Block-local document prefill is the case n_q == seq_len.
+ *   q, out           : [total_q][Hq][D] bf16 (q un-rotated)
+ *   block_table      : [num_reqs][max_pages_per_req] int32 physical page per slot
+ *   page_logical_pos : same shape, logical position of token 0 of that page
+ *   seq_lens         : [num_reqs] int32 KV length INCLUDING the chunk;  cu_q_lens : [num_reqs+1] int32
+ *   max_q_len        : host upper bound on n_q[r] (sizes the grid)
+ * Rows of a request with seq_len == 0 are written as zeros.  num_reqs == 0 or total_q == 0 -> no launch. */
+int lazy_attn_prefill(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                      const int32_t* block_table, const int32_t* page_logical_pos,
+                      const int32_t* seq_lens, const int32_t* cu_q_lens,
+                      int32_t num_reqs, int32_t total_q, int32_t max_q_len, void* out, void* stream);
+
+/* Decode: one query per request (its last token) over the whole sequence (Fig. 3c;
+ * T_decode ~ 2LD/B, L204-209).  Split-KV flash-decoding with an in-kernel combine.
+ *   q, out : [num_reqs][Hq][D] bf16.  Other arguments as for prefill. */
+int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                     const int32_t* block_table, const int32_t* page_logical_pos,
+                     const int32_t* seq_lens, int32_t num_reqs, void* out, void* stream);
+
+/* Static description of a status code (host string, never NULL). */
+const char* lazy_status_string(int status);
+
+/* Introspection for tests and bench.py: number of kernel launches this handle has enqueued so far. */
+int64_t lazy_launch_count(const lazy_handle* h);
+
+/* End-to-end convenience call over HOST buffers (the e2e leg of bench.py): one serving step =
+ * optional lazy_cache_write of the step's new tokens + one attention call, with every per-step input
+ * (q, k_new, v_new, slot_mapping, block_table, page_logical_pos, seq_lens, cu_q_lens) copied host->device
+ * into the caller's device staging area and `out` copied device->host, all enqueued on `stream`
+ * (cudaMemcpyAsync; host buffers should be pinned).  The KV pool stays resident on the device -- that is
+ * the point of the method (cached documents are served from GPU memory).
+ * Pointers named h_* are HOST, d_* DEVICE.  The tables are [num_reqs][max_pages_per_req] int32.
+ * The call returns after enqueueing; synchronise the stream before reading h_out. */
+typedef struct lazy_host_step_args {
+  int32_t kind;              /* 0 = decode, 1 = prefill                                   */
+  int32_t num_reqs;
+  int32_t total_q;           /* decode: == num_reqs                                       */
+  int32_t max_q_len;         /* decode: 1                                                 */
+  int32_t num_new_tokens;    /* rows of h_k_new/h_v_new/h_slot_mapping; 0 = no cache write */
+  int32_t reserved;
+  const void* h_q;           /* [total_q][Hq][D] bf16                                     */
+  const void* h_k_new;       /* [num_new_tokens][Hkv][D] bf16 or NULL                     */
+  const void* h_v_new;
+  const int64_t* h_slot_mapping;
+  const int32_t* h_block_table;
+  const int32_t* h_page_logical_pos;
+  const int32_t* h_seq_lens;
+  const int32_t* h_cu_q_lens; /* prefill only                                             */
+  void* h_out;               /* [total_q][Hq][D] bf16                                     */
+  void* d_k_cache;
+  void* d_v_cache;
+  void* d_staging;           /* device scratch, 256-byte aligned                          */
+  size_t staging_bytes;      /* >= lazy_host_step_staging_bytes(...)                      */
+} lazy_host_step_args;
+
+size_t lazy_host_step_staging_bytes(const lazy_handle* h, int32_t num_reqs, int32_t total_q,
+                                    int32_t num_new_tokens);
+int lazy_host_step(lazy_handle* h, const lazy_host_step_args* a, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LAZY_ATTN_H_ */

@@ -1,0 +1,187 @@
+"""Thin ctypes binding over liblazyattn.so (include/lazy_attn.h) -- argument marshalling only.
+
+Every function has the name and argument order of its C counterpart; tensors are torch CUDA tensors whose
+`data_ptr()` is handed through, the stream is `torch.cuda.current_stream().cuda_stream` unless given.
+Nothing here computes: if the CUDA library is missing the import of `lib()` raises (there is no fallback).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "csrc", "liblazyattn.so")
+
+LAZY_OK, LAZY_ERR_INVALID, LAZY_ERR_UNSUPPORTED, LAZY_ERR_WORKSPACE, LAZY_ERR_CUDA = 0, -1, -2, -3, -4
+LAZY_FLAG_ROWWISE_KERNELS = 1
+
+EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
+           "lazy_attn_decode", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step"]
+
+
+class LazyConfig(ctypes.Structure):
+    _fields_ = [("num_q_heads", ctypes.c_int32), ("num_kv_heads", ctypes.c_int32), ("head_dim", ctypes.c_int32),
+                ("page_size", ctypes.c_int32), ("num_pages", ctypes.c_int32), ("max_position", ctypes.c_int32),
+                ("max_reqs", ctypes.c_int32), ("max_pages_per_req", ctypes.c_int32),
+                ("rope_theta", ctypes.c_double), ("rope_style", ctypes.c_int32), ("dtype", ctypes.c_int32),
+                ("flags", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def lib() -> ctypes.CDLL:
+    """Loads the CUDA library; raises if it has not been built (python -m paper_2606_04302_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_2606_04302_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+        L.lazy_workspace_bytes.restype = ctypes.c_size_t
+        L.lazy_workspace_bytes.argtypes = [ctypes.POINTER(LazyConfig)]
+        L.lazy_create.restype = ctypes.c_int
+        L.lazy_create.argtypes = [ctypes.POINTER(LazyConfig), vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
+        L.lazy_destroy.restype = None
+        L.lazy_destroy.argtypes = [vp]
+        L.lazy_cache_write.restype = ctypes.c_int
+        L.lazy_cache_write.argtypes = [vp, vp, vp, vp, i32, vp, vp, vp]
+        L.lazy_attn_prefill.restype = ctypes.c_int
+        L.lazy_attn_prefill.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, vp]
+        L.lazy_attn_decode.restype = ctypes.c_int
+        L.lazy_attn_decode.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, vp, vp]
+        L.lazy_status_string.restype = ctypes.c_char_p
+        L.lazy_status_string.argtypes = [ctypes.c_int]
+        L.lazy_launch_count.restype = i64
+        L.lazy_launch_count.argtypes = [vp]
+        L.lazy_host_step_staging_bytes.restype = ctypes.c_size_t
+        L.lazy_host_step_staging_bytes.argtypes = [vp, i32, i32, i32]
+        L.lazy_host_step.restype = ctypes.c_int
+        L.lazy_host_step.argtypes = [vp, ctypes.POINTER(HostStep), vp]
+        _lib = L
+    return _lib
+
+
+class LazyError(RuntimeError):
+    def __init__(self, call: str, status: int):
+        super().__init__(f"{call} failed: {status} ({lazy_status_string(status)})")
+        self.status = status
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+def lazy_status_string(status: int) -> str:
+    return lib().lazy_status_string(int(status)).decode()
+
+
+def lazy_workspace_bytes(cfg: LazyConfig) -> int:
+    return int(lib().lazy_workspace_bytes(ctypes.byref(cfg)))
+
+
+class LazyHandle:
+    """Owns the torch workspace tensor and the C handle (lazy_create / lazy_destroy)."""
+
+    def __init__(self, cfg: LazyConfig, device="cuda", stream=None):
+        import torch
+        n = lazy_workspace_bytes(cfg)
+        if n == 0:
+            raise LazyError("lazy_workspace_bytes", LAZY_ERR_UNSUPPORTED)
+        self.cfg = cfg
+        self.workspace = torch.empty(n + 256, dtype=torch.uint8, device=device)
+        base = (self.workspace.data_ptr() + 255) // 256 * 256
+        out = ctypes.c_void_p()
+        rc = lib().lazy_create(ctypes.byref(cfg), base, n, _stream(stream), ctypes.byref(out))
+        if rc != 0:
+            raise LazyError("lazy_create", rc)
+        self._h = out
+
+    @property
+    def ptr(self):
+        return self._h
+
+    def launch_count(self) -> int:
+        return int(lib().lazy_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().lazy_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def lazy_create(num_q_heads: int, num_kv_heads: int, head_dim: int, *, num_pages: int, max_position: int,
+                max_reqs: int, max_pages_per_req: int, rope_theta: float, page_size: int = 16, flags: int = 0,
+                device="cuda", stream=None) -> LazyHandle:
+    cfg = LazyConfig(num_q_heads, num_kv_heads, head_dim, page_size, num_pages, max_position, max_reqs,
+                     max_pages_per_req, float(rope_theta), 0, 0, flags, 0)
+    return LazyHandle(cfg, device=device, stream=stream)
+
+
+def lazy_destroy(h: LazyHandle) -> None:
+    h.close()
+
+
+def lazy_cache_write(h: LazyHandle, k_new, v_new, slot_mapping, k_cache, v_cache, stream=None) -> None:
+    n = 0 if k_new is None else int(k_new.shape[0])
+    rc = lib().lazy_cache_write(h.ptr, _ptr(k_new), _ptr(v_new), _ptr(slot_mapping), n, _ptr(k_cache),
+                                _ptr(v_cache), _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_cache_write", rc)
+
+
+def lazy_attn_prefill(h: LazyHandle, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, cu_q_lens,
+                      max_q_len: int, out, stream=None) -> None:
+    num_reqs = int(seq_lens.shape[0])
+    total_q = int(q.shape[0])
+    rc = lib().lazy_attn_prefill(h.ptr, _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_table),
+                                 _ptr(page_logical_pos), _ptr(seq_lens), _ptr(cu_q_lens), num_reqs, total_q,
+                                 int(max_q_len), _ptr(out), _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_attn_prefill", rc)
+
+
+def lazy_attn_decode(h: LazyHandle, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, out,
+                     stream=None) -> None:
+    num_reqs = int(seq_lens.shape[0])
+    rc = lib().lazy_attn_decode(h.ptr, _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_table),
+                                _ptr(page_logical_pos), _ptr(seq_lens), num_reqs, _ptr(out), _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_attn_decode", rc)
+
+
+class HostStep(ctypes.Structure):
+    """Mirror of lazy_host_step_args (include/lazy_attn.h): one serving step with HOST buffers."""
+    _fields_ = [("kind", ctypes.c_int32), ("num_reqs", ctypes.c_int32), ("total_q", ctypes.c_int32),
+                ("max_q_len", ctypes.c_int32), ("num_new_tokens", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("h_q", ctypes.c_void_p), ("h_k_new", ctypes.c_void_p), ("h_v_new", ctypes.c_void_p),
+                ("h_slot_mapping", ctypes.c_void_p), ("h_block_table", ctypes.c_void_p),
+                ("h_page_logical_pos", ctypes.c_void_p), ("h_seq_lens", ctypes.c_void_p),
+                ("h_cu_q_lens", ctypes.c_void_p), ("h_out", ctypes.c_void_p),
+                ("d_k_cache", ctypes.c_void_p), ("d_v_cache", ctypes.c_void_p),
+                ("d_staging", ctypes.c_void_p), ("staging_bytes", ctypes.c_size_t)]
+
+
+def lazy_host_step_staging_bytes(h: LazyHandle, num_reqs: int, total_q: int, num_new_tokens: int) -> int:
+    return int(lib().lazy_host_step_staging_bytes(h.ptr, num_reqs, total_q, num_new_tokens))
+
+
+def lazy_host_step(h: LazyHandle, args: HostStep, stream=None) -> None:
+    rc = lib().lazy_host_step(h.ptr, ctypes.byref(args), _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_host_step", rc)

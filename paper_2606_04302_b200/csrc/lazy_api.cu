@@ -1,0 +1,275 @@
+// lazy_api.cu -- host side of the C ABI (include/lazy_attn.h): argument checks, workspace carving,
+// handle management and dispatch to the kernel launchers.  No torch types, no allocation per call.
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <cmath>
+#include <new>
+
+#include "lazy_internal.h"
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+bool config_supported(const lazy_config* c) {
+  if (c->head_dim != 64 && c->head_dim != 128) return false;
+  if (c->page_size != lazy::kPageSize) return false;
+  if (c->num_q_heads <= 0 || c->num_kv_heads <= 0) return false;
+  if (c->num_q_heads % c->num_kv_heads != 0) return false;
+  if (c->num_q_heads / c->num_kv_heads > 8) return false;
+  int hkv = c->num_kv_heads;
+  if (!(hkv == 1 || hkv == 2 || hkv == 4 || hkv % 8 == 0)) return false;
+  if (c->dtype != 0 || c->rope_style != 0) return false;
+  return true;
+}
+
+bool config_valid(const lazy_config* c) {
+  return c->num_pages > 0 && c->max_position > 0 && c->max_reqs > 0 && c->max_pages_per_req > 0 &&
+         c->rope_theta > 0.0;
+}
+
+struct Layout {
+  size_t cs, part_o, part_ml, req_counter, sched, total;
+};
+
+Layout workspace_layout(const lazy_config* c) {
+  Layout l{};
+  size_t off = 0;
+  size_t parts = (size_t)c->max_reqs + lazy::kMaxDecodeCtas;
+  l.cs = off;          off = align_up(off + (size_t)c->max_position * (c->head_dim / 2) * sizeof(float2), 256);
+  l.part_o = off;      off = align_up(off + parts * c->num_q_heads * c->head_dim * sizeof(float), 256);
+  l.part_ml = off;     off = align_up(off + parts * c->num_q_heads * sizeof(float2), 256);
+  l.req_counter = off; off = align_up(off + (size_t)c->max_reqs * sizeof(int), 256);
+  l.sched = off;       off = align_up(off + 1024 * sizeof(int), 256);
+  l.total = off;
+  return l;
+}
+
+inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+}  // namespace
+
+extern "C" {
+
+size_t lazy_workspace_bytes(const lazy_config* cfg) {
+  if (!cfg || !config_valid(cfg) || !config_supported(cfg)) return 0;
+  return workspace_layout(cfg).total;
+}
+
+int lazy_create(const lazy_config* cfg, void* workspace, size_t workspace_bytes, void* stream,
+                lazy_handle** out) {
+  if (!cfg || !out) return LAZY_ERR_INVALID;
+  *out = nullptr;
+  if (!config_valid(cfg)) return LAZY_ERR_INVALID;
+  if (!config_supported(cfg)) return LAZY_ERR_UNSUPPORTED;
+  Layout l = workspace_layout(cfg);
+  if (!workspace || (reinterpret_cast<uintptr_t>(workspace) & 255u) != 0 || workspace_bytes < l.total)
+    return LAZY_ERR_WORKSPACE;
+
+  lazy_handle* h = new (std::nothrow) lazy_handle();
+  if (!h) return LAZY_ERR_INVALID;
+  std::memset(h, 0, sizeof(*h));
+  h->cfg = *cfg;
+  h->shape.Hq = cfg->num_q_heads;
+  h->shape.Hkv = cfg->num_kv_heads;
+  h->shape.D = cfg->head_dim;
+  h->shape.group = cfg->num_q_heads / cfg->num_kv_heads;
+  h->shape.table_stride = cfg->max_pages_per_req;
+  h->shape.max_position = cfg->max_position;
+  h->shape.scale_log2 = (float)(1.4426950408889634 / std::sqrt((double)cfg->head_dim));
+  char* base = static_cast<char*>(workspace);
+  h->ws.cs = reinterpret_cast<float2*>(base + l.cs);
+  h->ws.part_o = reinterpret_cast<float*>(base + l.part_o);
+  h->ws.part_ml = reinterpret_cast<float2*>(base + l.part_ml);
+  h->ws.req_counter = reinterpret_cast<int*>(base + l.req_counter);
+  h->ws.sched = reinterpret_cast<int*>(base + l.sched);
+
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    delete h;
+    return LAZY_ERR_CUDA;
+  }
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (cudaMemsetAsync(h->ws.req_counter, 0, (size_t)cfg->max_reqs * sizeof(int), s) != cudaSuccess ||
+      cudaMemsetAsync(h->ws.sched, 0, 1024 * sizeof(int), s) != cudaSuccess) {
+    delete h;
+    return LAZY_ERR_CUDA;
+  }
+  int n = lazy::launch_build_tables(h, s);
+  if (n < 0) { delete h; return n; }
+  h->launches += n;
+  *out = h;
+  return LAZY_OK;
+}
+
+void lazy_destroy(lazy_handle* h) { delete h; }
+
+int lazy_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
+                     int32_t num_tokens, void* k_cache, void* v_cache, void* stream) {
+  if (!h || num_tokens < 0) return LAZY_ERR_INVALID;
+  if (num_tokens == 0) return LAZY_OK;
+  if (!k_new || !v_new || !slot_mapping || !k_cache || !v_cache) return LAZY_ERR_INVALID;
+  if (misaligned(k_new) || misaligned(v_new) || misaligned(k_cache) || misaligned(v_cache) ||
+      (reinterpret_cast<uintptr_t>(slot_mapping) & 7u))
+    return LAZY_ERR_INVALID;
+  int n = lazy::launch_cache_write(h, k_new, v_new, slot_mapping, num_tokens, k_cache, v_cache,
+                                   static_cast<cudaStream_t>(stream));
+  if (n < 0) return n;
+  h->launches += n;
+  return LAZY_OK;
+}
+
+static int check_attn_args(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                           const int32_t* block_table, const int32_t* page_logical_pos,
+                           const int32_t* seq_lens, int32_t num_reqs, void* out) {
+  if (!h || num_reqs < 0) return LAZY_ERR_INVALID;
+  if (num_reqs > h->cfg.max_reqs) return LAZY_ERR_INVALID;
+  if (num_reqs == 0) return LAZY_OK;
+  if (!q || !k_cache || !v_cache || !block_table || !page_logical_pos || !seq_lens || !out)
+    return LAZY_ERR_INVALID;
+  if (misaligned(q) || misaligned(k_cache) || misaligned(v_cache) || misaligned(out) ||
+      (reinterpret_cast<uintptr_t>(block_table) & 3u) || (reinterpret_cast<uintptr_t>(page_logical_pos) & 3u) ||
+      (reinterpret_cast<uintptr_t>(seq_lens) & 3u))
+    return LAZY_ERR_INVALID;
+  return LAZY_OK;
+}
+
+int lazy_attn_prefill(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                      const int32_t* block_table, const int32_t* page_logical_pos,
+                      const int32_t* seq_lens, const int32_t* cu_q_lens,
+                      int32_t num_reqs, int32_t total_q, int32_t max_q_len, void* out, void* stream) {
+  int rc = check_attn_args(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, num_reqs, out);
+  if (rc != LAZY_OK) return rc;
+  if (total_q < 0 || max_q_len < 0) return LAZY_ERR_INVALID;
+  if (num_reqs == 0 || total_q == 0) return LAZY_OK;
+  if (!cu_q_lens || (reinterpret_cast<uintptr_t>(cu_q_lens) & 3u) || max_q_len == 0) return LAZY_ERR_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  int n;
+  if (h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS)
+    n = lazy::launch_rowwise(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, cu_q_lens,
+                             num_reqs, total_q, max_q_len, out, s);
+  else
+    n = lazy::launch_prefill(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, cu_q_lens,
+                             num_reqs, total_q, max_q_len, out, s);
+  if (n < 0) return n;
+  h->launches += n;
+  return LAZY_OK;
+}
+
+int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                     const int32_t* block_table, const int32_t* page_logical_pos,
+                     const int32_t* seq_lens, int32_t num_reqs, void* out, void* stream) {
+  int rc = check_attn_args(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, num_reqs, out);
+  if (rc != LAZY_OK) return rc;
+  if (num_reqs == 0) return LAZY_OK;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  int n;
+  if (h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS)
+    n = lazy::launch_rowwise(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, nullptr,
+                             num_reqs, num_reqs, 1, out, s);
+  else
+    n = lazy::launch_decode(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, num_reqs, out, s);
+  if (n < 0) return n;
+  h->launches += n;
+  return LAZY_OK;
+}
+
+const char* lazy_status_string(int status) {
+  switch (status) {
+    case LAZY_OK: return "ok";
+    case LAZY_ERR_INVALID: return "invalid argument";
+    case LAZY_ERR_UNSUPPORTED: return "unsupported configuration";
+    case LAZY_ERR_WORKSPACE: return "workspace too small or misaligned";
+    case LAZY_ERR_CUDA: return "CUDA error at launch";
+    default: return "unknown status";
+  }
+}
+
+int64_t lazy_launch_count(const lazy_handle* h) { return h ? h->launches : 0; }
+
+}  // extern "C"
+
+namespace {
+struct StagePlan {
+  size_t q, k_new, v_new, slots, bt, pp, sl, cu, out, total;
+  size_t q_bytes, kv_bytes, slots_bytes, table_bytes, sl_bytes, cu_bytes;
+};
+StagePlan stage_plan(const lazy_handle* h, int num_reqs, int total_q, int num_new) {
+  StagePlan p{};
+  const lazy_config& c = h->cfg;
+  p.q_bytes = (size_t)total_q * c.num_q_heads * c.head_dim * 2;
+  p.kv_bytes = (size_t)num_new * c.num_kv_heads * c.head_dim * 2;
+  p.slots_bytes = (size_t)num_new * sizeof(int64_t);
+  p.table_bytes = (size_t)num_reqs * c.max_pages_per_req * sizeof(int32_t);
+  p.sl_bytes = (size_t)num_reqs * sizeof(int32_t);
+  p.cu_bytes = (size_t)(num_reqs + 1) * sizeof(int32_t);
+  size_t off = 0;
+  p.q = off;     off = align_up(off + p.q_bytes, 256);
+  p.k_new = off; off = align_up(off + p.kv_bytes, 256);
+  p.v_new = off; off = align_up(off + p.kv_bytes, 256);
+  p.slots = off; off = align_up(off + p.slots_bytes, 256);
+  p.bt = off;    off = align_up(off + p.table_bytes, 256);
+  p.pp = off;    off = align_up(off + p.table_bytes, 256);
+  p.sl = off;    off = align_up(off + p.sl_bytes, 256);
+  p.cu = off;    off = align_up(off + p.cu_bytes, 256);
+  p.out = off;   off = align_up(off + p.q_bytes, 256);
+  p.total = off;
+  return p;
+}
+}  // namespace
+
+extern "C" size_t lazy_host_step_staging_bytes(const lazy_handle* h, int32_t num_reqs, int32_t total_q,
+                                               int32_t num_new_tokens) {
+  if (!h || num_reqs < 0 || total_q < 0 || num_new_tokens < 0) return 0;
+  return stage_plan(h, num_reqs, total_q, num_new_tokens).total;
+}
+
+extern "C" int lazy_host_step(lazy_handle* h, const lazy_host_step_args* a, void* stream) {
+  if (!h || !a) return LAZY_ERR_INVALID;
+  if (a->num_reqs < 0 || a->total_q < 0 || a->num_new_tokens < 0) return LAZY_ERR_INVALID;
+  if (a->num_reqs == 0 || a->total_q == 0) return LAZY_OK;
+  if (!a->h_q || !a->h_block_table || !a->h_page_logical_pos || !a->h_seq_lens || !a->h_out ||
+      !a->d_k_cache || !a->d_v_cache || !a->d_staging)
+    return LAZY_ERR_INVALID;
+  if (a->kind == 1 && !a->h_cu_q_lens) return LAZY_ERR_INVALID;
+  if (a->num_new_tokens > 0 && (!a->h_k_new || !a->h_v_new || !a->h_slot_mapping)) return LAZY_ERR_INVALID;
+  StagePlan p = stage_plan(h, a->num_reqs, a->total_q, a->num_new_tokens);
+  if ((reinterpret_cast<uintptr_t>(a->d_staging) & 255u) || a->staging_bytes < p.total) return LAZY_ERR_WORKSPACE;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  char* d = static_cast<char*>(a->d_staging);
+  bool ok = true;
+  auto h2d = [&](size_t off, const void* src, size_t n) {
+    if (n) ok = ok && cudaMemcpyAsync(d + off, src, n, cudaMemcpyHostToDevice, s) == cudaSuccess;
+  };
+  h2d(p.q, a->h_q, p.q_bytes);
+  if (a->num_new_tokens > 0) {
+    h2d(p.k_new, a->h_k_new, p.kv_bytes);
+    h2d(p.v_new, a->h_v_new, p.kv_bytes);
+    h2d(p.slots, a->h_slot_mapping, p.slots_bytes);
+  }
+  h2d(p.bt, a->h_block_table, p.table_bytes);
+  h2d(p.pp, a->h_page_logical_pos, p.table_bytes);
+  h2d(p.sl, a->h_seq_lens, p.sl_bytes);
+  if (a->kind == 1) h2d(p.cu, a->h_cu_q_lens, p.cu_bytes);
+  if (!ok) return LAZY_ERR_CUDA;
+  int rc = LAZY_OK;
+  if (a->num_new_tokens > 0)
+    rc = lazy_cache_write(h, d + p.k_new, d + p.v_new, reinterpret_cast<const int64_t*>(d + p.slots),
+                          a->num_new_tokens, a->d_k_cache, a->d_v_cache, stream);
+  if (rc != LAZY_OK) return rc;
+  if (a->kind == 1)
+    rc = lazy_attn_prefill(h, d + p.q, a->d_k_cache, a->d_v_cache, reinterpret_cast<const int32_t*>(d + p.bt),
+                           reinterpret_cast<const int32_t*>(d + p.pp), reinterpret_cast<const int32_t*>(d + p.sl),
+                           reinterpret_cast<const int32_t*>(d + p.cu), a->num_reqs, a->total_q, a->max_q_len,
+                           d + p.out, stream);
+  else
+    rc = lazy_attn_decode(h, d + p.q, a->d_k_cache, a->d_v_cache, reinterpret_cast<const int32_t*>(d + p.bt),
+                          reinterpret_cast<const int32_t*>(d + p.pp), reinterpret_cast<const int32_t*>(d + p.sl),
+                          a->num_reqs, d + p.out, stream);
+  if (rc != LAZY_OK) return rc;
+  if (cudaMemcpyAsync(a->h_out, d + p.out, p.q_bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess)
+    return LAZY_ERR_CUDA;
+  return LAZY_OK;
+}

@@ -1,0 +1,71 @@
+// lazy_internal.h -- shared by the translation units of liblazyattn.so (never by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+#include <stdint.h>
+#include <stddef.h>
+
+#include "lazy_attn.h"
+
+namespace lazy {
+
+constexpr int kPageSize = 16;
+constexpr int kMaxDecodeCtas = 1024;   // upper bound on the decode grid (sizes the partial buffers)
+
+// Device-side views the kernels take by value.
+struct Shape {
+  int Hq, Hkv, D, group;
+  int table_stride;      // max_pages_per_req
+  int max_position;
+  float scale_log2;      // log2(e) / sqrt(D)
+};
+
+struct Workspace {
+  float2* cs;            // [max_position][D/2] (cos, sin) of pos * theta_j, built from fp64 angles
+  float*  part_o;        // [max_reqs + kMaxDecodeCtas][Hq][D] fp32 un-normalised partial outputs
+  float2* part_ml;       // [max_reqs + kMaxDecodeCtas][Hq] (running max in log2 units, sum)
+  int*    req_counter;   // [max_reqs] arrival counters for the in-kernel combine (self-resetting)
+  int*    sched;         // small scratch for device-side scheduling
+};
+
+}  // namespace lazy
+
+struct lazy_handle {
+  lazy_config cfg;
+  lazy::Shape shape;
+  lazy::Workspace ws;
+  int num_sms;
+  int64_t launches;
+  // cached TMA descriptors (128 bytes each), keyed by the pool pointer they were encoded for
+  alignas(64) unsigned char tmap_k[128];
+  alignas(64) unsigned char tmap_v[128];
+  const void* tmap_k_ptr;
+  const void* tmap_v_ptr;
+  alignas(64) unsigned char tmap_pk[128];
+  alignas(64) unsigned char tmap_pv[128];
+  alignas(64) unsigned char tmap_pq[128];
+  const void* tmap_pk_ptr;
+  const void* tmap_pv_ptr;
+  const void* tmap_pq_ptr;
+  int tmap_pq_rows;
+};
+
+namespace lazy {
+
+// Each launcher enqueues on `stream` and returns the number of kernels launched (<0: LAZY_ERR_*).
+int launch_build_tables(lazy_handle* h, cudaStream_t stream);
+int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
+                       int num_tokens, void* k_cache, void* v_cache, cudaStream_t stream);
+int launch_rowwise(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                   const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
+                   const int32_t* cu_q_lens, int num_reqs, int total_q, int max_q_len, void* out,
+                   cudaStream_t stream);
+int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                  const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
+                  int num_reqs, void* out, cudaStream_t stream);
+int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                   const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
+                   const int32_t* cu_q_lens, int num_reqs, int total_q, int max_q_len, void* out,
+                   cudaStream_t stream);
+
+}  // namespace lazy

@@ -1,0 +1,55 @@
+"""Helpers shared by the -m gpu parity tests: run a LazyBatch through the CUDA path (C ABI) and through the
+fp64 oracle on the same seeded inputs, and compare.  Tolerances: BASELINE.json north_star (max abs <= 2e-2,
+mean abs <= 2e-3 on outputs) plus the tighter self-imposed normalised gates of DESIGN.md "Tolerances"."""
+from __future__ import annotations
+
+import numpy as np
+import torch
+
+from oracle import oracle as O
+from paper_2606_04302_b200.runner import DeviceBatch
+
+MAX_ABS, MEAN_ABS = 2e-2, 2e-3          # contract (north_star)
+REL_RMS, REL_MAX = 1.5e-2, 5e-2         # self-imposed: RMS(err)/RMS(ref), max|err| / max|ref|
+
+
+def compare(got: torch.Tensor, ref: np.ndarray, what: str = "", rows=None):
+    g = got.detach().double().cpu().numpy()
+    if rows is not None:
+        g, ref = g[rows], ref[rows]
+    assert np.isfinite(g).all(), f"{what}: non-finite GPU output"
+    err = np.abs(g - ref)
+    rms_ref = float(np.sqrt((ref ** 2).mean()))
+    stats = dict(max_abs=float(err.max()), mean_abs=float(err.mean()),
+                 rel_rms=float(np.sqrt((err ** 2).mean()) / max(rms_ref, 1e-30)),
+                 rel_max=float(err.max() / max(np.abs(ref).max(), 1e-30)))
+    assert stats["max_abs"] <= MAX_ABS and stats["mean_abs"] <= MEAN_ABS, f"{what}: contract violated {stats}"
+    assert stats["rel_rms"] <= REL_RMS and stats["rel_max"] <= REL_MAX, f"{what}: normalised gate violated {stats}"
+    return stats
+
+
+def run_and_compare(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, max_position=None):
+    """Runs every step on the GPU and on the oracle (oracle pools are separate CPU copies).  With
+    sample_rows > 0 the oracle computes only that many seeded query rows per attention step."""
+    dev = DeviceBatch(batch, flags=flags, max_position=max_position)
+    k_ref, v_ref = batch.k_pool.clone(), batch.v_pool.clone()
+    rng = np.random.default_rng(seed)
+    all_stats = []
+    try:
+        for si, step in enumerate(batch.steps):
+            got = dev.run_step(step)
+            torch.cuda.synchronize()
+            sel = rows = None
+            if step.q is not None and sample_rows and step.q.shape[0] > sample_rows:
+                rows = np.sort(rng.choice(step.q.shape[0], size=sample_rows, replace=False))
+                sel = np.zeros(step.q.shape[0], dtype=np.uint8)
+                sel[rows] = 1
+            ref = O.run_step(batch, step, k_ref, v_ref, row_select=sel)
+            # pools must agree bit for bit after the step's cache write, and stay so after the read path
+            assert torch.equal(dev.k_pool.cpu().view(torch.int16), k_ref.view(torch.int16)), f"step {si}: K pool"
+            assert torch.equal(dev.v_pool.cpu().view(torch.int16), v_ref.view(torch.int16)), f"step {si}: V pool"
+            if got is not None:
+                all_stats.append(compare(got, ref, f"{batch.name} step {si} ({step.kind})", rows=rows))
+    finally:
+        dev.close()
+    return all_stats

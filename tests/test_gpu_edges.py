@@ -1,0 +1,191 @@
+"""-m gpu edge cases: empty and ragged inputs, partial pages, repeated pages, position gaps, skipped slots,
+argument errors, and the read-only property of the read path."""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_04302_b200 import binding as B
+from paper_2606_04302_b200 import workloads as W
+from paper_2606_04302_b200.runner import DeviceBatch
+
+pytestmark = pytest.mark.gpu
+FLAGS = [pytest.param(0, id="prod"), pytest.param(B.LAZY_FLAG_ROWWISE_KERNELS, id="rowwise")]
+
+
+def _custom(shape, seq_lens, q_lens, *, seed, repeat_pages=False, pos_gap=0, unaligned_pos=False, kind="prefill"):
+    """Hand-built batch: every request owns ceil(L/16) pages (or re-uses its first page repeatedly);
+    positions may have gaps and need not be multiples of 16."""
+    P = shape.page_size
+    gen = torch.Generator().manual_seed(seed)
+    rng = np.random.default_rng(seed)
+    R = len(seq_lens)
+    npages = [(L + P - 1) // P for L in seq_lens]
+    pmax = max(max(npages), 1)
+    total_pages = sum(npages) + 3
+    k_pool = W._randn_bf16(gen, (total_pages, shape.num_kv_heads, P, shape.head_dim))
+    v_pool = W._randn_bf16(gen, (total_pages, shape.num_kv_heads, P, shape.head_dim))
+    perm = rng.permutation(total_pages)
+    bt = np.zeros((R, pmax), dtype=np.int32)
+    pp = np.zeros((R, pmax), dtype=np.int32)
+    c = 0
+    for r in range(R):
+        ids = perm[c:c + npages[r]].copy()
+        c += npages[r]
+        if repeat_pages and npages[r] > 2:
+            ids[2::2] = ids[0]                      # the same physical page at several slots of one request
+        bt[r, :npages[r]] = ids
+        pos = P * np.arange(npages[r])
+        if pos_gap:
+            pos = pos + pos_gap * (np.arange(npages[r]) // 3)      # jump every 3 pages
+        if unaligned_pos:
+            pos = pos + 5
+        pp[r, :npages[r]] = pos
+    # poison the tail of every last page (tokens >= L must never be read into the result)
+    for r in range(R):
+        L = seq_lens[r]
+        if L % P and not repeat_pages:
+            k_pool[bt[r, npages[r] - 1], :, L % P:, :] = float("nan")
+            v_pool[bt[r, npages[r] - 1], :, L % P:, :] = float("nan")
+    tq = int(sum(q_lens))
+    q = W._randn_bf16(gen, (max(tq, 1), shape.num_q_heads, shape.head_dim))[:tq]
+    cu = np.concatenate([[0], np.cumsum(q_lens)]).astype(np.int32)
+    step = W.Step(kind=kind, q=q, seq_lens=torch.tensor(seq_lens, dtype=torch.int32),
+                  cu_q_lens=torch.from_numpy(cu))
+    return W.LazyBatch(name="custom", shape=shape, k_pool=k_pool, v_pool=v_pool,
+                       block_table=torch.from_numpy(bt), page_logical_pos=torch.from_numpy(pp), steps=[step])
+
+
+def _check(batch, flags=0):
+    from gpu_util import run_and_compare
+    return run_and_compare(batch, flags=flags)
+
+
+SH128 = W.LazyShape(32, 8, 128, 5.0e5)
+SH64 = W.LazyShape(4, 1, 64, 1.0e4)
+SH7 = W.LazyShape(28, 4, 128, 1.0e6)
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+@pytest.mark.parametrize("shape", [SH128, SH64, SH7], ids=["g4d128", "g4d64", "g7d128"])
+def test_ragged_decode(shape, flags):
+    seq = [1, 2, 15, 16, 17, 31, 33, 100, 257, 640, 1000, 3]
+    _check(_custom(shape, seq, [1] * len(seq), seed=11, kind="decode"), flags)
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+@pytest.mark.parametrize("shape", [SH128, SH64, SH7], ids=["g4d128", "g4d64", "g7d128"])
+def test_ragged_prefill(shape, flags):
+    seq = [5, 16, 200, 129, 300, 47, 1]
+    qls = [5, 3, 200, 1, 130, 47, 1]          # includes block-local (q_len == seq_len) and single rows
+    _check(_custom(shape, seq, qls, seed=12), flags)
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+def test_zero_length_requests(flags):
+    seq = [0, 40, 0]
+    b = _custom(SH128, seq, [1, 1, 1], seed=13, kind="decode")
+    dev = DeviceBatch(b, flags=flags)
+    out = dev.run_step(b.steps[0])
+    torch.cuda.synchronize()
+    assert (out[0] == 0).all() and (out[2] == 0).all() and out[1].float().abs().sum() > 0
+    dev.close()
+    _check(b, flags)
+    # prefill with an empty request in the middle (no query rows, seq_len 0)
+    _check(_custom(SH128, [33, 0, 20], [4, 0, 20], seed=14), flags)
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+def test_repeated_pages_gaps_and_unaligned_positions(flags):
+    _check(_custom(SH128, [200, 333], [1, 1], seed=15, repeat_pages=True, kind="decode"), flags)
+    _check(_custom(SH128, [200, 333], [8, 70], seed=16, repeat_pages=True, pos_gap=1000), flags)
+    _check(_custom(SH128, [77, 160], [1, 1], seed=17, pos_gap=4096, unaligned_pos=True, kind="decode"), flags)
+    _check(_custom(SH64, [77, 160], [30, 160], seed=18, pos_gap=512, unaligned_pos=True), flags)
+
+
+def test_one_page_two_positions_equals_two_copies():
+    """north_star check 4 / PAPER.md L37, L88: a page used at two slots == a byte-identical duplicate."""
+    b = _custom(SH128, [160], [1], seed=19, kind="decode")
+    bt = b.block_table.clone()
+    x, dup = int(bt[0, 1]), int(bt[0, 5])
+    shared = W.LazyBatch(name="s", shape=b.shape, k_pool=b.k_pool.clone(), v_pool=b.v_pool.clone(),
+                         block_table=bt.clone(), page_logical_pos=b.page_logical_pos, steps=b.steps)
+    shared.block_table[0, 5] = x                      # page x at slots 1 and 5
+    copied = W.LazyBatch(name="c", shape=b.shape, k_pool=b.k_pool.clone(), v_pool=b.v_pool.clone(),
+                         block_table=bt.clone(), page_logical_pos=b.page_logical_pos, steps=b.steps)
+    copied.k_pool[dup] = copied.k_pool[x]
+    copied.v_pool[dup] = copied.v_pool[x]
+    outs = []
+    for bb in (shared, copied):
+        dev = DeviceBatch(bb)
+        outs.append(dev.run_step(bb.steps[0]).float().cpu())
+        dev.close()
+    assert torch.equal(outs[0], outs[1])
+    _check(shared)
+
+
+def test_empty_calls_and_errors():
+    b = W.config1()
+    dev = DeviceBatch(b)
+    h = dev.handle
+    n0 = h.launch_count()
+    L = B.lib()
+    z = torch.zeros(16, dtype=torch.int32, device="cuda")
+    # zero-sized calls launch nothing and succeed
+    assert L.lazy_cache_write(h.ptr, None, None, None, 0, None, None, None) == 0
+    assert L.lazy_attn_decode(h.ptr, None, None, None, None, None, None, 0, None, None) == 0
+    assert L.lazy_attn_prefill(h.ptr, None, None, None, None, None, None, None, 0, 0, 0, None, None) == 0
+    assert h.launch_count() == n0
+    # errors: too many requests, null pointers, misaligned pointer
+    p = z.data_ptr()
+    assert L.lazy_attn_decode(h.ptr, p, p, p, p, p, p, 2, p, None) == B.LAZY_ERR_INVALID      # max_reqs = 1
+    assert L.lazy_attn_decode(h.ptr, None, p, p, p, p, p, 1, p, None) == B.LAZY_ERR_INVALID
+    assert L.lazy_attn_decode(h.ptr, p + 2, p, p, p, p, p, 1, p, None) == B.LAZY_ERR_INVALID
+    assert L.lazy_cache_write(h.ptr, p, p, p, -1, p, p, None) == B.LAZY_ERR_INVALID
+    assert h.launch_count() == n0
+    dev.close()
+
+
+def test_cache_write_skips_negative_slots_and_is_bit_exact():
+    from oracle import oracle as O
+    b = W.config5(scale=0.25)
+    step = b.steps[0]
+    slots = step.slot_mapping.clone()
+    slots[::7] = -1
+    s2 = W.Step(kind="write_only", k_new=step.k_new, v_new=step.v_new, slot_mapping=slots)
+    dev = DeviceBatch(b)
+    k_ref, v_ref = b.k_pool.clone(), b.v_pool.clone()
+    dev.write(s2)
+    torch.cuda.synchronize()
+    O.cache_write(s2.k_new, s2.v_new, slots.numpy(), k_ref, v_ref, 16)
+    assert torch.equal(dev.k_pool.cpu().view(torch.int16), k_ref.view(torch.int16))
+    assert torch.equal(dev.v_pool.cpu().view(torch.int16), v_ref.view(torch.int16))
+    dev.close()
+
+
+def test_host_step_matches_device_calls():
+    """lazy_host_step (HOST buffers, copies inside) == the device-pointer calls."""
+    b = W.config2(scale=0.1)
+    step = b.steps[-1]
+    dev = DeviceBatch(b)
+    dev.write(b.steps[0])
+    want = dev.run_step(step)
+    torch.cuda.synchronize()
+    dev2 = DeviceBatch(b)
+    dev2.write(b.steps[0])
+    pin = lambda t: t.contiguous().pin_memory()
+    hq, hk, hv, hs = pin(step.q), pin(step.k_new), pin(step.v_new), pin(step.slot_mapping)
+    hbt, hpp, hsl = pin(b.block_table), pin(b.page_logical_pos), pin(step.seq_lens)
+    hout = torch.empty_like(step.q).pin_memory()
+    R = step.seq_lens.shape[0]
+    nbytes = B.lazy_host_step_staging_bytes(dev2.handle, R, R, step.k_new.shape[0])
+    staging = torch.empty(nbytes + 256, dtype=torch.uint8, device="cuda")
+    base = (staging.data_ptr() + 255) // 256 * 256
+    a = B.HostStep(0, R, R, 1, step.k_new.shape[0], 0, hq.data_ptr(), hk.data_ptr(), hv.data_ptr(), hs.data_ptr(),
+                   hbt.data_ptr(), hpp.data_ptr(), hsl.data_ptr(), None, hout.data_ptr(),
+                   dev2.k_pool.data_ptr(), dev2.v_pool.data_ptr(), base, nbytes)
+    B.lazy_host_step(dev2.handle, a)
+    torch.cuda.synchronize()
+    assert torch.equal(hout.view(torch.int16), want.cpu().view(torch.int16))
+    dev.close(); dev2.close()
