@@ -8,6 +8,7 @@
 //    angle from the table, online softmax.  It follows PAPER.md Eq. 4 (L94-106) directly and is kept as the
 //    LAZY_FLAG_ROWWISE_KERNELS debugging path; the production kernels are decode_splitkv.cu / prefill_umma.cu.
 #include "lazy_internal.h"
+#include "ptx_util.cuh"
 
 namespace lazy {
 
@@ -20,7 +21,7 @@ __global__ void build_cs_table_kernel(float2* __restrict__ cs, int max_position,
   double inv_freq = pow(theta, -2.0 * (double)j / (double)D);
   double s, c;
   sincos((double)pos * inv_freq, &s, &c);
-  cs[idx] = make_float2((float)c, (float)s);
+  cs[pos * half + cs_index(j, D)] = make_float2((float)c, (float)s);
 }
 
 int launch_build_tables(lazy_handle* h, cudaStream_t stream) {
@@ -112,7 +113,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     for (int e = 0; e < PER; ++e) {
       int j = lane * PER + e;
       float a = __bfloat162float(qp[j]), b = __bfloat162float(qp[j + HALF]);
-      float2 t = cs[(size_t)pos_q * HALF + j];
+      float2 t = cs[(size_t)pos_q * HALF + cs_index(j, D)];
       q1[e] = (a * t.x - b * t.y) * sh.scale_log2;
       q2[e] = (a * t.y + b * t.x) * sh.scale_log2;
     }
@@ -131,7 +132,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     for (int e = 0; e < PER; ++e) {
       int j = lane * PER + e;
       float a = __bfloat162float(k_cache[base + j]), b = __bfloat162float(k_cache[base + j + HALF]);
-      float2 tcs = cs[(size_t)pos * HALF + j];
+      float2 tcs = cs[(size_t)pos * HALF + cs_index(j, D)];
       dot += q1[e] * (a * tcs.x - b * tcs.y) + q2[e] * (a * tcs.y + b * tcs.x);
       v1[e] = __bfloat162float(v_cache[base + j]);
       v2[e] = __bfloat162float(v_cache[base + j + HALF]);

@@ -1,10 +1,534 @@
-// decode_splitkv.cu -- placeholder: routes to the row-wise kernel until the split-KV kernel lands.
+// decode_splitkv.cu -- lazy_attn_decode: split-KV flash-decoding over position-free paged K (sm_100a).
+//
+// Path rows: a1 metadata fetch, a2 page gather (TMA, 128B-swizzled boxes), a3/a4 rotation in
+// fp32 registers, a5 QK^T, a6 online softmax (warp-shuffle max), a7 PV, a8 split-KV combine, a9 epilogue.
+//
+// Rotation identity used (PAPER.md Fact 3.2, L154-158; "rotate Q when the document changes", L175):
+//     score(query at m, key t of a page starting at p0) = (R_{m-p0} q)^T (R_t k)
+// so K is rotated only by its in-page offset t in [0,16) -- 16 x D/2 angles that live in shared memory for
+// the whole kernel (rows 0..15 of the cos/sin table) -- and q is re-rotated once per page by m - p0 with one
+// D/2-entry cos/sin row fetched by the same bulk-copy pipeline that brings the page.  No per-token table
+// traffic, no writes to the cache.
+//
+// Work decomposition: the (request, page-group) units of the whole batch are cut into gridDim.x equal
+// contiguous ranges (stream-K style), so every SM streams the same number of bytes whatever the length mix.
+// A CTA owns HKV_CTA kv heads of a page (8 / HKV_CTA pages per pipeline stage); each of its 8 consumer warps
+// owns one (page-lane, kv head) tile per stage and all q heads of that kv head's GQA group.  A 9th warp
+// produces: block-table prefetch, TMA issue, mbarrier bookkeeping.  Per tile a warp does
+//   S[16 tok x 8 heads] = Khat[16 x D] Qhat^T   (mma.sync m16n8k16, tokens as M so a page is exactly one tile)
+//   online softmax over tokens, P -> bf16, transposed in registers with movmatrix
+//   O^T[D x 8 heads]  += V^T[D x 16] P          (V^T fragments via ldmatrix.trans from the swizzled tile)
+// The legacy mma.sync path is deliberate: this kernel is HBM-bound (512 B per (token, kv head)); the tensor
+// work per page is 32 small MMAs and tcgen05's 128-row tiles would be >90% padding at 4-8 query rows.
+// Partials (o, m, l) go to the workspace; the last CTA to finish a request combines them (no second launch).
+#include <climits>
+
 #include "lazy_internal.h"
+#include "ptx_util.cuh"
+
 namespace lazy {
+namespace {
+
+constexpr int kConsumerWarps = 8;
+constexpr int kDecodeThreads = (kConsumerWarps + 1) * 32;
+constexpr int kMaxReqsSmem = 2048;
+
+template <int D, int HKV_CTA>
+struct DecodeCfg {
+  static constexpr int NH = D / 64;                     // 128-byte column blocks per row
+  static constexpr int PPS = kConsumerWarps / HKV_CTA;  // pages per pipeline stage
+  static constexpr int BOX_ROWS = 16 * HKV_CTA;
+  static constexpr int BOX_BYTES = BOX_ROWS * 128;
+  static constexpr int PAGE_BYTES = NH * BOX_BYTES;     // K (or V) of one page, HKV_CTA heads
+  static constexpr int CS_ROW_BYTES = D / 2 * 8;
+  static constexpr int OFF_V = PPS * PAGE_BYTES;
+  static constexpr int OFF_CS = 2 * PPS * PAGE_BYTES;
+  static constexpr int OFF_META = OFF_CS + PPS * CS_ROW_BYTES;
+  static constexpr int STAGE_BYTES = (OFF_META + PPS * 4 + 1023) / 1024 * 1024;
+  static constexpr int NSTAGES = (STAGE_BYTES > 40000) ? 3 : 4;
+  static constexpr int JT = D / 8;                      // rotation pairs (j values) per thread
+  static constexpr int NL = JT / 2;                     // 16-byte cos/sin loads per thread per token row
+  static constexpr int NLK = JT / 8;                    // 16-byte K loads per thread per row per half
+  static constexpr int NC = D / 16;                     // MMA k-chunks (QK^T) == dim tiles (PV)
+  static constexpr int CTAB_BYTES = 2 * NL * 32 * 16;
+  static constexpr int OFF_CTAB = NSTAGES * STAGE_BYTES;
+  static constexpr int OFF_CUM = OFF_CTAB + CTAB_BYTES;
+  static constexpr int OFF_LEN = OFF_CUM + (kMaxReqsSmem + 4) * 4;   // keeps the mbarriers 16-byte aligned
+  static constexpr int OFF_BAR = OFF_LEN + kMaxReqsSmem * 4;
+  static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGES * 8 + 16 + 1024;  // + alignment slack
+};
+
+struct DecodeArgs {
+  const __nv_bfloat16* q;
+  const int* block_table;
+  const int* page_pos;
+  const int* seq_lens;
+  __nv_bfloat16* out;
+  const float2* cs;
+  float* part_o;
+  float2* part_ml;
+  int* req_counter;
+  int num_reqs;
+  Shape sh;
+};
+
+template <int D, int HKV_CTA>
+__global__ void __launch_bounds__(kDecodeThreads, 1)
+decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
+                      const DecodeArgs a) {
+  using C = DecodeCfg<D, HKV_CTA>;
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const uint32_t smem_base = ptx::smem_u32(smem);
+  int* s_cum = reinterpret_cast<int*>(smem + C::OFF_CUM);
+  int* s_len = reinterpret_cast<int*>(smem + C::OFF_LEN);
+  const uint32_t bar_full = smem_base + C::OFF_BAR;
+  const uint32_t bar_empty = bar_full + C::NSTAGES * 8;
+  int* s_flag = reinterpret_cast<int*>(smem + C::OFF_BAR + 2 * C::NSTAGES * 8);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int R = a.num_reqs;
+  const int hg = blockIdx.y;                       // kv-head group of this CTA
+  const int HG = gridDim.y;
+  int G = gridDim.x;                               // clamped to the unit count below: no CTA range is empty
+  const Shape sh = a.sh;
+
+  // ---- prologue: barriers, unit prefix sums, in-page rotation constants -------------------------------
+  if (tid == 0) {
+    for (int s = 0; s < C::NSTAGES; ++s) {
+      ptx::mbar_init(bar_full + 8 * s, 1);
+      ptx::mbar_init(bar_empty + 8 * s, kConsumerWarps);
+    }
+    ptx::fence_mbar_init();
+  }
+  if (warp == kConsumerWarps && lane == 0) {
+    ptx::prefetch_tmap(&tmap_k);
+    ptx::prefetch_tmap(&tmap_v);
+  }
+  if (warp == 0) {
+    // units per request (a unit = PPS consecutive pages; empty requests get one empty unit), inclusive scan
+    int carry = 0;
+    if (lane == 0) s_cum[0] = 0;
+    for (int base = 0; base < R; base += 32) {
+      int r = base + lane;
+      int L = (r < R) ? a.seq_lens[r] : 0;
+      if (L < 0) L = 0;
+      int np = (L + kPageSize - 1) / kPageSize;
+      int nu = (r < R) ? max(1, (np + C::PPS - 1) / C::PPS) : 0;
+      int x = nu;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+      }
+      if (r < R) { s_cum[r + 1] = carry + x; s_len[r] = L; }
+      carry += __shfl_sync(0xffffffffu, x, 31);
+    }
+  }
+  {
+    // ctab[k'][lane] (16 B each): (cos,sin) pairs of the in-page offsets, pre-multiplied by log2(e)/sqrt(D),
+    // in the order thread (g,tq) consumes them: row t = g + 8*(k'/NL), pairs j = JT*tq + 2*(k'%NL), +1.
+    float4* ctab = reinterpret_cast<float4*>(smem + C::OFF_CTAB);
+    const float4* cs4 = reinterpret_cast<const float4*>(a.cs);
+    for (int i = tid; i < 2 * C::NL * 32; i += kDecodeThreads) {
+      int kk = i >> 5, ln = i & 31;
+      int g = ln >> 2, tq = ln & 3;
+      int t = g + 8 * (kk / C::NL);
+      float4 v = cs4[(size_t)t * (D / 4) + (kk % C::NL) * 4 + tq];
+      v.x *= sh.scale_log2; v.y *= sh.scale_log2; v.z *= sh.scale_log2; v.w *= sh.scale_log2;
+      ctab[i] = v;
+    }
+  }
+  __syncthreads();
+
+  const long long U = s_cum[R];
+  if (U < G) G = (int)U;
+  if ((int)blockIdx.x >= G) return;
+  const int u_begin = (int)(((long long)blockIdx.x * U) / G);
+  const int u_end = (int)(((long long)(blockIdx.x + 1) * U) / G);
+  if (u_begin >= u_end) return;
+  int r0;
+  {
+    int lo = 0, hi = R;                             // smallest r with cum[r+1] > u_begin
+    while (lo < hi) { int mid = (lo + hi) >> 1; if (s_cum[mid + 1] > u_begin) hi = mid; else lo = mid + 1; }
+    r0 = lo;
+  }
+
+  if (warp == kConsumerWarps) {
+    // ================================= producer warp =====================================================
+    const int pl = lane;                            // page lane within a stage (lanes < PPS are active)
+    int r = r0, u = u_begin;
+    int it = 0;
+    // state of the unit about to be issued
+    auto load_unit = [&](int rr, int uu, int& pg, int& delta, int& nvalid) {
+      int L = s_len[rr];
+      int np = (L + kPageSize - 1) / kPageSize;
+      int ul = uu - s_cum[rr];
+      int p = ul * C::PPS + pl;
+      nvalid = min(C::PPS, max(0, np - ul * C::PPS));
+      pg = 0; delta = 0;
+      if (pl < C::PPS && p < np) {
+        const int* bt = a.block_table + (size_t)rr * sh.table_stride;
+        const int* pp = a.page_pos + (size_t)rr * sh.table_stride;
+        int mq = pp[(L - 1) / kPageSize] + (L - 1) % kPageSize;    // position of the query token
+        pg = bt[p];
+        delta = mq - pp[p];
+      }
+    };
+    int pg, delta, nvalid;
+    load_unit(r, u, pg, delta, nvalid);
+    while (u < u_end) {
+      // prefetch the table entries of the next unit before blocking on the ring
+      int rn = r, un = u + 1;
+      if (un >= s_cum[rn + 1]) rn++;
+      int pg_n = 0, delta_n = 0, nvalid_n = 0;
+      if (un < u_end) load_unit(rn, un, pg_n, delta_n, nvalid_n);
+
+      const int stage = it % C::NSTAGES;
+      const uint32_t parity = (it / C::NSTAGES) & 1;
+      ptx::mbar_wait(bar_empty + 8 * stage, parity ^ 1);
+      unsigned char* st = smem + stage * C::STAGE_BYTES;
+      const uint32_t st_u32 = smem_base + stage * C::STAGE_BYTES;
+      const uint32_t full = bar_full + 8 * stage;
+      const bool active = pl < nvalid;
+      if (pl < C::PPS) reinterpret_cast<int*>(st + C::OFF_META)[pl] = delta;
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive_expect_tx(full, nvalid * (2 * C::PAGE_BYTES + C::CS_ROW_BYTES));
+      __syncwarp();
+      if (active) {
+        const int row0 = (pg * sh.Hkv + hg * HKV_CTA) * kPageSize;
+#pragma unroll
+        for (int h = 0; h < C::NH; ++h) {
+          ptx::tma_load_2d(st_u32 + pl * C::PAGE_BYTES + h * C::BOX_BYTES, &tmap_k, full, h * 64, row0);
+          ptx::tma_load_2d(st_u32 + C::OFF_V + pl * C::PAGE_BYTES + h * C::BOX_BYTES, &tmap_v, full, h * 64, row0);
+        }
+        int ad = delta < 0 ? -delta : delta;
+        ptx::bulk_load_1d(st_u32 + C::OFF_CS + pl * C::CS_ROW_BYTES, a.cs + (size_t)ad * (D / 2),
+                          C::CS_ROW_BYTES, full);
+      }
+      pg = pg_n; delta = delta_n; nvalid = nvalid_n;
+      r = rn; u = un; ++it;
+    }
+    return;
+  }
+
+  // =================================== consumer warps ====================================================
+  const int g = lane >> 2, tq = lane & 3;
+  const int pl = warp / HKV_CTA;                    // page lane within a stage
+  const int hl = warp % HKV_CTA;                    // kv head within the CTA's head group
+  const int hk = hg * HKV_CTA + hl;
+  const int group = sh.group;
+  const float4* ctab = reinterpret_cast<const float4*>(smem + C::OFF_CTAB);
+
+  int r = r0, u = u_begin, it = 0;
+  while (u < u_end) {
+    const int L = s_len[r];
+    const int seg_lo = u - s_cum[r];
+    const int seg_hi = min(u_end, s_cum[r + 1]) - s_cum[r];
+
+    // un-rotated q of head g of this kv head's group, as packed bf16 in this thread's k-slot order
+    uint32_t qraw[2][C::NL];
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int w = 0; w < C::NL; ++w) qraw[h][w] = 0u;
+    if (g < group) {
+      const uint4* qp = reinterpret_cast<const uint4*>(a.q + ((size_t)r * sh.Hq + hk * group + g) * D);
+#pragma unroll
+      for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int x = 0; x < C::NLK; ++x) {
+          uint4 v = qp[(h * (D / 2) + C::JT * tq) / 8 + x];
+          qraw[h][4 * x + 0] = v.x; qraw[h][4 * x + 1] = v.y; qraw[h][4 * x + 2] = v.z; qraw[h][4 * x + 3] = v.w;
+        }
+    }
+
+    float oacc[C::NC][4];
+#pragma unroll
+    for (int i = 0; i < C::NC; ++i) { oacc[i][0] = oacc[i][1] = oacc[i][2] = oacc[i][3] = 0.f; }
+    float m_run[2] = {-INFINITY, -INFINITY};        // heads 2tq, 2tq+1 (log2 units)
+    float l_run[2] = {0.f, 0.f};                    // this thread's share (rows g, g+8) of the softmax sums
+
+    for (int ul = seg_lo; ul < seg_hi; ++ul, ++it) {
+      const int stage = it % C::NSTAGES;
+      const uint32_t parity = (it / C::NSTAGES) & 1;
+      ptx::mbar_wait(bar_full + 8 * stage, parity);
+      const int p = ul * C::PPS + pl;
+      const int nv = min(kPageSize, L - p * kPageSize);      // valid tokens of this page (<= 0: no page)
+      if (nv > 0) {
+        unsigned char* st = smem + stage * C::STAGE_BYTES;
+        const int delta = reinterpret_cast<const int*>(st + C::OFF_META)[pl];
+        // ---- K tile -> registers (rows g, g+8 of head hl; this thread's JT dims of each half)
+        uint32_t kreg[2][2][C::NL];                 // [half][row][word]
+        const int R0 = hl * 16 + g;
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+          for (int rw = 0; rw < 2; ++rw)
+#pragma unroll
+            for (int x = 0; x < C::NLK; ++x) {
+              int d = h * (D / 2) + C::JT * tq + 8 * x;
+              int Rr = R0 + 8 * rw;
+              const unsigned char* ptr = st + pl * C::PAGE_BYTES + (d / 64) * C::BOX_BYTES + Rr * 128 +
+                                         ((((d % 64) / 8) ^ (Rr & 7)) * 16);
+              uint4 v = *reinterpret_cast<const uint4*>(ptr);
+              kreg[h][rw][4 * x + 0] = v.x; kreg[h][rw][4 * x + 1] = v.y;
+              kreg[h][rw][4 * x + 2] = v.z; kreg[h][rw][4 * x + 3] = v.w;
+            }
+        // ---- q re-rotated for this page: Qhat = R_{m - p0} q   (a3/a4; one cos/sin row per page)
+        uint32_t qhat[2][C::NL];
+        {
+          const float4* qcs = reinterpret_cast<const float4*>(st + C::OFF_CS + pl * C::CS_ROW_BYTES);
+          const float sgn = delta < 0 ? -1.f : 1.f;
+#pragma unroll
+          for (int w = 0; w < C::NL; ++w) {
+            float4 c = qcs[w * 4 + tq];
+            c.y *= sgn; c.w *= sgn;
+            float a_lo = ptx::bf16_lo(qraw[0][w]), a_hi = ptx::bf16_hi(qraw[0][w]);
+            float b_lo = ptx::bf16_lo(qraw[1][w]), b_hi = ptx::bf16_hi(qraw[1][w]);
+            qhat[0][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
+            qhat[1][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
+          }
+        }
+        // ---- Khat = scale * R_t k in fp32 registers, rounded to bf16 for the MMA
+#pragma unroll
+        for (int rw = 0; rw < 2; ++rw)
+#pragma unroll
+          for (int w = 0; w < C::NL; ++w) {
+            float4 c = ctab[(rw * C::NL + w) * 32 + lane];
+            float a_lo = ptx::bf16_lo(kreg[0][rw][w]), a_hi = ptx::bf16_hi(kreg[0][rw][w]);
+            float b_lo = ptx::bf16_lo(kreg[1][rw][w]), b_hi = ptx::bf16_hi(kreg[1][rw][w]);
+            kreg[0][rw][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
+            kreg[1][rw][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
+          }
+        // ---- S = Khat Qhat^T : rows = tokens (g, g+8), cols = heads (2tq, 2tq+1)
+        float s[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int c = 0; c < C::NC; ++c) {
+          const int h = c / (C::NC / 2), cc = c % (C::NC / 2);
+          ptx::mma_bf16_16816(s, kreg[h][0][2 * cc], kreg[h][1][2 * cc], kreg[h][0][2 * cc + 1],
+                              kreg[h][1][2 * cc + 1], qhat[h][2 * cc], qhat[h][2 * cc + 1]);
+        }
+        if (g >= nv) { s[0] = -INFINITY; s[1] = -INFINITY; }
+        if (g + 8 >= nv) { s[2] = -INFINITY; s[3] = -INFINITY; }
+        // ---- online softmax over the 16 tokens (a6): max across the 8 row-lanes with shuffles
+        float mx0 = fmaxf(s[0], s[2]), mx1 = fmaxf(s[1], s[3]);
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+          mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, o));
+          mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, o));
+        }
+        const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);   // finite: token 0 is valid
+        const float corr0 = exp2f(m_run[0] - mn0), corr1 = exp2f(m_run[1] - mn1);
+        m_run[0] = mn0; m_run[1] = mn1;
+        const float p0 = exp2f(s[0] - mn0), p1 = exp2f(s[1] - mn1);
+        const float p2 = exp2f(s[2] - mn0), p3 = exp2f(s[3] - mn1);
+        l_run[0] = l_run[0] * corr0 + p0 + p2;
+        l_run[1] = l_run[1] * corr1 + p1 + p3;
+#pragma unroll
+        for (int i = 0; i < C::NC; ++i) {
+          oacc[i][0] *= corr0; oacc[i][1] *= corr1; oacc[i][2] *= corr0; oacc[i][3] *= corr1;
+        }
+        // ---- P (bf16) transposed into the B-fragment layout: k = tokens, n = heads
+        const uint32_t pb0 = ptx::movmatrix_trans(ptx::pack_bf16(p0, p1));
+        const uint32_t pb1 = ptx::movmatrix_trans(ptx::pack_bf16(p2, p3));
+        // ---- O^T += V^T P  (a7): V^T fragments straight from the swizzled tile
+        uint32_t vmask_lo = 0xffffffffu, vmask_hi = 0xffffffffu;   // tail: never let bytes past seq_len in
+        if (nv < kPageSize) {
+          int t0 = 2 * tq, t1 = 2 * tq + 8;
+          vmask_lo = (t0 < nv ? 0x0000ffffu : 0u) | (t0 + 1 < nv ? 0xffff0000u : 0u);
+          vmask_hi = (t1 < nv ? 0x0000ffffu : 0u) | (t1 + 1 < nv ? 0xffff0000u : 0u);
+        }
+        const int mi = lane >> 3;
+        const int vrow = hl * 16 + (lane & 7) + 8 * (mi >> 1);
+        const uint32_t vbase = smem_base + stage * C::STAGE_BYTES + C::OFF_V + pl * C::PAGE_BYTES + vrow * 128;
+#pragma unroll
+        for (int i = 0; i < C::NC; ++i) {
+          const int chunk = 2 * i + (mi & 1);       // 16-byte chunk (8 dims) along the row
+          const uint32_t addr = vbase + (chunk / 8) * C::BOX_BYTES + (((chunk % 8) ^ (vrow & 7)) * 16);
+          uint32_t a0, a1, a2, a3;
+          ptx::ldmatrix_x4_trans(a0, a1, a2, a3, addr);
+          if (nv < kPageSize) { a0 &= vmask_lo; a1 &= vmask_lo; a2 &= vmask_hi; a3 &= vmask_hi; }
+          ptx::mma_bf16_16816(oacc[i], a0, a1, a2, a3, pb0, pb1);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(bar_empty + 8 * stage);
+    }
+
+    // ---- segment done: this warp's partial (o, m, l) for its kv head -> workspace (a8)
+#pragma unroll
+    for (int o = 4; o < 32; o <<= 1) {
+      l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], o);
+      l_run[1] += __shfl_xor_sync(0xffffffffu, l_run[1], o);
+    }
+    const int slot = (r + blockIdx.x) * C::PPS + pl;
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const int n = 2 * tq + e;
+      if (n < group) {
+        const int hq = hk * group + n;
+        float* po = a.part_o + ((size_t)slot * sh.Hq + hq) * D;
+#pragma unroll
+        for (int i = 0; i < C::NC; ++i) {
+          po[16 * i + g] = oacc[i][e];
+          po[16 * i + g + 8] = oacc[i][2 + e];
+        }
+        if (g == 0) a.part_ml[(size_t)slot * sh.Hq + hq] = make_float2(m_run[e], l_run[e]);
+      }
+    }
+    __threadfence();
+    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    // number of CTAs that hold a piece of request r: those containing units cum[r] .. cum[r+1]-1
+    const long long c0 = s_cum[r], c1 = s_cum[r + 1];
+    const int b_first = (int)(((c0 + 1) * G + U - 1) / U) - 1;
+    const int b_last = (int)((c1 * G + U - 1) / U) - 1;
+    const int n_parts = b_last - b_first + 1;
+    if (tid == 0) {
+      int old = atomicAdd(&a.req_counter[r * HG + hg], 1);
+      int last = (old == n_parts - 1);
+      if (last) a.req_counter[r * HG + hg] = 0;     // self-resetting: ready for the next call
+      *s_flag = last;
+    }
+    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    if (*s_flag) {
+      __threadfence();
+      // ---- combine (a8) + epilogue (a9): warp w takes q heads w, w+8, ... of this CTA's head group
+      const int heads_cta = HKV_CTA * group;
+      for (int hh = warp; hh < heads_cta; hh += kConsumerWarps) {
+        const int hq = hg * heads_cta + hh;
+        const int n_slots = n_parts * C::PPS;
+        const int slot0 = (r + b_first) * C::PPS;
+        float mstar = -INFINITY;
+        for (int sidx = 0; sidx < n_slots; ++sidx)
+          mstar = fmaxf(mstar, __ldcg(&a.part_ml[(size_t)(slot0 + sidx) * sh.Hq + hq]).x);
+        float acc[D / 32];
+#pragma unroll
+        for (int x = 0; x < D / 32; ++x) acc[x] = 0.f;
+        float lsum = 0.f;
+        for (int sidx = 0; sidx < n_slots; ++sidx) {
+          float2 ml = __ldcg(&a.part_ml[(size_t)(slot0 + sidx) * sh.Hq + hq]);
+          if (ml.x == -INFINITY) continue;
+          float w = exp2f(ml.x - mstar);
+          lsum += w * ml.y;
+          const float* po = a.part_o + ((size_t)(slot0 + sidx) * sh.Hq + hq) * D + lane * (D / 32);
+#pragma unroll
+          for (int x = 0; x < D / 32; x += 2) {
+            float2 v = __ldcg(reinterpret_cast<const float2*>(po + x));
+            acc[x] += w * v.x; acc[x + 1] += w * v.y;
+          }
+        }
+        const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
+        __nv_bfloat16* op = a.out + ((size_t)r * sh.Hq + hq) * D + lane * (D / 32);
+#pragma unroll
+        for (int x = 0; x < D / 32; x += 2)
+          *reinterpret_cast<uint32_t*>(op + x) = ptx::pack_bf16(acc[x] * inv, acc[x + 1] * inv);
+      }
+    }
+    ptx::named_bar_sync(1, kConsumerWarps * 32);    // s_flag is reused by the next segment
+    u = s_cum[r] + seg_hi;
+    ++r;
+  }
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  return fn;
+}
+
+}  // namespace
+
+// 2-D view of a pool: rows = num_pages*Hkv*16 tokens-of-a-head, cols = D; box = [box_rows][64 cols], 128B swizzle.
+bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, int box_rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t gdim[2] = {(cuuint64_t)D, (cuuint64_t)rows};
+  cuuint64_t gstride[1] = {(cuuint64_t)D * 2};
+  cuuint32_t box[2] = {64u, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1u, 1u};
+  CUresult rc = fn(reinterpret_cast<CUtensorMap*>(out_map), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2,
+                   const_cast<void*>(pool), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return rc == CUDA_SUCCESS;
+}
+
+template <int D, int HKV_CTA>
+static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, int grid_y, cudaStream_t stream) {
+  using C = DecodeCfg<D, HKV_CTA>;
+  static bool attr_set = false;
+  auto kern = decode_splitkv_kernel<D, HKV_CTA>;
+  if (!attr_set) {
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
+      return LAZY_ERR_CUDA;
+    attr_set = true;
+  }
+  const CUtensorMap* mk = reinterpret_cast<const CUtensorMap*>(h->tmap_k);
+  const CUtensorMap* mv = reinterpret_cast<const CUtensorMap*>(h->tmap_v);
+  kern<<<dim3(grid_x, grid_y), kDecodeThreads, C::SMEM_BYTES, stream>>>(*mk, *mv, args);
+  return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
+}
+
 int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                   const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                   int num_reqs, void* out, cudaStream_t stream) {
-  return launch_rowwise(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, nullptr, num_reqs,
-                        num_reqs, 1, out, stream);
+  const lazy_config& c = h->cfg;
+  const int hkv_cta = c.num_kv_heads >= 8 ? 8 : c.num_kv_heads;
+  const int HG = c.num_kv_heads / hkv_cta;
+  const long long rows = (long long)c.num_pages * c.num_kv_heads * kPageSize;
+  if (h->tmap_k_ptr != k_cache) {
+    if (!encode_pool_tmap(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta)) return LAZY_ERR_CUDA;
+    h->tmap_k_ptr = k_cache;
+  }
+  if (h->tmap_v_ptr != v_cache) {
+    if (!encode_pool_tmap(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta)) return LAZY_ERR_CUDA;
+    h->tmap_v_ptr = v_cache;
+  }
+  int launches = 0;
+  for (int r0 = 0; r0 < num_reqs; r0 += kMaxReqsSmem) {
+    const int n = (num_reqs - r0 < kMaxReqsSmem) ? num_reqs - r0 : kMaxReqsSmem;
+    DecodeArgs a;
+    a.q = static_cast<const __nv_bfloat16*>(q) + (size_t)r0 * c.num_q_heads * c.head_dim;
+    a.out = static_cast<__nv_bfloat16*>(out) + (size_t)r0 * c.num_q_heads * c.head_dim;
+    a.block_table = block_table + (size_t)r0 * c.max_pages_per_req;
+    a.page_pos = page_logical_pos + (size_t)r0 * c.max_pages_per_req;
+    a.seq_lens = seq_lens + r0;
+    a.cs = h->ws.cs;
+    a.part_o = h->ws.part_o;
+    a.part_ml = h->ws.part_ml;
+    a.req_counter = h->ws.req_counter;
+    a.num_reqs = n;
+    a.sh = h->shape;
+    int gx = h->num_sms / HG;
+    if (gx < 1) gx = 1;
+    if (gx > kMaxDecodeCtas) gx = kMaxDecodeCtas;
+    int rc;
+    if (c.head_dim == 128) {
+      if (hkv_cta == 8) rc = launch_decode_t<128, 8>(h, a, gx, HG, stream);
+      else if (hkv_cta == 4) rc = launch_decode_t<128, 4>(h, a, gx, HG, stream);
+      else if (hkv_cta == 2) rc = launch_decode_t<128, 2>(h, a, gx, HG, stream);
+      else rc = launch_decode_t<128, 1>(h, a, gx, HG, stream);
+    } else {
+      if (hkv_cta == 8) rc = launch_decode_t<64, 8>(h, a, gx, HG, stream);
+      else if (hkv_cta == 4) rc = launch_decode_t<64, 4>(h, a, gx, HG, stream);
+      else if (hkv_cta == 2) rc = launch_decode_t<64, 2>(h, a, gx, HG, stream);
+      else rc = launch_decode_t<64, 1>(h, a, gx, HG, stream);
+    }
+    if (rc < 0) return rc;
+    launches += rc;
+  }
+  return launches;
 }
+
 }  // namespace lazy

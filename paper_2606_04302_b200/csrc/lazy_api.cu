@@ -36,11 +36,14 @@ struct Layout {
 Layout workspace_layout(const lazy_config* c) {
   Layout l{};
   size_t off = 0;
-  size_t parts = (size_t)c->max_reqs + lazy::kMaxDecodeCtas;
+  // decode partials: one slot per (request, CTA) intersection and page lane (8 / kv-heads-per-CTA lanes)
+  int hkv_cta = c->num_kv_heads >= 8 ? 8 : c->num_kv_heads;
+  size_t parts = ((size_t)c->max_reqs + lazy::kMaxDecodeCtas) * (8 / hkv_cta);
+  size_t head_groups = (size_t)c->num_kv_heads / hkv_cta;
   l.cs = off;          off = align_up(off + (size_t)c->max_position * (c->head_dim / 2) * sizeof(float2), 256);
   l.part_o = off;      off = align_up(off + parts * c->num_q_heads * c->head_dim * sizeof(float), 256);
   l.part_ml = off;     off = align_up(off + parts * c->num_q_heads * sizeof(float2), 256);
-  l.req_counter = off; off = align_up(off + (size_t)c->max_reqs * sizeof(int), 256);
+  l.req_counter = off; off = align_up(off + (size_t)c->max_reqs * head_groups * sizeof(int), 256);
   l.sched = off;       off = align_up(off + 1024 * sizeof(int), 256);
   l.total = off;
   return l;
@@ -92,7 +95,7 @@ int lazy_create(const lazy_config* cfg, void* workspace, size_t workspace_bytes,
     return LAZY_ERR_CUDA;
   }
   cudaStream_t s = static_cast<cudaStream_t>(stream);
-  if (cudaMemsetAsync(h->ws.req_counter, 0, (size_t)cfg->max_reqs * sizeof(int), s) != cudaSuccess ||
+  if (cudaMemsetAsync(h->ws.req_counter, 0, l.sched - l.req_counter, s) != cudaSuccess ||
       cudaMemsetAsync(h->ws.sched, 0, 1024 * sizeof(int), s) != cudaSuccess) {
     delete h;
     return LAZY_ERR_CUDA;

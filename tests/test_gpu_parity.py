@@ -45,7 +45,7 @@ def test_configs_reduced_full_compare(cfg, scale, flags):
 def test_configs_peaked_queries(cfg):
     """q scaled x4: softmax is peaked, so positions matter strongly (SURVEY 8.c tolerance warning)."""
     scale = {2: 0.1, 3: 0.07, 4: 0.25, 5: 0.25}[cfg]
-    _run(W.CONFIGS[cfg](scale=scale, q_scale=4.0))
+    _run(W.CONFIGS[cfg](scale=scale, q_scale=4.0), scale_abs_by_output=True)
 
 
 @pytest.mark.parametrize("cfg,rows", [(2, 0), (3, 96), (4, 0), (5, 64)])
