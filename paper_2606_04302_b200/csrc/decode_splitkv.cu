@@ -464,6 +464,21 @@ bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, in
   return rc == CUDA_SUCCESS;
 }
 
+bool encode_q_tmap(void* out_map, const void* q, int total_q, int Hq, int Hkv, int D, int tokens_per_tile) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  const int group = Hq / Hkv;
+  cuuint64_t gdim[4] = {(cuuint64_t)D, (cuuint64_t)group, (cuuint64_t)Hkv, (cuuint64_t)total_q};
+  cuuint64_t gstride[3] = {(cuuint64_t)D * 2, (cuuint64_t)group * D * 2, (cuuint64_t)Hq * D * 2};
+  cuuint32_t box[4] = {64u, (cuuint32_t)group, 1u, (cuuint32_t)tokens_per_tile};
+  cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+  CUresult rc = fn(reinterpret_cast<CUtensorMap*>(out_map), CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4,
+                   const_cast<void*>(q), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return rc == CUDA_SUCCESS;
+}
+
 template <int D, int HKV_CTA>
 static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, int grid_y, cudaStream_t stream) {
   using C = DecodeCfg<D, HKV_CTA>;

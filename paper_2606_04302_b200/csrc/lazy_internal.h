@@ -52,6 +52,13 @@ struct lazy_handle {
 
 namespace lazy {
 
+// TMA descriptors (cuTensorMapEncodeTiled through the runtime's driver entry point; 128-byte swizzle).
+//   pool : 2-D view [num_pages*Hkv*16 rows][D], box = [box_rows][64 columns]
+//   q    : 4-D view (D, group, Hkv, total_q) of q [total_q][Hq][D], box = (64, group, 1, tokens_per_tile):
+//          lands as rows token*group + head-in-group of one kv head's GQA group.
+bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, int box_rows);
+bool encode_q_tmap(void* out_map, const void* q, int total_q, int Hq, int Hkv, int D, int tokens_per_tile);
+
 // Each launcher enqueues on `stream` and returns the number of kernels launched (<0: LAZY_ERR_*).
 int launch_build_tables(lazy_handle* h, cudaStream_t stream);
 int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
