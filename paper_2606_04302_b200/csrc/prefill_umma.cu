@@ -36,20 +36,26 @@ struct PrefillCfg {
   static constexpr int NH = D / 64;                 // 128-byte column slabs per row
   static constexpr int TILE_BYTES = NH * kHalfBytes;
   static constexpr int CPR = D / 16;                // rotation chunk-pairs (8 pairs each) per row
+  static constexpr int CS_ROW_BYTES = D / 2 * 8;    // one table row: D/2 (cos, sin) float2
+  static constexpr int CS_STAGE_BYTES = kPagesPerTile * CS_ROW_BYTES;
   static constexpr int OFF_Q = 0;                   // 2 tiles
   static constexpr int OFF_K = 2 * TILE_BYTES;      // 2 stages
   static constexpr int OFF_V = 4 * TILE_BYTES;      // 2 stages
-  static constexpr int OFF_BAR = 6 * TILE_BYTES;
+  static constexpr int OFF_CS = 6 * TILE_BYTES;     // 2 stages of 8 table rows (e^{i p0 theta_j} per page)
+  static constexpr int OFF_BAR = OFF_CS + 2 * CS_STAGE_BYTES;
   static constexpr int NUM_BARS = 24;
   static constexpr int OFF_TMEM = OFF_BAR + NUM_BARS * 8;
   static constexpr int SMEM_BYTES = OFF_TMEM + 16 + 1024;   // + alignment slack
 };
 
+// register budgets per warpgroup (setmaxnreg; 2*128*184 + 128*104 + 128*40 = 65536)
+constexpr int kRegsSoftmax = 184, kRegsRotate = 104, kRegsMisc = 40;
+
 // barrier indices
 enum : int {
   B_QFULL = 0,    // +t   TMA -> softmax WG t
   B_QREADY = 2,   // +t   softmax WG t (4 warps) -> MMA
-  B_KFULL = 4,    // +s   TMA -> rotate WG
+  B_KFULL = 4,    // +s   TMA (K boxes + table rows) -> rotate WG
   B_KREADY = 6,   // +s   rotate WG (4 warps) -> MMA
   B_KEMPTY = 8,   // +s   MMA commit -> TMA
   B_VFULL = 10,   // +s   TMA -> MMA, fixer
@@ -86,18 +92,32 @@ __device__ __forceinline__ float ex2(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+__device__ __forceinline__ float f32(uint32_t x) { return __uint_as_float(x); }
 
-// (cos, sin) of the 8 rotation pairs j = 8c .. 8c+7 from one row of the table (layout: cs_index in ptx_util.cuh):
-// four 16-byte loads, each holding (cos j, sin j, cos j+1, sin j+1).
+// Index (in 16-byte units) inside a table row of the chunk holding (cos j, sin j, cos j+1, sin j+1), j = 8c + 2x
+// (row layout: cs_index in ptx_util.cuh).
+template <int D>
+__device__ __forceinline__ int cs_f4_index(int c, int x) {
+  constexpr int JT = D / 8;
+  const int j0 = 8 * c;
+  return ((j0 % JT) / 2 + x) * 4 + j0 / JT;
+}
+// (cos, sin) of the 8 rotation pairs j = 8c .. 8c+7 from one table row in global memory / in shared memory.
 template <int D>
 __device__ __forceinline__ void load_cs8(const float2* __restrict__ cs_row, int c, float (&co)[8], float (&si)[8]) {
-  constexpr int JT = D / 8;
-  const int j0 = 8 * c, tq = j0 / JT, k0 = (j0 % JT) / 2;
   const float4* p = reinterpret_cast<const float4*>(cs_row);
 #pragma unroll
   for (int x = 0; x < 4; ++x) {
-    float4 v = __ldg(p + (k0 + x) * 4 + tq);
+    float4 v = __ldg(p + cs_f4_index<D>(c, x));
     co[2 * x] = v.x; si[2 * x] = v.y; co[2 * x + 1] = v.z; si[2 * x + 1] = v.w;
+  }
+}
+template <int D>
+__device__ __forceinline__ void load_cs8_smem(uint32_t row_addr, int c, float (&co)[8], float (&si)[8]) {
+#pragma unroll
+  for (int x = 0; x < 4; ++x) {
+    uint4 v = ptx::lds128(row_addr + 16 * cs_f4_index<D>(c, x));
+    co[2 * x] = f32(v.x); si[2 * x] = f32(v.y); co[2 * x + 1] = f32(v.z); si[2 * x + 1] = f32(v.w);
   }
 }
 
@@ -106,17 +126,16 @@ __device__ __forceinline__ uint32_t chunk_off(int row, int ci) {
   return (ci >> 3) * kHalfBytes + row * 128 + (((ci & 7) ^ (row & 7)) << 4);
 }
 
-// rotate 8 pairs held as two 16-byte chunks (x1 = dims j, x2 = dims j + D/2) by (co, si), scale, round to bf16
-__device__ __forceinline__ void rotate8(uint4& a, uint4& b, const float (&co)[8], const float (&si)[8], float scale) {
+// rotate 8 pairs held as two 16-byte chunks (x1 = dims j, x2 = dims j + D/2) by (co, si), round to bf16
+__device__ __forceinline__ void rotate8(uint4& a, uint4& b, const float (&co)[8], const float (&si)[8]) {
   uint32_t* aw = reinterpret_cast<uint32_t*>(&a);
   uint32_t* bw = reinterpret_cast<uint32_t*>(&b);
 #pragma unroll
   for (int w = 0; w < 4; ++w) {
     float a0 = ptx::bf16_lo(aw[w]), a1 = ptx::bf16_hi(aw[w]);
     float b0 = ptx::bf16_lo(bw[w]), b1 = ptx::bf16_hi(bw[w]);
-    float c0 = co[2 * w] * scale, s0 = si[2 * w] * scale, c1 = co[2 * w + 1] * scale, s1 = si[2 * w + 1] * scale;
-    aw[w] = ptx::pack_bf16(a0 * c0 - b0 * s0, a1 * c1 - b1 * s1);
-    bw[w] = ptx::pack_bf16(a0 * s0 + b0 * c0, a1 * s1 + b1 * c1);
+    aw[w] = ptx::pack_bf16(a0 * co[2 * w] - b0 * si[2 * w], a1 * co[2 * w + 1] - b1 * si[2 * w + 1]);
+    bw[w] = ptx::pack_bf16(a0 * si[2 * w] + b0 * co[2 * w], a1 * si[2 * w + 1] + b1 * co[2 * w + 1]);
   }
 }
 
@@ -129,6 +148,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const uint32_t smem_base = ptx::smem_u32(smem);
   const uint32_t sQ = smem_base + C::OFF_Q, sK = smem_base + C::OFF_K, sV = smem_base + C::OFF_V;
+  const uint32_t sCS = smem_base + C::OFF_CS;
   const uint32_t bars = smem_base + C::OFF_BAR;
   auto bar = [&](int idx) { return bars + 8u * idx; };
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + C::OFF_TMEM);
@@ -181,109 +201,125 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
   ptx::tc_fence_after();
   const uint32_t tbase = *tmem_slot;
 
-  if (warp == 12) {
-    // ================================ TMA producer ==========================================================
-    if (lane == 0) { ptx::prefetch_tmap(&tmap_q); ptx::prefetch_tmap(&tmap_k); ptx::prefetch_tmap(&tmap_v); }
-    if (lane < 2) {
-      const int t = lane;
-      ptx::mbar_arrive_expect_tx(bar(B_QFULL + t), C::NH * group * TPT * 128);
+  if (warp >= 12) {
+    ptx::setmaxnreg_dec<kRegsMisc>();
+    if (warp == 12) {
+      // ================================ TMA producer ========================================================
+      if (lane == 0) { ptx::prefetch_tmap(&tmap_q); ptx::prefetch_tmap(&tmap_k); ptx::prefetch_tmap(&tmap_v); }
+      if (lane < 2) {
+        const int t = lane;
+        ptx::mbar_arrive_expect_tx(bar(B_QFULL + t), C::NH * group * TPT * 128);
 #pragma unroll
-      for (int h = 0; h < C::NH; ++h)
-        tma_load_4d(sQ + t * C::TILE_BYTES + h * kHalfBytes, &tmap_q, bar(B_QFULL + t), h * 64, 0, hk,
-                    q_begin + i0 + t * TPT);
-    }
-    const int kvsel = lane >> 4, half = (lane >> 3) & 1, pg = lane & 7;
-    const bool lane_on = half < C::NH;
-    int page_next = (pg < num_pages) ? bt[pg] : 0;
-    for (int j = 0; j < n_kv; ++j) {
-      const int s = j & 1, ph = (j >> 1) & 1;
-      const int page = page_next;
-      if (j + 1 < n_kv) {
-        const int idx = (j + 1) * kPagesPerTile + pg;
-        page_next = idx < num_pages ? bt[idx] : 0;
+        for (int h = 0; h < C::NH; ++h)
+          tma_load_4d(sQ + t * C::TILE_BYTES + h * kHalfBytes, &tmap_q, bar(B_QFULL + t), h * 64, 0, hk,
+                      q_begin + i0 + t * TPT);
       }
-      const int npv = min(kPagesPerTile, num_pages - j * kPagesPerTile);
-      const int row0 = (page * sh.Hkv + hk) * kPageSize;
-      const uint32_t dst = s * C::TILE_BYTES + half * kHalfBytes + pg * (kPageSize * 128);
-      ptx::mbar_wait(bar(B_KEMPTY + s), ph ^ 1);
-      if (lane == 0) ptx::mbar_arrive_expect_tx(bar(B_KFULL + s), npv * C::NH * kPageSize * 128);
-      __syncwarp();
-      if (kvsel == 0 && lane_on && pg < npv) ptx::tma_load_2d(sK + dst, &tmap_k, bar(B_KFULL + s), half * 64, row0);
-      ptx::mbar_wait(bar(B_VEMPTY + s), ph ^ 1);
-      if (lane == 0) ptx::mbar_arrive_expect_tx(bar(B_VFULL + s), npv * C::NH * kPageSize * 128);
-      __syncwarp();
-      if (kvsel == 1 && lane_on && pg < npv) ptx::tma_load_2d(sV + dst, &tmap_v, bar(B_VFULL + s), half * 64, row0);
-    }
-  } else if (warp == 13) {
-    // ================================ MMA issuer (one lane) =================================================
-    if (lane == 0) {
-      constexpr uint32_t IDESC_QK = ptx::umma_idesc_bf16(128, 128, 0, 0);
-      constexpr uint32_t IDESC_PV = ptx::umma_idesc_bf16(128, D, 0, 1);     // B = V is MN-major
-      auto qk = [&](int t, int s) {
-#pragma unroll
-        for (int k = 0; k < D / 16; ++k) {
-          const uint32_t off = (k >> 2) * kHalfBytes + (k & 3) * 32;
-          ptx::umma_ss(tbase + t * 128, ptx::umma_desc_sw128(sQ + t * C::TILE_BYTES + off, 0, 1024),
-                       ptx::umma_desc_sw128(sK + s * C::TILE_BYTES + off, 0, 1024), IDESC_QK, k > 0);
-        }
-      };
-      auto pv = [&](int t, int s, uint32_t acc) {
-#pragma unroll
-        for (int k = 0; k < kTileRows / 16; ++k)
-          ptx::umma_ts(tbase + 256 + t * 128, tbase + t * 128 + k * 8,
-                       ptx::umma_desc_sw128(sV + s * C::TILE_BYTES + k * 2048, kHalfBytes, 1024), IDESC_PV,
-                       acc | (uint32_t)(k > 0));
-      };
-      ptx::mbar_wait(bar(B_KREADY + 0), 0);
-      for (int t = 0; t < 2; ++t) {
-        ptx::mbar_wait(bar(B_QREADY + t), 0);
-        ptx::tc_fence_after();
-        qk(t, 0);
-        ptx::umma_commit(bar(B_SFULL + t));
-      }
-      ptx::umma_commit(bar(B_KEMPTY + 0));
+      // lane -> (K or V, column slab, page of the tile); the K lanes of slab 0 also fetch the page's table row
+      const int kvsel = lane >> 4, half = (lane >> 3) & 1, pg = lane & 7;
+      const bool lane_on = half < C::NH;
+      int page_next = (pg < num_pages) ? bt[pg] : 0;
+      int pos_next = (pg < num_pages) ? ppos[pg] : 0;
       for (int j = 0; j < n_kv; ++j) {
-        const int s = j & 1;
-        ptx::mbar_wait(bar(B_VFULL + s), (j >> 1) & 1);
-        if (j == n_kv - 1) ptx::mbar_wait(bar(B_VFIXED), 0);
+        const int s = j & 1, ph = (j >> 1) & 1;
+        const int page = page_next, p0 = pos_next;
+        if (j + 1 < n_kv) {
+          const int idx = (j + 1) * kPagesPerTile + pg;
+          page_next = idx < num_pages ? bt[idx] : 0;
+          pos_next = idx < num_pages ? ppos[idx] : 0;
+        }
+        const int npv = min(kPagesPerTile, num_pages - j * kPagesPerTile);
+        const int row0 = (page * sh.Hkv + hk) * kPageSize;
+        const uint32_t dst = s * C::TILE_BYTES + half * kHalfBytes + pg * (kPageSize * 128);
+        ptx::mbar_wait_sleep(bar(B_KEMPTY + s), ph ^ 1);
+        if (lane == 0)
+          ptx::mbar_arrive_expect_tx(bar(B_KFULL + s), npv * (C::NH * kPageSize * 128 + C::CS_ROW_BYTES));
+        __syncwarp();
+        if (kvsel == 0 && lane_on && pg < npv) {
+          ptx::tma_load_2d(sK + dst, &tmap_k, bar(B_KFULL + s), half * 64, row0);
+          if (half == 0)
+            ptx::bulk_load_1d(sCS + s * C::CS_STAGE_BYTES + pg * C::CS_ROW_BYTES, a.cs + (size_t)p0 * (D / 2),
+                              C::CS_ROW_BYTES, bar(B_KFULL + s));
+        }
+        ptx::mbar_wait_sleep(bar(B_VEMPTY + s), ph ^ 1);
+        if (lane == 0) ptx::mbar_arrive_expect_tx(bar(B_VFULL + s), npv * C::NH * kPageSize * 128);
+        __syncwarp();
+        if (kvsel == 1 && lane_on && pg < npv) ptx::tma_load_2d(sV + dst, &tmap_v, bar(B_VFULL + s), half * 64, row0);
+      }
+    } else if (warp == 13) {
+      // ================================ MMA issuer (one lane) ===============================================
+      if (lane == 0) {
+        constexpr uint32_t IDESC_QK = ptx::umma_idesc_bf16(128, 128, 0, 0);
+        constexpr uint32_t IDESC_PV = ptx::umma_idesc_bf16(128, D, 0, 1);     // B = V is MN-major
+        // descriptor bases are laundered through an empty asm so the 8+8 per-k descriptors are re-derived with a
+        // couple of uniform ops per MMA instead of being hoisted out of the KV loop and spilled
+        auto qk = [&](int t, int s) {
+          uint32_t qa = sQ + t * C::TILE_BYTES, ka = sK + s * C::TILE_BYTES;
+          asm volatile("" : "+r"(qa), "+r"(ka));
+#pragma unroll
+          for (int k = 0; k < D / 16; ++k) {
+            const uint32_t off = (k >> 2) * kHalfBytes + (k & 3) * 32;
+            ptx::umma_ss(tbase + t * 128, ptx::umma_desc_sw128(qa + off, 0, 1024),
+                         ptx::umma_desc_sw128(ka + off, 0, 1024), IDESC_QK, k > 0);
+          }
+        };
+        auto pv = [&](int t, int s, uint32_t acc) {
+          uint32_t va = sV + s * C::TILE_BYTES;
+          asm volatile("" : "+r"(va));
+#pragma unroll
+          for (int k = 0; k < kTileRows / 16; ++k)
+            ptx::umma_ts(tbase + 256 + t * 128, tbase + t * 128 + k * 8,
+                         ptx::umma_desc_sw128(va + k * 2048, kHalfBytes, 1024), IDESC_PV, acc | (uint32_t)(k > 0));
+        };
+        ptx::mbar_wait(bar(B_KREADY + 0), 0);
         for (int t = 0; t < 2; ++t) {
-          ptx::mbar_wait(bar(B_PREADY + t), j & 1);
+          ptx::mbar_wait(bar(B_QREADY + t), 0);
           ptx::tc_fence_after();
-          pv(t, s, j > 0);
-          if (t == 1) ptx::umma_commit(bar(B_VEMPTY + s));
-          if (j + 1 < n_kv) {
-            if (t == 0) {
-              ptx::mbar_wait(bar(B_KREADY + (s ^ 1)), ((j + 1) >> 1) & 1);
-              ptx::tc_fence_after();
+          qk(t, 0);
+          ptx::umma_commit(bar(B_SFULL + t));
+        }
+        ptx::umma_commit(bar(B_KEMPTY + 0));
+        for (int j = 0; j < n_kv; ++j) {
+          const int s = j & 1;
+          ptx::mbar_wait(bar(B_VFULL + s), (j >> 1) & 1);
+          if (j == n_kv - 1) ptx::mbar_wait(bar(B_VFIXED), 0);
+          for (int t = 0; t < 2; ++t) {
+            ptx::mbar_wait(bar(B_PREADY + t), j & 1);
+            ptx::tc_fence_after();
+            pv(t, s, j > 0);
+            if (t == 1) ptx::umma_commit(bar(B_VEMPTY + s));
+            if (j + 1 < n_kv) {
+              if (t == 0) {
+                ptx::mbar_wait(bar(B_KREADY + (s ^ 1)), ((j + 1) >> 1) & 1);
+                ptx::tc_fence_after();
+              }
+              qk(t, s ^ 1);
+              ptx::umma_commit(bar(B_SFULL + t));
+              if (t == 1) ptx::umma_commit(bar(B_KEMPTY + (s ^ 1)));
+            } else {
+              ptx::umma_commit(bar(B_OFULL + t));
             }
-            qk(t, s ^ 1);
-            ptx::umma_commit(bar(B_SFULL + t));
-            if (t == 1) ptx::umma_commit(bar(B_KEMPTY + (s ^ 1)));
-          } else {
-            ptx::umma_commit(bar(B_OFULL + t));
           }
         }
       }
-    }
-    __syncwarp();
-  } else if (warp == 14) {
-    // ================================ V tail fixer ==========================================================
-    for (int j = 0; j < n_kv; ++j) ptx::mbar_wait(bar(B_VFULL + (j & 1)), (j >> 1) & 1);
-    const int jl = n_kv - 1;
-    const int rows_valid = min(kTileRows, L - jl * kTileRows);
-    if (rows_valid < kTileRows) {
-      const int n = (kTileRows - rows_valid) * 8 * C::NH;       // 16-byte chunks to clear
-      unsigned char* vb = smem + C::OFF_V + (jl & 1) * C::TILE_BYTES;
-      for (int x = lane; x < n; x += 32) {
-        const int h = x / ((kTileRows - rows_valid) * 8), y = x % ((kTileRows - rows_valid) * 8);
-        *reinterpret_cast<uint4*>(vb + h * kHalfBytes + rows_valid * 128 + y * 16) = make_uint4(0, 0, 0, 0);
+      __syncwarp();
+    } else if (warp == 14) {
+      // ================================ V tail fixer ========================================================
+      for (int j = 0; j < n_kv; ++j) ptx::mbar_wait_sleep(bar(B_VFULL + (j & 1)), (j >> 1) & 1);
+      const int jl = n_kv - 1;
+      const int rows_valid = min(kTileRows, L - jl * kTileRows);
+      if (rows_valid < kTileRows) {
+        const int per_half = (kTileRows - rows_valid) * 8;          // 16-byte chunks to clear per column slab
+        const uint32_t vb = sV + (jl & 1) * C::TILE_BYTES + rows_valid * 128;
+        for (int x = lane; x < per_half * C::NH; x += 32)
+          ptx::sts128(vb + (x / per_half) * kHalfBytes + (x % per_half) * 16, make_uint4(0, 0, 0, 0));
       }
+      ptx::fence_proxy_async();
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(bar(B_VFIXED));
     }
-    ptx::fence_proxy_async();
-    __syncwarp();
-    if (lane == 0) ptx::mbar_arrive(bar(B_VFIXED));
-  } else if (warp >= 8 && warp < 12) {
-    // ================================ K-rotate warpgroup ====================================================
+  } else if (warp >= 8) {
+    // ================================ K-rotate warpgroup ======================================================
+    ptx::setmaxnreg_dec<kRegsRotate>();
     constexpr int TPP = 16 * C::CPR;                // threads per page
     constexpr int PPP = 128 / TPP;                  // pages per pass
     constexpr int PASSES = kPagesPerTile / PPP;
@@ -294,41 +330,35 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     for (int j = 0; j < n_kv; ++j) {
       const int s = j & 1;
       const int npv = min(kPagesPerTile, num_pages - j * kPagesPerTile);
-      int p0s[PASSES];
-#pragma unroll
-      for (int ps = 0; ps < PASSES; ++ps) {
-        const int i = ps * PPP + pp_;
-        p0s[ps] = (i < npv) ? ppos[j * kPagesPerTile + i] : 0;
-      }
-      float wc[2][8], ws[2][8];                     // e^{i p0 theta_j} of the page being / about to be rotated
-      load_cs8<D>(a.cs + (size_t)p0s[0] * (D / 2), c, wc[0], ws[0]);
+      const uint32_t kb = sK + s * C::TILE_BYTES;
+      const uint32_t cb = sCS + s * C::CS_STAGE_BYTES;
       ptx::mbar_wait(bar(B_KFULL + s), (j >> 1) & 1);
-      unsigned char* kb = smem + C::OFF_K + s * C::TILE_BYTES;
 #pragma unroll
       for (int ps = 0; ps < PASSES; ++ps) {
-        if (ps + 1 < PASSES) load_cs8<D>(a.cs + (size_t)p0s[ps + 1] * (D / 2), c, wc[(ps + 1) & 1], ws[(ps + 1) & 1]);
         const int i = ps * PPP + pp_;
         if (i < npv) {
-          float zc[8], zs[8];
+          float wc[8], ws[8], zc[8], zs[8];         // e^{i p0 theta_j} of the page, then e^{i (p0+t) theta_j}
+          load_cs8_smem<D>(cb + i * C::CS_ROW_BYTES, c, wc, ws);
+          const int row = i * kPageSize + t;
+          const uint32_t pa = kb + chunk_off(row, c), pb = kb + chunk_off(row, c + C::CPR);
+          uint4 va = ptx::lds128(pa), vb = ptx::lds128(pb);
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
-            zc[e] = wc[ps & 1][e] * uc[e] - ws[ps & 1][e] * us[e];
-            zs[e] = ws[ps & 1][e] * uc[e] + wc[ps & 1][e] * us[e];
+            zc[e] = wc[e] * uc[e] - ws[e] * us[e];
+            zs[e] = ws[e] * uc[e] + wc[e] * us[e];
           }
-          const int row = i * kPageSize + t;
-          uint4* pa = reinterpret_cast<uint4*>(kb + chunk_off(row, c));
-          uint4* pb = reinterpret_cast<uint4*>(kb + chunk_off(row, c + C::CPR));
-          uint4 va = *pa, vb = *pb;
-          rotate8(va, vb, zc, zs, 1.0f);
-          *pa = va; *pb = vb;
+          rotate8(va, vb, zc, zs);
+          ptx::sts128(pa, va);
+          ptx::sts128(pb, vb);
         }
       }
       ptx::fence_proxy_async();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(bar(B_KREADY + s));
     }
-  } else if (warp < 8) {
-    // ================================ softmax warpgroups ====================================================
+  } else {
+    // ================================ softmax warpgroups ======================================================
+    ptx::setmaxnreg_inc<kRegsSoftmax>();
     const int t = warp >> 2;
     const int row = tid - t * 128;
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
@@ -343,7 +373,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     // ---- Q tile: rotate by the query position, fold in log2(e)/sqrt(D), in place ----------------------------
     ptx::mbar_wait(bar(B_QFULL + t), 0);
     {
-      unsigned char* qb = smem + C::OFF_Q + t * C::TILE_BYTES;
+      const uint32_t qb = sQ + t * C::TILE_BYTES;
       if (valid) {
         const int pos = ppos[sq / kPageSize] + sq % kPageSize;
         const float2* cs_row = a.cs + (size_t)pos * (D / 2);
@@ -351,16 +381,17 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         for (int c = 0; c < C::CPR; ++c) {
           float co[8], si[8];
           load_cs8<D>(cs_row, c, co, si);
-          uint4* pa = reinterpret_cast<uint4*>(qb + chunk_off(row, c));
-          uint4* pb = reinterpret_cast<uint4*>(qb + chunk_off(row, c + C::CPR));
-          uint4 va = *pa, vb = *pb;
-          rotate8(va, vb, co, si, sh.scale_log2);
-          *pa = va; *pb = vb;
+#pragma unroll
+          for (int e = 0; e < 8; ++e) { co[e] *= sh.scale_log2; si[e] *= sh.scale_log2; }
+          const uint32_t pa = qb + chunk_off(row, c), pb = qb + chunk_off(row, c + C::CPR);
+          uint4 va = ptx::lds128(pa), vb = ptx::lds128(pb);
+          rotate8(va, vb, co, si);
+          ptx::sts128(pa, va);
+          ptx::sts128(pb, vb);
         }
       } else {
 #pragma unroll
-        for (int c = 0; c < 2 * C::CPR; ++c)
-          *reinterpret_cast<uint4*>(qb + chunk_off(row, c)) = make_uint4(0, 0, 0, 0);
+        for (int c = 0; c < 2 * C::CPR; ++c) ptx::sts128(qb + chunk_off(row, c), make_uint4(0, 0, 0, 0));
       }
     }
     ptx::fence_proxy_async();
@@ -369,24 +400,27 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 
     float m_used = -INFINITY, l_run = 0.f;
     for (int j = 0; j < n_kv; ++j) {
+      uint32_t sreg[128];                                     // this row of S (fp32 bits), later packed P
       ptx::mbar_wait(bar(B_SFULL + t), j & 1);
       ptx::tc_fence_after();
-      const int lim_col = lim_row - j * kTileRows;            // column visible iff col <= lim_col
-      const bool need_mask = j * kTileRows + kTileRows - 1 > lim_min;
-      float mx = -INFINITY;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        uint32_t rr[32];
-        ptx::tmem_ld32(tS + c * 32, rr);
-        ptx::tmem_wait_ld();
+      for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
+      ptx::tmem_wait_ld();
+      if (j * kTileRows + kTileRows - 1 > lim_min) {          // tile touches the causal edge / the tail: rare
+        const int lim_col = lim_row - j * kTileRows;          // column visible iff col <= lim_col
 #pragma unroll
-        for (int x = 0; x < 32; ++x) {
-          float v = __uint_as_float(rr[x]);
-          if (need_mask && c * 32 + x > lim_col) v = -INFINITY;
-          mx = fmaxf(mx, v);
-        }
+        for (int x = 0; x < 128; ++x)
+          if (x > lim_col) sreg[x] = 0xff800000u;             // -inf replaces the value (NaN-safe)
       }
-      const float m_new = fmaxf(m_used, mx);
+      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+      for (int x = 0; x < 128; x += 8) {
+        mx0 = fmaxf(fmaxf(mx0, f32(sreg[x + 0])), f32(sreg[x + 1]));
+        mx1 = fmaxf(fmaxf(mx1, f32(sreg[x + 2])), f32(sreg[x + 3]));
+        mx2 = fmaxf(fmaxf(mx2, f32(sreg[x + 4])), f32(sreg[x + 5]));
+        mx3 = fmaxf(fmaxf(mx3, f32(sreg[x + 6])), f32(sreg[x + 7]));
+      }
+      const float m_new = fmaxf(m_used, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
       if (j == 0) {
         m_used = m_new;
       } else {
@@ -395,34 +429,34 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
           const float f = grow ? ex2(m_used - m_new) : 1.f;
           if (grow) m_used = m_new;
           l_run *= f;
-#pragma unroll
-          for (int c = 0; c < D / 32; ++c) {
-            uint32_t rr[32];
-            ptx::tmem_ld32(tO + c * 32, rr);
+#pragma unroll 1
+          for (int c = 0; c < D / 16; ++c) {
+            uint32_t rr[16];
+            ptx::tmem_ld16(tO + c * 16, rr);
             ptx::tmem_wait_ld();
 #pragma unroll
-            for (int x = 0; x < 32; ++x) rr[x] = __float_as_uint(__uint_as_float(rr[x]) * f);
-            ptx::tmem_st32(tO + c * 32, rr);
+            for (int x = 0; x < 16; ++x) rr[x] = __float_as_uint(f32(rr[x]) * f);
+            ptx::tmem_st16(tO + c * 16, rr);
           }
           ptx::tmem_wait_st();
         }
       }
+      const float2 negm = make_float2(-m_used, -m_used);
+      float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        uint32_t rr[32], pk[16];
-        ptx::tmem_ld32(tS + c * 32, rr);
-        ptx::tmem_wait_ld();
-#pragma unroll
-        for (int x = 0; x < 16; ++x) {
-          float v0 = __uint_as_float(rr[2 * x]), v1 = __uint_as_float(rr[2 * x + 1]);
-          if (need_mask && c * 32 + 2 * x > lim_col) v0 = -INFINITY;
-          if (need_mask && c * 32 + 2 * x + 1 > lim_col) v1 = -INFINITY;
-          const float p0 = ex2(v0 - m_used), p1 = ex2(v1 - m_used);
-          l_run += p0 + p1;
-          pk[x] = ptx::pack_bf16(p0, p1);
-        }
-        ptx::tmem_st16(tS + c * 16, pk);                      // P over the already-consumed part of S
+      for (int x = 0; x < 64; x += 2) {
+        const float2 v0 = __fadd2_rn(make_float2(f32(sreg[2 * x]), f32(sreg[2 * x + 1])), negm);
+        const float2 v1 = __fadd2_rn(make_float2(f32(sreg[2 * x + 2]), f32(sreg[2 * x + 3])), negm);
+        const float2 p0 = make_float2(ex2(v0.x), ex2(v0.y));
+        const float2 p1 = make_float2(ex2(v1.x), ex2(v1.y));
+        sum0 = __fadd2_rn(sum0, p0);
+        sum1 = __fadd2_rn(sum1, p1);
+        sreg[x] = ptx::pack_bf16(p0.x, p0.y);
+        sreg[x + 1] = ptx::pack_bf16(p1.x, p1.y);
       }
+      l_run += (sum0.x + sum0.y) + (sum1.x + sum1.y);
+      ptx::tmem_st32(tS, sreg);                               // P (bf16 pairs) over the first 64 columns of S
+      ptx::tmem_st32(tS + 32, sreg + 32);
       ptx::tmem_wait_st();
       ptx::tc_fence_before();
       __syncwarp();
@@ -443,10 +477,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 #pragma unroll
         for (int x = 0; x < 4; ++x) {
           uint4 o;
-          o.x = ptx::pack_bf16(__uint_as_float(rr[8 * x + 0]) * inv, __uint_as_float(rr[8 * x + 1]) * inv);
-          o.y = ptx::pack_bf16(__uint_as_float(rr[8 * x + 2]) * inv, __uint_as_float(rr[8 * x + 3]) * inv);
-          o.z = ptx::pack_bf16(__uint_as_float(rr[8 * x + 4]) * inv, __uint_as_float(rr[8 * x + 5]) * inv);
-          o.w = ptx::pack_bf16(__uint_as_float(rr[8 * x + 6]) * inv, __uint_as_float(rr[8 * x + 7]) * inv);
+          o.x = ptx::pack_bf16(f32(rr[8 * x + 0]) * inv, f32(rr[8 * x + 1]) * inv);
+          o.y = ptx::pack_bf16(f32(rr[8 * x + 2]) * inv, f32(rr[8 * x + 3]) * inv);
+          o.z = ptx::pack_bf16(f32(rr[8 * x + 4]) * inv, f32(rr[8 * x + 5]) * inv);
+          o.w = ptx::pack_bf16(f32(rr[8 * x + 6]) * inv, f32(rr[8 * x + 7]) * inv);
           reinterpret_cast<uint4*>(orow + c * 32)[x] = o;
         }
       }
