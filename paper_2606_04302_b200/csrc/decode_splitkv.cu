@@ -218,7 +218,7 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
   const int hl = warp % HKV_CTA;                    // kv head within the CTA's head group
   const int hk = hg * HKV_CTA + hl;
   const int group = sh.group;
-  const float4* ctab = reinterpret_cast<const float4*>(smem + C::OFF_CTAB);
+  const uint32_t ctab_u32 = smem_base + C::OFF_CTAB + lane * 16;   // explicit ld.shared: generic LD costs a long scoreboard
 
   int r = r0, u = u_begin, it = 0;
   while (u < u_end) {
@@ -256,8 +256,8 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
       const int p = ul * C::PPS + pl;
       const int nv = min(kPageSize, L - p * kPageSize);      // valid tokens of this page (<= 0: no page)
       if (nv > 0) {
-        unsigned char* st = smem + stage * C::STAGE_BYTES;
-        const int delta = reinterpret_cast<const int*>(st + C::OFF_META)[pl];
+        const uint32_t st = smem_base + stage * C::STAGE_BYTES;
+        const int delta = ptx::lds32(st + C::OFF_META + pl * 4);
         // ---- K tile -> registers (rows g, g+8 of head hl; this thread's JT dims of each half)
         uint32_t kreg[2][2][C::NL];                 // [half][row][word]
         const int R0 = hl * 16 + g;
@@ -269,20 +269,19 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
             for (int x = 0; x < C::NLK; ++x) {
               int d = h * (D / 2) + C::JT * tq + 8 * x;
               int Rr = R0 + 8 * rw;
-              const unsigned char* ptr = st + pl * C::PAGE_BYTES + (d / 64) * C::BOX_BYTES + Rr * 128 +
-                                         ((((d % 64) / 8) ^ (Rr & 7)) * 16);
-              uint4 v = *reinterpret_cast<const uint4*>(ptr);
+              const uint4 v = ptx::lds128(st + pl * C::PAGE_BYTES + (d / 64) * C::BOX_BYTES + Rr * 128 +
+                                          ((((d % 64) / 8) ^ (Rr & 7)) * 16));
               kreg[h][rw][4 * x + 0] = v.x; kreg[h][rw][4 * x + 1] = v.y;
               kreg[h][rw][4 * x + 2] = v.z; kreg[h][rw][4 * x + 3] = v.w;
             }
         // ---- q re-rotated for this page: Qhat = R_{m - p0} q   (a3/a4; one cos/sin row per page)
         uint32_t qhat[2][C::NL];
         {
-          const float4* qcs = reinterpret_cast<const float4*>(st + C::OFF_CS + pl * C::CS_ROW_BYTES);
+          const uint32_t qcs = st + C::OFF_CS + pl * C::CS_ROW_BYTES + tq * 16;
           const float sgn = delta < 0 ? -1.f : 1.f;
 #pragma unroll
           for (int w = 0; w < C::NL; ++w) {
-            float4 c = qcs[w * 4 + tq];
+            float4 c = ptx::lds128f(qcs + w * 64);
             c.y *= sgn; c.w *= sgn;
             float a_lo = ptx::bf16_lo(qraw[0][w]), a_hi = ptx::bf16_hi(qraw[0][w]);
             float b_lo = ptx::bf16_lo(qraw[1][w]), b_hi = ptx::bf16_hi(qraw[1][w]);
@@ -295,20 +294,23 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
         for (int rw = 0; rw < 2; ++rw)
 #pragma unroll
           for (int w = 0; w < C::NL; ++w) {
-            float4 c = ctab[(rw * C::NL + w) * 32 + lane];
+            const float4 c = ptx::lds128f(ctab_u32 + (rw * C::NL + w) * 512);
             float a_lo = ptx::bf16_lo(kreg[0][rw][w]), a_hi = ptx::bf16_hi(kreg[0][rw][w]);
             float b_lo = ptx::bf16_lo(kreg[1][rw][w]), b_hi = ptx::bf16_hi(kreg[1][rw][w]);
             kreg[0][rw][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
             kreg[1][rw][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
           }
         // ---- S = Khat Qhat^T : rows = tokens (g, g+8), cols = heads (2tq, 2tq+1)
-        float s[4] = {0.f, 0.f, 0.f, 0.f};
+        float s[4] = {0.f, 0.f, 0.f, 0.f}, s_b[4] = {0.f, 0.f, 0.f, 0.f};   // two chains: halves the MMA latency chain
 #pragma unroll
-        for (int c = 0; c < C::NC; ++c) {
-          const int h = c / (C::NC / 2), cc = c % (C::NC / 2);
-          ptx::mma_bf16_16816(s, kreg[h][0][2 * cc], kreg[h][1][2 * cc], kreg[h][0][2 * cc + 1],
-                              kreg[h][1][2 * cc + 1], qhat[h][2 * cc], qhat[h][2 * cc + 1]);
+        for (int cc = 0; cc < C::NC / 2; ++cc) {
+          ptx::mma_bf16_16816(s, kreg[0][0][2 * cc], kreg[0][1][2 * cc], kreg[0][0][2 * cc + 1],
+                              kreg[0][1][2 * cc + 1], qhat[0][2 * cc], qhat[0][2 * cc + 1]);
+          ptx::mma_bf16_16816(s_b, kreg[1][0][2 * cc], kreg[1][1][2 * cc], kreg[1][0][2 * cc + 1],
+                              kreg[1][1][2 * cc + 1], qhat[1][2 * cc], qhat[1][2 * cc + 1]);
         }
+#pragma unroll
+        for (int x = 0; x < 4; ++x) s[x] += s_b[x];
         if (g >= nv) { s[0] = -INFINITY; s[1] = -INFINITY; }
         if (g + 8 >= nv) { s[2] = -INFINITY; s[3] = -INFINITY; }
         // ---- online softmax over the 16 tokens (a6): max across the 8 row-lanes with shuffles
@@ -319,16 +321,19 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
           mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, o));
         }
         const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);   // finite: token 0 is valid
-        const float corr0 = exp2f(m_run[0] - mn0), corr1 = exp2f(m_run[1] - mn1);
-        m_run[0] = mn0; m_run[1] = mn1;
+        if (__any_sync(0xffffffffu, mn0 > m_run[0] || mn1 > m_run[1])) {      // rare after the first pages
+          const float corr0 = exp2f(m_run[0] - mn0), corr1 = exp2f(m_run[1] - mn1);
+          m_run[0] = mn0; m_run[1] = mn1;
+          l_run[0] *= corr0; l_run[1] *= corr1;
+#pragma unroll
+          for (int i = 0; i < C::NC; ++i) {
+            oacc[i][0] *= corr0; oacc[i][1] *= corr1; oacc[i][2] *= corr0; oacc[i][3] *= corr1;
+          }
+        }
         const float p0 = exp2f(s[0] - mn0), p1 = exp2f(s[1] - mn1);
         const float p2 = exp2f(s[2] - mn0), p3 = exp2f(s[3] - mn1);
-        l_run[0] = l_run[0] * corr0 + p0 + p2;
-        l_run[1] = l_run[1] * corr1 + p1 + p3;
-#pragma unroll
-        for (int i = 0; i < C::NC; ++i) {
-          oacc[i][0] *= corr0; oacc[i][1] *= corr1; oacc[i][2] *= corr0; oacc[i][3] *= corr1;
-        }
+        l_run[0] += p0 + p2;
+        l_run[1] += p1 + p3;
         // ---- P (bf16) transposed into the B-fragment layout: k = tokens, n = heads
         const uint32_t pb0 = ptx::movmatrix_trans(ptx::pack_bf16(p0, p1));
         const uint32_t pb1 = ptx::movmatrix_trans(ptx::pack_bf16(p2, p3));
