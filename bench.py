@@ -36,6 +36,19 @@ def load_peaks():
     return dict(hbm=6650.0, tensor=1590.0, tensor_sustained=1400.0, source="fallback")
 
 
+def ncu_traffic(kernel: str, workload: str):
+    """dram read + write bytes per launch of the dominant kernel from the committed ncu --set full capture
+    (profiles/*_traffic.csv, latest round wins); None when that workload has not been captured."""
+    import csv
+    import glob
+    val = None
+    for f in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv"))):
+        for row in csv.DictReader(open(f)):
+            if row["kernel"] == kernel and row["workload"] == workload:
+                val = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+    return val
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
@@ -403,20 +416,26 @@ def main():
     _, e2e1, _ = headline(args.workload, work, e2e_ms)
     value, e2e_value = value1 * world, e2e1 * world           # whole-job aggregate (weak scaling: same work per rank)
 
+    wl_name = args.workload + ("_noshare" if args.noshare else "")
     if args.workload in ("cfg2", "cfg4", "cfg5"):
         ach = work["logical_bytes"] / (ms_attn * 1e-3) / 1e9 if args.workload != "cfg5" else None
     roof = None
     if args.workload in ("cfg2", "cfg4"):
         ub = unique_bytes(batch, [r["step"] for r in job.timed])
         roof = {"bound": "hbm", "kernel": "lazy_attn_decode (split-KV + combine)", "achieved": ach,
-                "peak": peaks["hbm"], "unit": "GB/s", "frac": ach / peaks["hbm"], "traffic": None,
+                "peak": peaks["hbm"], "unit": "GB/s", "frac": ach / peaks["hbm"],
+                "traffic": ncu_traffic("decode", wl_name),
+                "note": ("algorithmic bytes = K and V once per (token, kv head) per request; with Zipf page sharing the "
+                         "L2 serves repeats, so achieved can exceed the HBM peak -- the HBM-bound fraction is the "
+                         "noshare variant's (logical == unique == DRAM bytes), reported under decode_noshare"),
                 "peak_source": peaks["source"], "algorithmic_bytes_per_launch": work["logical_bytes"],
                 "unique_bytes_per_launch": ub, "achieved_unique": ub / (ms_attn * 1e-3) / 1e9,
                 "kernel_ms": ms_attn}
     elif args.workload == "cfg3":
         ach = work["flops"] / (ms_attn * 1e-3) / 1e12
         roof = {"bound": "tensor", "kernel": "lazy_attn_prefill", "achieved": ach, "peak": peaks["tensor"],
-                "unit": "TFLOP/s", "frac": ach / peaks["tensor"], "traffic": None, "peak_source": peaks["source"],
+                "unit": "TFLOP/s", "frac": ach / peaks["tensor"], "traffic": ncu_traffic("prefill", wl_name),
+                "peak_source": peaks["source"],
                 "algorithmic_flops_per_launch": work["flops"], "kernel_ms": ms_attn}
     else:
         roof = {"bound": "hbm", "kernel": "mixed step (prefill + decode)", "achieved": None, "peak": peaks["hbm"],
