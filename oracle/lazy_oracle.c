@@ -140,11 +140,39 @@ int lazy_oracle_attend_core(const double* q, const double* k, const double* v,
  *   out [total_q][Hq][D] double.  row_select optional [total_q] (0 = skip row, left untouched).
  * Rows of requests with seq_len == 0 are written as zeros.
  */
+int lazy_oracle_attend_paged_stored(const void* q, int dtype_q, const void* k_pool, const void* v_pool,
+                                    int dtype_kv, const int32_t* block_table, const int32_t* page_logical_pos,
+                                    int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
+                                    int num_reqs, int Hq, int Hkv, int D, int P, double theta,
+                                    int k_storage, const int32_t* page_stored_pos,
+                                    const uint8_t* row_select, double* out);
+
 int lazy_oracle_attend_paged(const void* q, int dtype_q, const void* k_pool, const void* v_pool, int dtype_kv,
                              const int32_t* block_table, const int32_t* page_logical_pos, int64_t table_stride,
                              const int32_t* seq_lens, const int32_t* cu_q_lens, int num_reqs,
                              int Hq, int Hkv, int D, int P, double theta,
                              const uint8_t* row_select, double* out) {
+    return lazy_oracle_attend_paged_stored(q, dtype_q, k_pool, v_pool, dtype_kv, block_table, page_logical_pos,
+                                           table_stride, seq_lens, cu_q_lens, num_reqs, Hq, Hkv, D, P, theta,
+                                           0, NULL, row_select, out);
+}
+
+/* Same call for the three ways a page's K can be STORED:
+ *   k_storage 0  un-rotated (north_star): key s is rotated by its logical position;
+ *   k_storage 1  the paper's own layout ("local position ... indexing from 0", L409): token t of
+ *                physical page g was stored rotated by page_stored_pos[g] + t, so reaching logical position
+ *                page_logical_pos + t needs ONE relative rotation by D = page_logical_pos - page_stored_pos[g]
+ *                for the whole page (R_{p+D} = R_D R_p);
+ *   k_storage 2  position-dependent cache (the standard-attention baseline of PAPER.md Fig. 5 / Table 12):
+ *                K is stored already rotated at its final position, no rotation is left to do.
+ * In every mode q is rotated by the logical position of its own token and the rest is Eq. 4. */
+int lazy_oracle_attend_paged_stored(const void* q, int dtype_q, const void* k_pool, const void* v_pool,
+                                    int dtype_kv, const int32_t* block_table, const int32_t* page_logical_pos,
+                                    int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
+                                    int num_reqs, int Hq, int Hkv, int D, int P, double theta,
+                                    int k_storage, const int32_t* page_stored_pos,
+                                    const uint8_t* row_select, double* out) {
+    if (k_storage < 0 || k_storage > 2 || (k_storage == 1 && !page_stored_pos)) return -1;
     for (int r = 0; r < num_reqs; ++r) {
         int64_t L = seq_lens[r];
         int q0 = cu_q_lens[r], n_q = cu_q_lens[r + 1] - cu_q_lens[r];
@@ -162,16 +190,21 @@ int lazy_oracle_attend_paged(const void* q, int dtype_q, const void* k_pool, con
         double* kg = (double*)malloc(sizeof(double) * (size_t)L * Hkv * D);
         double* vg = (double*)malloc(sizeof(double) * (size_t)L * Hkv * D);
         double* pos = (double*)malloc(sizeof(double) * (size_t)L);
+        double* rot = (double*)malloc(sizeof(double) * (size_t)L);   /* rotation still owed to key s */
         double* qd = (double*)malloc(sizeof(double) * (size_t)n_q * Hq * D);
         double* pos_q = (double*)malloc(sizeof(double) * (size_t)n_q);
         int64_t* vis = (int64_t*)malloc(sizeof(int64_t) * (size_t)n_q);
-        if (!kg || !vg || !pos || !qd || !pos_q || !vis) return -2;
+        if (!kg || !vg || !pos || !rot || !qd || !pos_q || !vis) return -2;
         /* gather the request's rows through the block table */
 #pragma omp parallel for schedule(static)
         for (int64_t s = 0; s < L; ++s) {
             int64_t slot = s / P, t = s % P;
             int64_t page = block_table[(size_t)r * table_stride + slot];
             pos[s] = (double)page_logical_pos[(size_t)r * table_stride + slot] + (double)t;
+            if (k_storage == 0) rot[s] = pos[s];
+            else if (k_storage == 1)
+                rot[s] = (double)page_logical_pos[(size_t)r * table_stride + slot] - (double)page_stored_pos[page];
+            else rot[s] = 0.0;
             for (int hk = 0; hk < Hkv; ++hk) {
                 int64_t base = (((int64_t)page * Hkv + hk) * P + t) * D;
                 for (int d = 0; d < D; ++d) {
@@ -186,10 +219,10 @@ int lazy_oracle_attend_paged(const void* q, int dtype_q, const void* k_pool, con
             vis[i] = sq;
             pos_q[i] = pos[sq];
         }
-        int rc = lazy_oracle_attend_core(qd, kg, vg, pos_q, pos, vis, n_q, L, Hq, Hkv, D, theta,
+        int rc = lazy_oracle_attend_core(qd, kg, vg, pos_q, rot, vis, n_q, L, Hq, Hkv, D, theta,
                                          row_select ? row_select + q0 : NULL,
                                          out + (size_t)q0 * Hq * D, NULL, NULL, NULL);
-        free(kg); free(vg); free(pos); free(qd); free(pos_q); free(vis);
+        free(kg); free(vg); free(pos); free(rot); free(qd); free(pos_q); free(vis);
         if (rc) return rc;
     }
     return 0;
@@ -213,6 +246,29 @@ int lazy_oracle_cache_write(const uint16_t* k_new, const uint16_t* v_new, const 
             memcpy(v_pool + dst, v_new + src, sizeof(uint16_t) * D);
         }
     }
+    return 0;
+}
+
+/* Materialising re-encoding of whole pages -- what position-dependent caches do on a position mismatch
+ * ("allocate + copy + rotate", App. B) and what LazyAttention avoids.  For i < num:
+ *   out[i][hk][t][:] = rope(K[src_pages[i]][hk][t][:], rot_pos[i] + (per_token ? t : 0))
+ * per_token = 1 encodes an un-rotated page at logical start rot_pos[i]; per_token = 0 applies one relative
+ * rotation D = rot_pos[i] (may be negative) to a page that already carries positions.
+ * out is fp64 [num][Hkv][P][D]; the CUDA call rounds the same quantity to bf16. */
+int lazy_oracle_materialize_pages(const void* k_pool, int dtype_kv, const int32_t* src_pages,
+                                  const int32_t* rot_pos, int per_token, int64_t num,
+                                  int Hkv, int D, int P, double theta, double* out) {
+    double* x = (double*)malloc(sizeof(double) * D);
+    if (!x) return -2;
+    for (int64_t i = 0; i < num; ++i)
+        for (int hk = 0; hk < Hkv; ++hk)
+            for (int t = 0; t < P; ++t) {
+                int64_t base = (((int64_t)src_pages[i] * Hkv + hk) * P + t) * D;
+                for (int d = 0; d < D; ++d) x[d] = load_elem(k_pool, dtype_kv, base + d);
+                lazy_oracle_rope(x, (double)rot_pos[i] + (per_token ? (double)t : 0.0), D, theta,
+                                 out + ((((size_t)i * Hkv + hk) * P) + t) * D);
+            }
+    free(x);
     return 0;
 }
 

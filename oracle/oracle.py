@@ -98,8 +98,10 @@ def attend_core(q, k, v, pos_q, pos_k, vis, theta: float, row_select=None, want_
 
 def attend_paged(q, k_pool, v_pool, block_table, page_logical_pos, seq_lens, cu_q_lens, *,
                  num_q_heads: int, num_kv_heads: int, head_dim: int, page_size: int, theta: float,
-                 row_select=None) -> np.ndarray:
+                 row_select=None, k_storage: int = 0, page_stored_pos=None) -> np.ndarray:
     """Paged interface.  q [total_q,Hq,D]; pools [num_pages,Hkv,P,D] (torch bf16 or float arrays).
+    k_storage 0: pages hold un-rotated K; 1: page g holds K rotated at page_stored_pos[g] + t (the paper's
+    document-local layout); 2: K already rotated at its final position.
     Returns out [total_q,Hq,D] float64 (rows not selected stay 0)."""
     qa, dq = _as_kernel_input(q)
     ka, dk = _as_kernel_input(k_pool)
@@ -114,14 +116,33 @@ def attend_paged(q, k_pool, v_pool, block_table, page_logical_pos, seq_lens, cu_
     total_q = int(cu[-1])
     out = np.zeros((total_q, num_q_heads, head_dim), dtype=np.float64)
     rs = None if row_select is None else np.ascontiguousarray(np.asarray(row_select, dtype=np.uint8))
-    f = lib().lazy_oracle_attend_paged
+    sp = None if page_stored_pos is None else np.ascontiguousarray(np.asarray(page_stored_pos, dtype=np.int32))
+    f = lib().lazy_oracle_attend_paged_stored
     f.restype = ctypes.c_int
     rc = f(_p(qa), ctypes.c_int(dq), _p(ka), _p(va), ctypes.c_int(dk), _p(bt), _p(pp),
            ctypes.c_int64(bt.shape[1]), _p(sl), _p(cu), ctypes.c_int(R), ctypes.c_int(num_q_heads),
            ctypes.c_int(num_kv_heads), ctypes.c_int(head_dim), ctypes.c_int(page_size), ctypes.c_double(theta),
-           _p(rs), _p(out))
+           ctypes.c_int(k_storage), _p(sp), _p(rs), _p(out))
     if rc != 0:
-        raise RuntimeError(f"lazy_oracle_attend_paged failed: {rc}")
+        raise RuntimeError(f"lazy_oracle_attend_paged_stored failed: {rc}")
+    return out
+
+
+def materialize_pages(k_pool, src_pages, rot_pos, per_token: bool, theta: float) -> np.ndarray:
+    """fp64 [num,Hkv,P,D]: page src_pages[i] rotated by rot_pos[i] (+ t if per_token)."""
+    ka, dk = _as_kernel_input(k_pool)
+    _, Hkv, P, D = ka.shape
+    sp = np.ascontiguousarray(np.asarray(src_pages, dtype=np.int32))
+    rp = np.ascontiguousarray(np.asarray(rot_pos, dtype=np.int32))
+    assert sp.shape == rp.shape and sp.ndim == 1
+    out = np.zeros((sp.shape[0], Hkv, P, D), dtype=np.float64)
+    f = lib().lazy_oracle_materialize_pages
+    f.restype = ctypes.c_int
+    rc = f(_p(ka), ctypes.c_int(dk), _p(sp), _p(rp), ctypes.c_int(1 if per_token else 0),
+           ctypes.c_int64(sp.shape[0]), ctypes.c_int(Hkv), ctypes.c_int(D), ctypes.c_int(P), ctypes.c_double(theta),
+           _p(out))
+    if rc != 0:
+        raise RuntimeError(f"lazy_oracle_materialize_pages failed: {rc}")
     return out
 
 

@@ -379,3 +379,75 @@ def test_long_position_numerics_stateless():
     out = oracle.attend_core(q, k, v, [131071.0], pos_k, [L - 1], 5e5)
     ref, _ = brute_force(q, k, v, np.array([131071.0]), pos_k, np.array([L - 1]), 5e5)
     assert np.abs(out - ref).max() < 1e-9
+
+
+# ---- stored-position layouts and the materialising re-encoding -----------------------
+def _np_rope_pool(kp, start_of_page, theta, per_token=True):
+    """Independent numpy statement of PAPER.md L164-166 on a whole pool [pages,Hkv,P,D]: token t of page g is
+    rotated by start_of_page[g] (+ t), pair (j, j + D/2), angle * theta^(-2j/D)."""
+    g, Hkv, P, D = kp.shape
+    h = D // 2
+    inv = theta ** (-2.0 * np.arange(h) / D)
+    pos = np.asarray(start_of_page, dtype=np.float64)[:, None] + (np.arange(P)[None, :] if per_token else 0.0)
+    ang = pos[:, None, :, None] * inv[None, None, None, :]                     # [g,1,P,h]
+    c, s = np.cos(ang), np.sin(ang)
+    x1, x2 = kp[..., :h], kp[..., h:]
+    return np.concatenate([x1 * c - x2 * s, x1 * s + x2 * c], axis=-1)
+
+
+def test_materialize_closed_form_group_property_and_norm():
+    """f2: re-encoding a page is a rotation: closed form on one-hot rows (cos / sin of (p+t)*theta_j), R_a R_b =
+    R_{a+b} (a cached page moves by one relative rotation), R_{-a} undoes R_a, norms kept."""
+    P, D, Hkv, theta = 4, 8, 2, 1e4
+    h = D // 2
+    kp = np.zeros((3, Hkv, P, D))
+    kp[1, :, :, 2] = 1.0                                    # e_2 in every row of page 1
+    out = oracle.materialize_pages(kp, [1], [37], True, theta)
+    for t in range(P):
+        a = (37 + t) * theta ** (-2.0 * 2 / D)
+        expect = np.zeros(D); expect[2] = math.cos(a); expect[2 + h] = math.sin(a)
+        assert np.abs(out[0, :, t] - expect).max() < 1e-14
+    r = _rng(61)
+    kp = r.standard_normal((5, Hkv, P, D))
+    a = oracle.materialize_pages(kp, [3, 0, 3], [100, 7, 0], True, theta)      # page 3 twice, two positions
+    assert np.abs(a - _np_rope_pool(kp[[3, 0, 3]], [100, 7, 0], theta)).max() < 1e-12
+    b = oracle.materialize_pages(a, [0, 1, 2], [23, -7, 500], False, theta)    # one relative rotation per page
+    c = oracle.materialize_pages(kp, [3, 0, 3], [123, 0, 500], True, theta)
+    assert np.abs(b - c).max() < 1e-11
+    back = oracle.materialize_pages(b, [0, 1, 2], [-23, 7, -500], False, theta)
+    assert np.abs(back - a).max() < 1e-11
+    assert np.abs(np.linalg.norm(a, axis=-1) - np.linalg.norm(kp[[3, 0, 3]], axis=-1)).max() < 1e-12
+
+
+def test_stored_position_layouts_equal_unrotated_cache():
+    """f1 (PAPER.md L37 'mathematically identical'; L173 document-local cache + one offset per document; L409):
+    attention over (i) un-rotated pages, (ii) pages stored rotated at a page-local position and moved by one
+    relative rotation, (iii) private copies already rotated at their final positions -- all the same numbers.
+    The pre-rotated pools are built by the independent numpy statement above, not by the oracle."""
+    r = _rng(67)
+    Hq, Hkv, D, P, theta = 4, 2, 8, 4, 5e5
+    num_pages = 7
+    kp = r.standard_normal((num_pages, Hkv, P, D)); vp = r.standard_normal((num_pages, Hkv, P, D))
+    bt = np.array([[5, 2, 6, 2, 0], [1, 2, 3, 0, 0]], np.int32)                # page 2 shared, twice in request 0
+    pp = np.array([[0, 4, 40, 44, 48], [100, 104, 108, 0, 0]], np.int32)
+    sl = np.array([18, 10], np.int32); cu = np.array([0, 3, 5], np.int32)
+    q = r.standard_normal((5, Hq, D))
+    kw = dict(num_q_heads=Hq, num_kv_heads=Hkv, head_dim=D, page_size=P, theta=theta)
+    base = oracle.attend_paged(q, kp, vp, bt, pp, sl, cu, **kw)
+    # (ii) document-local storage: stored start of every physical page, incl. one larger than its logical start
+    stored = np.array([0, 4, 8, 12, 0, 60, 16], np.int32)
+    kp_local = _np_rope_pool(kp, stored, theta)
+    got = oracle.attend_paged(q, kp_local, vp, bt, pp, sl, cu, k_storage=1, page_stored_pos=stored, **kw)
+    assert np.abs(got - base).max() < 1e-10
+    # a wrong sign of the relative rotation must be visible
+    bad = oracle.attend_paged(q, kp_local, vp, bt, pp, sl, cu, k_storage=1, page_stored_pos=-stored, **kw)
+    assert np.abs(bad - base).max() > 1e-3
+    # (iii) private absolute copies: every (request, slot) gets its own physical page
+    n_slots = bt.shape[1]
+    src = bt.reshape(-1); starts = pp.reshape(-1)
+    kp_abs = _np_rope_pool(kp[src], starts, theta); vp_abs = vp[src]
+    bt_abs = np.arange(2 * n_slots, dtype=np.int32).reshape(2, n_slots)
+    got = oracle.attend_paged(q, kp_abs, vp_abs, bt_abs, pp, sl, cu, k_storage=2, **kw)
+    assert np.abs(got - base).max() < 1e-10
+    # and the oracle's own materialiser builds exactly those copies
+    assert np.abs(oracle.materialize_pages(kp, src, starts, True, theta) - kp_abs).max() < 1e-12
