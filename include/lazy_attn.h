@@ -61,8 +61,24 @@ typedef struct lazy_config {
   int32_t rope_style;        /* 0 = half-split (the only style)                                 */
   int32_t dtype;             /* 0 = bf16 (the only dtype)                                       */
   int32_t flags;             /* LAZY_FLAG_* (0 for production)                                  */
-  int32_t reserved;
+  int32_t k_storage;         /* LAZY_K_* : how the pages hold K (0 = un-rotated, the product)    */
 } lazy_config;
+
+/* k_storage: what a physical page's K rows carry (V is position-free in every mode).
+ *   LAZY_K_UNROTATED  the product path (north_star): K is the projection output, the kernels
+ *                     rotate token t of a page by page_logical_pos + t.
+ *   LAZY_K_STORED_POS the paper's own layout ("local position ... indexing from 0", L409): token
+ *                     t of physical page g was stored rotated by page_stored_pos[g] + t
+ *                     (lazy_set_page_stored_pos); the kernels apply ONE relative rotation per page by
+ *                     D = page_logical_pos - page_stored_pos[g] -- to the K tile in prefill (Eq. 5),
+ *                     to q in decode (Eq. 6).  |D| and every position must be < max_position.
+ *   LAZY_K_ABSOLUTE   position-dependent cache (standard attention, the "without deferred rotation" arm of
+ *                     PAPER.md Fig. 5 / L271-297): K is stored rotated at its final position, nothing is
+ *                     rotated but q (by the position of its own token).  Pages cannot be shared across
+ *                     positions in this mode; it exists to measure what the rotation costs. */
+#define LAZY_K_UNROTATED  0
+#define LAZY_K_STORED_POS 1
+#define LAZY_K_ABSOLUTE   2
 
 /* flags: debugging aids, never set by bench.py */
 #define LAZY_FLAG_ROWWISE_KERNELS 1  /* run the simple one-row-per-CTA CUDA kernels for prefill and decode */
@@ -114,6 +130,27 @@ int lazy_attn_prefill(lazy_handle* h, const void* q, const void* k_cache, const 
 int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                      const int32_t* block_table, const int32_t* page_logical_pos,
                      const int32_t* seq_lens, int32_t num_reqs, void* out, void* stream);
+
+/* LAZY_K_STORED_POS only: device array [num_pages] int32, position at which token 0 of each physical page
+ * was rotated when it was stored.  The pointer is kept (not copied) and read by every later attention call;
+ * it must stay valid until lazy_destroy or the next lazy_set_page_stored_pos.  Host-side, no launch. */
+int lazy_set_page_stored_pos(lazy_handle* h, const int32_t* page_stored_pos);
+
+/* f2. Materialising re-encoding of whole pages: what a position-dependent cache does on a position mismatch
+ * ("allocate + copy + rotate", App. B; "read-modify-write ... doubling HBM traffic", L447) and
+ * what the lazy path avoids.  It is also the writer for the LAZY_K_STORED_POS / LAZY_K_ABSOLUTE layouts.
+ * For i < num, every kv head, token t < page_size:
+ *     k_dst[dst_pages[i]][hk][t][:] = bf16( RoPE(k_src[src_pages[i]][hk][t][:], rot_pos[i] + (per_token ? t : 0)) )
+ *     v_dst[dst_pages[i]][hk][t][:] = v_src[src_pages[i]][hk][t][:]          (skipped if v_src or v_dst is NULL)
+ * per_token = 1 encodes an un-rotated page at logical start rot_pos[i] >= 0; per_token = 0 applies one
+ * relative rotation rot_pos[i] (may be negative) to a page that already carries positions.
+ *   src_pages, dst_pages, rot_pos : device int32 [num];  |rot_pos[i]| + page_size <= max_position.
+ * Source and destination pools have the pool layout; they may be the same pool (dst_pages[i] == src_pages[i]
+ * re-encodes in place: the in-place update that races under sharing).  Destination pages must be
+ * distinct.  fp32 rotation from the fp64-built table, one rounding to bf16.  num == 0 -> no launch. */
+int lazy_materialize_pages(lazy_handle* h, const void* k_src, const void* v_src, const int32_t* src_pages,
+                           const int32_t* rot_pos, int32_t per_token, void* k_dst, void* v_dst,
+                           const int32_t* dst_pages, int32_t num, void* stream);
 
 /* Static description of a status code (host string, never NULL). */
 const char* lazy_status_string(int status);

@@ -15,9 +15,10 @@ LIB_PATH = os.path.join(_HERE, "csrc", "liblazyattn.so")
 
 LAZY_OK, LAZY_ERR_INVALID, LAZY_ERR_UNSUPPORTED, LAZY_ERR_WORKSPACE, LAZY_ERR_CUDA = 0, -1, -2, -3, -4
 LAZY_FLAG_ROWWISE_KERNELS = 1
+LAZY_K_UNROTATED, LAZY_K_STORED_POS, LAZY_K_ABSOLUTE = 0, 1, 2
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
-           "lazy_attn_decode", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step"]
+           "lazy_attn_decode", "lazy_set_page_stored_pos", "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step"]
 
 
 class LazyConfig(ctypes.Structure):
@@ -25,7 +26,7 @@ class LazyConfig(ctypes.Structure):
                 ("page_size", ctypes.c_int32), ("num_pages", ctypes.c_int32), ("max_position", ctypes.c_int32),
                 ("max_reqs", ctypes.c_int32), ("max_pages_per_req", ctypes.c_int32),
                 ("rope_theta", ctypes.c_double), ("rope_style", ctypes.c_int32), ("dtype", ctypes.c_int32),
-                ("flags", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("flags", ctypes.c_int32), ("k_storage", ctypes.c_int32)]
 
 
 _lib: Optional[ctypes.CDLL] = None
@@ -52,6 +53,10 @@ def lib() -> ctypes.CDLL:
         L.lazy_attn_prefill.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, vp]
         L.lazy_attn_decode.restype = ctypes.c_int
         L.lazy_attn_decode.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, vp, vp]
+        L.lazy_set_page_stored_pos.restype = ctypes.c_int
+        L.lazy_set_page_stored_pos.argtypes = [vp, vp]
+        L.lazy_materialize_pages.restype = ctypes.c_int
+        L.lazy_materialize_pages.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, vp, i32, vp]
         L.lazy_status_string.restype = ctypes.c_char_p
         L.lazy_status_string.argtypes = [ctypes.c_int]
         L.lazy_launch_count.restype = i64
@@ -127,9 +132,9 @@ class LazyHandle:
 
 def lazy_create(num_q_heads: int, num_kv_heads: int, head_dim: int, *, num_pages: int, max_position: int,
                 max_reqs: int, max_pages_per_req: int, rope_theta: float, page_size: int = 16, flags: int = 0,
-                device="cuda", stream=None) -> LazyHandle:
+                k_storage: int = LAZY_K_UNROTATED, device="cuda", stream=None) -> LazyHandle:
     cfg = LazyConfig(num_q_heads, num_kv_heads, head_dim, page_size, num_pages, max_position, max_reqs,
-                     max_pages_per_req, float(rope_theta), 0, 0, flags, 0)
+                     max_pages_per_req, float(rope_theta), 0, 0, flags, k_storage)
     return LazyHandle(cfg, device=device, stream=stream)
 
 
@@ -163,6 +168,23 @@ def lazy_attn_decode(h: LazyHandle, q, k_cache, v_cache, block_table, page_logic
                                 _ptr(page_logical_pos), _ptr(seq_lens), num_reqs, _ptr(out), _stream(stream))
     if rc != 0:
         raise LazyError("lazy_attn_decode", rc)
+
+
+def lazy_set_page_stored_pos(h: LazyHandle, page_stored_pos) -> None:
+    rc = lib().lazy_set_page_stored_pos(h.ptr, _ptr(page_stored_pos))
+    if rc != 0:
+        raise LazyError("lazy_set_page_stored_pos", rc)
+    h._stored_pos = page_stored_pos          # the library keeps the pointer: keep the tensor alive with the handle
+
+
+def lazy_materialize_pages(h: LazyHandle, k_src, v_src, src_pages, rot_pos, per_token: bool, k_dst, v_dst,
+                           dst_pages, stream=None) -> None:
+    num = int(src_pages.shape[0])
+    rc = lib().lazy_materialize_pages(h.ptr, _ptr(k_src), _ptr(v_src), _ptr(src_pages), _ptr(rot_pos),
+                                      1 if per_token else 0, _ptr(k_dst), _ptr(v_dst), _ptr(dst_pages), num,
+                                      _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_materialize_pages", rc)
 
 
 class HostStep(ctypes.Structure):

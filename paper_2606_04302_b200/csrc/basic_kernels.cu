@@ -70,6 +70,73 @@ int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, con
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// Materialising re-encoding ("allocate + copy + rotate", L447).  HBM-bound:
+// per page it reads Hkv*16*D*2 B of K (and of V) and writes the same.  One thread owns one 8-pair chunk of one
+// row: two 16-byte loads (dims 8c.. and D/2+8c..), fp32 rotation from the fp64-built table, two 16-byte stores.
+template <int D>
+__global__ void __launch_bounds__(256)
+materialize_pages_kernel(const uint4* __restrict__ k_src, const uint4* __restrict__ v_src,
+                         const int* __restrict__ src_pages, const int* __restrict__ rot_pos, int per_token,
+                         uint4* __restrict__ k_dst, uint4* __restrict__ v_dst, const int* __restrict__ dst_pages,
+                         long long num_items, int Hkv, const float2* __restrict__ cs) {
+  constexpr int CPR = D / 16;                       // chunk pairs per row
+  constexpr int CH = D / 8;                         // 16-byte chunks per row
+  long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= num_items) return;
+  const int c = (int)(idx % CPR);
+  long long row = idx / CPR;                        // (i, hk, t)
+  const int t = (int)(row % kPageSize);
+  const int hk = (int)((row / kPageSize) % Hkv);
+  const int i = (int)(row / ((long long)kPageSize * Hkv));
+  const int sp = src_pages[i], dp = dst_pages[i];
+  int pos = rot_pos[i] + (per_token ? t : 0);
+  const float sgn = pos < 0 ? -1.f : 1.f;
+  pos = pos < 0 ? -pos : pos;
+  const long long srow = (((long long)sp * Hkv + hk) * kPageSize + t) * CH;
+  const long long drow = (((long long)dp * Hkv + hk) * kPageSize + t) * CH;
+  uint4 va = k_src[srow + c], vb = k_src[srow + c + CPR];
+  uint32_t* aw = reinterpret_cast<uint32_t*>(&va);
+  uint32_t* bw = reinterpret_cast<uint32_t*>(&vb);
+  const float2* row_cs = cs + (size_t)pos * (D / 2);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    const float2 c0 = __ldg(row_cs + cs_index(8 * c + 2 * w, D));
+    const float2 c1 = __ldg(row_cs + cs_index(8 * c + 2 * w + 1, D));
+    const float a0 = ptx::bf16_lo(aw[w]), a1 = ptx::bf16_hi(aw[w]);
+    const float b0 = ptx::bf16_lo(bw[w]), b1 = ptx::bf16_hi(bw[w]);
+    const float s0 = c0.y * sgn, s1 = c1.y * sgn;
+    aw[w] = ptx::pack_bf16(a0 * c0.x - b0 * s0, a1 * c1.x - b1 * s1);
+    bw[w] = ptx::pack_bf16(a0 * s0 + b0 * c0.x, a1 * s1 + b1 * c1.x);
+  }
+  k_dst[drow + c] = va;
+  k_dst[drow + c + CPR] = vb;
+  if (v_src != nullptr && v_dst != nullptr) {
+    v_dst[drow + c] = v_src[srow + c];
+    v_dst[drow + c + CPR] = v_src[srow + c + CPR];
+  }
+}
+
+int launch_materialize(lazy_handle* h, const void* k_src, const void* v_src, const int32_t* src_pages,
+                       const int32_t* rot_pos, int per_token, void* k_dst, void* v_dst, const int32_t* dst_pages,
+                       int num, cudaStream_t stream) {
+  const int D = h->cfg.head_dim;
+  const long long items = (long long)num * h->cfg.num_kv_heads * kPageSize * (D / 16);
+  const int threads = 256;
+  const long long blocks = (items + threads - 1) / threads;
+  auto ks = static_cast<const uint4*>(k_src);
+  auto vs = static_cast<const uint4*>(v_src);
+  auto kd = static_cast<uint4*>(k_dst);
+  auto vd = static_cast<uint4*>(v_dst);
+  if (D == 128)
+    materialize_pages_kernel<128><<<(unsigned)blocks, threads, 0, stream>>>(
+        ks, vs, src_pages, rot_pos, per_token, kd, vd, dst_pages, items, h->cfg.num_kv_heads, h->ws.cs);
+  else
+    materialize_pages_kernel<64><<<(unsigned)blocks, threads, 0, stream>>>(
+        ks, vs, src_pages, rot_pos, per_token, kd, vd, dst_pages, items, h->cfg.num_kv_heads, h->ws.cs);
+  return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // Row-wise attention (debug path).  PER = D/64 rotation pairs per lane: lane owns j = lane*PER + i.
 template <int D>
 __global__ void __launch_bounds__(128)
@@ -77,7 +144,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
                     const __nv_bfloat16* __restrict__ v_cache, const int* __restrict__ block_table,
                     const int* __restrict__ page_pos, const int* __restrict__ seq_lens,
                     const int* __restrict__ cu_q_lens, int num_reqs, Shape sh, const float2* __restrict__ cs,
-                    __nv_bfloat16* __restrict__ out) {
+                    int k_storage, const int* __restrict__ stored_pos, __nv_bfloat16* __restrict__ out) {
   constexpr int HALF = D / 2;
   constexpr int PER = D / 64;
   const int row = blockIdx.x;
@@ -125,7 +192,12 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
   for (int s = warp; s <= sq; s += 4) {
     int slot = s / kPageSize, t = s % kPageSize;
     int page = bt[slot];
-    int pos = pp[slot] + t;
+    // rotation still owed to this key: its logical position (un-rotated pages), one relative offset per page
+    // (stored-position pages), nothing (absolute pages; table row 0 is the identity)
+    int pos = k_storage == LAZY_K_UNROTATED ? pp[slot] + t
+              : k_storage == LAZY_K_STORED_POS ? pp[slot] - stored_pos[page] : 0;
+    const float sgn = pos < 0 ? -1.f : 1.f;
+    pos = pos < 0 ? -pos : pos;
     size_t base = (((size_t)page * sh.Hkv + hk) * kPageSize + t) * D;
     float dot = 0.f, v1[PER], v2[PER];
 #pragma unroll
@@ -133,6 +205,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
       int j = lane * PER + e;
       float a = __bfloat162float(k_cache[base + j]), b = __bfloat162float(k_cache[base + j + HALF]);
       float2 tcs = cs[(size_t)pos * HALF + cs_index(j, D)];
+      tcs.y *= sgn;
       dot += q1[e] * (a * tcs.x - b * tcs.y) + q2[e] * (a * tcs.y + b * tcs.x);
       v1[e] = __bfloat162float(v_cache[base + j]);
       v2[e] = __bfloat162float(v_cache[base + j + HALF]);
@@ -176,10 +249,12 @@ int launch_rowwise(lazy_handle* h, const void* q, const void* k_cache, const voi
   auto op = static_cast<__nv_bfloat16*>(out);
   if (h->cfg.head_dim == 128)
     rowwise_attn_kernel<128><<<grid, 128, 0, stream>>>(qp, kp, vp, block_table, page_logical_pos, seq_lens,
-                                                       cu_q_lens, num_reqs, h->shape, h->ws.cs, op);
+                                                       cu_q_lens, num_reqs, h->shape, h->ws.cs, h->cfg.k_storage,
+                                                       h->page_stored_pos, op);
   else
     rowwise_attn_kernel<64><<<grid, 128, 0, stream>>>(qp, kp, vp, block_table, page_logical_pos, seq_lens,
-                                                      cu_q_lens, num_reqs, h->shape, h->ws.cs, op);
+                                                      cu_q_lens, num_reqs, h->shape, h->ws.cs, h->cfg.k_storage,
+                                                      h->page_stored_pos, op);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
 

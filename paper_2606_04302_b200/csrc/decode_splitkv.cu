@@ -65,6 +65,7 @@ struct DecodeArgs {
   const int* seq_lens;
   __nv_bfloat16* out;
   const float2* cs;
+  const int* stored_pos;   // LAZY_K_STORED_POS: [num_pages] position each physical page was stored at
   float* part_o;
   float2* part_ml;
   int* req_counter;
@@ -72,7 +73,11 @@ struct DecodeArgs {
   Shape sh;
 };
 
-template <int D, int HKV_CTA>
+// KM = lazy_config.k_storage.  LAZY_K_UNROTATED: the identity above.  LAZY_K_STORED_POS (Eq. 6,
+// L175-182: "rotate Q" by the page's relative offset): K is consumed as stored, q is re-rotated once per page
+// by m - (p0 - stored[page]).  LAZY_K_ABSOLUTE: K as stored, q rotated once per request by m (no table rows
+// travel with the pages): the "rotation compiled out" arm of the overhead ablation (Fig. 5).
+template <int D, int HKV_CTA, int KM>
 __global__ void __launch_bounds__(kDecodeThreads, 1)
 decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
                       const DecodeArgs a) {
@@ -173,6 +178,7 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
         int mq = pp[(L - 1) / kPageSize] + (L - 1) % kPageSize;    // position of the query token
         pg = bt[p];
         delta = mq - pp[p];
+        if (KM == LAZY_K_STORED_POS) delta += a.stored_pos[pg];
       }
     };
     int pg, delta, nvalid;
@@ -193,7 +199,8 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
       const bool active = pl < nvalid;
       if (pl < C::PPS) reinterpret_cast<int*>(st + C::OFF_META)[pl] = delta;
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive_expect_tx(full, nvalid * (2 * C::PAGE_BYTES + C::CS_ROW_BYTES));
+      if (lane == 0)
+        ptx::mbar_arrive_expect_tx(full, nvalid * (2 * C::PAGE_BYTES + (KM == LAZY_K_ABSOLUTE ? 0 : C::CS_ROW_BYTES)));
       __syncwarp();
       if (active) {
         const int row0 = (pg * sh.Hkv + hg * HKV_CTA) * kPageSize;
@@ -202,9 +209,11 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
           ptx::tma_load_2d(st_u32 + pl * C::PAGE_BYTES + h * C::BOX_BYTES, &tmap_k, full, h * 64, row0);
           ptx::tma_load_2d(st_u32 + C::OFF_V + pl * C::PAGE_BYTES + h * C::BOX_BYTES, &tmap_v, full, h * 64, row0);
         }
-        int ad = delta < 0 ? -delta : delta;
-        ptx::bulk_load_1d(st_u32 + C::OFF_CS + pl * C::CS_ROW_BYTES, a.cs + (size_t)ad * (D / 2),
-                          C::CS_ROW_BYTES, full);
+        if (KM != LAZY_K_ABSOLUTE) {
+          int ad = delta < 0 ? -delta : delta;
+          ptx::bulk_load_1d(st_u32 + C::OFF_CS + pl * C::CS_ROW_BYTES, a.cs + (size_t)ad * (D / 2),
+                            C::CS_ROW_BYTES, full);
+        }
       }
       pg = pg_n; delta = delta_n; nvalid = nvalid_n;
       r = rn; u = un; ++it;
@@ -243,6 +252,27 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
         }
     }
 
+    // Qhat = scale * R_angle q from one cos/sin row (a3/a4); `scale` is 1 when the K side carries the scale
+    uint32_t qhat[2][C::NL];
+    auto rotate_q = [&](auto&& load_cs, float sgn, float scale) {
+#pragma unroll
+      for (int w = 0; w < C::NL; ++w) {
+        float4 c = load_cs(w);
+        c.x *= scale; c.z *= scale;
+        c.y *= sgn * scale; c.w *= sgn * scale;
+        float a_lo = ptx::bf16_lo(qraw[0][w]), a_hi = ptx::bf16_hi(qraw[0][w]);
+        float b_lo = ptx::bf16_lo(qraw[1][w]), b_hi = ptx::bf16_hi(qraw[1][w]);
+        qhat[0][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
+        qhat[1][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
+      }
+    };
+    if (KM == LAZY_K_ABSOLUTE && L > 0) {           // once per request: rotate q by the query token's position
+      const int* pp = a.page_pos + (size_t)r * sh.table_stride;
+      const int mq = pp[(L - 1) / kPageSize] + (L - 1) % kPageSize;
+      const float4* row = reinterpret_cast<const float4*>(a.cs + (size_t)mq * (D / 2)) + tq;
+      rotate_q([&](int w) { return __ldg(row + w * 4); }, 1.f, sh.scale_log2);
+    }
+
     float oacc[C::NC][4];
 #pragma unroll
     for (int i = 0; i < C::NC; ++i) { oacc[i][0] = oacc[i][1] = oacc[i][2] = oacc[i][3] = 0.f; }
@@ -275,31 +305,24 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
               kreg[h][rw][4 * x + 2] = v.z; kreg[h][rw][4 * x + 3] = v.w;
             }
         // ---- q re-rotated for this page: Qhat = R_{m - p0} q   (a3/a4; one cos/sin row per page)
-        uint32_t qhat[2][C::NL];
-        {
+        if (KM != LAZY_K_ABSOLUTE) {
           const uint32_t qcs = st + C::OFF_CS + pl * C::CS_ROW_BYTES + tq * 16;
-          const float sgn = delta < 0 ? -1.f : 1.f;
-#pragma unroll
-          for (int w = 0; w < C::NL; ++w) {
-            float4 c = ptx::lds128f(qcs + w * 64);
-            c.y *= sgn; c.w *= sgn;
-            float a_lo = ptx::bf16_lo(qraw[0][w]), a_hi = ptx::bf16_hi(qraw[0][w]);
-            float b_lo = ptx::bf16_lo(qraw[1][w]), b_hi = ptx::bf16_hi(qraw[1][w]);
-            qhat[0][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
-            qhat[1][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
-          }
+          rotate_q([&](int w) { return ptx::lds128f(qcs + w * 64); }, delta < 0 ? -1.f : 1.f,
+                   KM == LAZY_K_UNROTATED ? 1.f : sh.scale_log2);
         }
-        // ---- Khat = scale * R_t k in fp32 registers, rounded to bf16 for the MMA
+        // ---- Khat = scale * R_t k in fp32 registers, rounded to bf16 for the MMA (un-rotated pages only)
+        if (KM == LAZY_K_UNROTATED) {
 #pragma unroll
-        for (int rw = 0; rw < 2; ++rw)
+          for (int rw = 0; rw < 2; ++rw)
 #pragma unroll
-          for (int w = 0; w < C::NL; ++w) {
-            const float4 c = ptx::lds128f(ctab_u32 + (rw * C::NL + w) * 512);
-            float a_lo = ptx::bf16_lo(kreg[0][rw][w]), a_hi = ptx::bf16_hi(kreg[0][rw][w]);
-            float b_lo = ptx::bf16_lo(kreg[1][rw][w]), b_hi = ptx::bf16_hi(kreg[1][rw][w]);
-            kreg[0][rw][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
-            kreg[1][rw][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
-          }
+            for (int w = 0; w < C::NL; ++w) {
+              const float4 c = ptx::lds128f(ctab_u32 + (rw * C::NL + w) * 512);
+              float a_lo = ptx::bf16_lo(kreg[0][rw][w]), a_hi = ptx::bf16_hi(kreg[0][rw][w]);
+              float b_lo = ptx::bf16_lo(kreg[1][rw][w]), b_hi = ptx::bf16_hi(kreg[1][rw][w]);
+              kreg[0][rw][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
+              kreg[1][rw][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
+            }
+        }
         // ---- S = Khat Qhat^T : rows = tokens (g, g+8), cols = heads (2tq, 2tq+1)
         float s[4] = {0.f, 0.f, 0.f, 0.f}, s_b[4] = {0.f, 0.f, 0.f, 0.f};   // two chains: halves the MMA latency chain
 #pragma unroll
@@ -484,11 +507,11 @@ bool encode_q_tmap(void* out_map, const void* q, int total_q, int Hq, int Hkv, i
   return rc == CUDA_SUCCESS;
 }
 
-template <int D, int HKV_CTA>
-static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, int grid_y, cudaStream_t stream) {
+template <int D, int HKV_CTA, int KM>
+static int launch_decode_km(lazy_handle* h, const DecodeArgs& args, int grid_x, int grid_y, cudaStream_t stream) {
   using C = DecodeCfg<D, HKV_CTA>;
   static bool attr_set = false;
-  auto kern = decode_splitkv_kernel<D, HKV_CTA>;
+  auto kern = decode_splitkv_kernel<D, HKV_CTA, KM>;
   if (!attr_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
       return LAZY_ERR_CUDA;
@@ -498,6 +521,15 @@ static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, i
   const CUtensorMap* mv = reinterpret_cast<const CUtensorMap*>(h->tmap_v);
   kern<<<dim3(grid_x, grid_y), kDecodeThreads, C::SMEM_BYTES, stream>>>(*mk, *mv, args);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
+}
+
+template <int D, int HKV_CTA>
+static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, int grid_y, cudaStream_t stream) {
+  switch (h->cfg.k_storage) {
+    case LAZY_K_STORED_POS: return launch_decode_km<D, HKV_CTA, LAZY_K_STORED_POS>(h, args, grid_x, grid_y, stream);
+    case LAZY_K_ABSOLUTE:   return launch_decode_km<D, HKV_CTA, LAZY_K_ABSOLUTE>(h, args, grid_x, grid_y, stream);
+    default:                return launch_decode_km<D, HKV_CTA, LAZY_K_UNROTATED>(h, args, grid_x, grid_y, stream);
+  }
 }
 
 int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
@@ -525,6 +557,7 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
     a.page_pos = page_logical_pos + (size_t)r0 * c.max_pages_per_req;
     a.seq_lens = seq_lens + r0;
     a.cs = h->ws.cs;
+    a.stored_pos = h->page_stored_pos;
     a.part_o = h->ws.part_o;
     a.part_ml = h->ws.part_ml;
     a.req_counter = h->ws.req_counter;

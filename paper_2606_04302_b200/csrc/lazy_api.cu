@@ -21,6 +21,7 @@ bool config_supported(const lazy_config* c) {
   int hkv = c->num_kv_heads;
   if (!(hkv == 1 || hkv == 2 || hkv == 4 || hkv % 8 == 0)) return false;
   if (c->dtype != 0 || c->rope_style != 0) return false;
+  if (c->k_storage < LAZY_K_UNROTATED || c->k_storage > LAZY_K_ABSOLUTE) return false;
   return true;
 }
 
@@ -124,10 +125,35 @@ int lazy_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const
   return LAZY_OK;
 }
 
+int lazy_set_page_stored_pos(lazy_handle* h, const int32_t* page_stored_pos) {
+  if (!h || !page_stored_pos || (reinterpret_cast<uintptr_t>(page_stored_pos) & 3u)) return LAZY_ERR_INVALID;
+  if (h->cfg.k_storage != LAZY_K_STORED_POS) return LAZY_ERR_UNSUPPORTED;
+  h->page_stored_pos = page_stored_pos;
+  return LAZY_OK;
+}
+
+int lazy_materialize_pages(lazy_handle* h, const void* k_src, const void* v_src, const int32_t* src_pages,
+                           const int32_t* rot_pos, int32_t per_token, void* k_dst, void* v_dst,
+                           const int32_t* dst_pages, int32_t num, void* stream) {
+  if (!h || num < 0) return LAZY_ERR_INVALID;
+  if (num == 0) return LAZY_OK;
+  if (!k_src || !k_dst || !src_pages || !rot_pos || !dst_pages) return LAZY_ERR_INVALID;
+  if (misaligned(k_src) || misaligned(k_dst) || misaligned(v_src) || misaligned(v_dst) ||
+      (reinterpret_cast<uintptr_t>(src_pages) & 3u) || (reinterpret_cast<uintptr_t>(rot_pos) & 3u) ||
+      (reinterpret_cast<uintptr_t>(dst_pages) & 3u))
+    return LAZY_ERR_INVALID;
+  int n = lazy::launch_materialize(h, k_src, v_src, src_pages, rot_pos, per_token != 0, k_dst, v_dst, dst_pages,
+                                   num, static_cast<cudaStream_t>(stream));
+  if (n < 0) return n;
+  h->launches += n;
+  return LAZY_OK;
+}
+
 static int check_attn_args(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                            const int32_t* block_table, const int32_t* page_logical_pos,
                            const int32_t* seq_lens, int32_t num_reqs, void* out) {
   if (!h || num_reqs < 0) return LAZY_ERR_INVALID;
+  if (h->cfg.k_storage == LAZY_K_STORED_POS && !h->page_stored_pos) return LAZY_ERR_INVALID;
   if (num_reqs > h->cfg.max_reqs) return LAZY_ERR_INVALID;
   if (num_reqs == 0) return LAZY_OK;
   if (!q || !k_cache || !v_cache || !block_table || !page_logical_pos || !seq_lens || !out)

@@ -36,6 +36,7 @@ struct lazy_handle {
   lazy::Workspace ws;
   int num_sms;
   int64_t launches;
+  const int32_t* page_stored_pos;   // LAZY_K_STORED_POS: device [num_pages], caller-owned
   // cached TMA descriptors (128 bytes each), keyed by the pool pointer they were encoded for
   alignas(64) unsigned char tmap_k[128];
   alignas(64) unsigned char tmap_v[128];
@@ -63,6 +64,9 @@ bool encode_q_tmap(void* out_map, const void* q, int total_q, int Hq, int Hkv, i
 int launch_build_tables(lazy_handle* h, cudaStream_t stream);
 int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
                        int num_tokens, void* k_cache, void* v_cache, cudaStream_t stream);
+int launch_materialize(lazy_handle* h, const void* k_src, const void* v_src, const int32_t* src_pages,
+                       const int32_t* rot_pos, int per_token, void* k_dst, void* v_dst, const int32_t* dst_pages,
+                       int num, cudaStream_t stream);
 int launch_rowwise(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                    const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                    const int32_t* cu_q_lens, int num_reqs, int total_q, int max_q_len, void* out,

@@ -45,7 +45,8 @@ struct PrefillCfg {
   static constexpr int OFF_BAR = OFF_CS + 2 * CS_STAGE_BYTES;
   static constexpr int NUM_BARS = 24;
   static constexpr int OFF_TMEM = OFF_BAR + NUM_BARS * 8;
-  static constexpr int SMEM_BYTES = OFF_TMEM + 16 + 1024;   // + alignment slack
+  static constexpr int OFF_SIGN = OFF_TMEM + 16;    // 2 stages x 8 pages: sign of the page's relative offset
+  static constexpr int SMEM_BYTES = OFF_SIGN + 2 * kPagesPerTile * 4 + 1024;   // + alignment slack
 };
 
 // register budgets per warpgroup (setmaxnreg; 2*128*184 + 128*104 + 128*40 = 65536)
@@ -73,6 +74,7 @@ struct PrefillArgs {
   const int* cu_q_lens;
   __nv_bfloat16* out;
   const float2* cs;
+  const int* stored_pos;   // LAZY_K_STORED_POS: [num_pages] position each physical page was stored at
   int num_reqs;
   int mblocks;          // CTAs per (request, kv head)
   int tokens_per_tile;  // 128 / group
@@ -139,7 +141,11 @@ __device__ __forceinline__ void rotate8(uint4& a, uint4& b, const float (&co)[8]
   }
 }
 
-template <int D>
+// KM = lazy_config.k_storage.  LAZY_K_UNROTATED: K tile rotated by the absolute angle of its tokens.
+// LAZY_K_STORED_POS (Eq. 5): K tile rotated once by the page's relative offset
+// D = p0 - stored[page] (one table row per page, no in-page composition).  LAZY_K_ABSOLUTE: the K tile goes to
+// the MMA as it landed (the "rotation compiled out" arm of the overhead ablation, Fig. 5).
+template <int D, int KM>
 __global__ void __launch_bounds__(kPrefillThreads, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
                     const __grid_constant__ CUtensorMap tmap_v, const PrefillArgs a) {
@@ -219,24 +225,32 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       const bool lane_on = half < C::NH;
       int page_next = (pg < num_pages) ? bt[pg] : 0;
       int pos_next = (pg < num_pages) ? ppos[pg] : 0;
+      if (KM == LAZY_K_STORED_POS) pos_next -= a.stored_pos[page_next];
+      int* s_sign = reinterpret_cast<int*>(smem + C::OFF_SIGN);
       for (int j = 0; j < n_kv; ++j) {
         const int s = j & 1, ph = (j >> 1) & 1;
-        const int page = page_next, p0 = pos_next;
+        const int page = page_next;
+        const int p0 = pos_next < 0 ? -pos_next : pos_next;      // negative only for LAZY_K_STORED_POS
+        const int p0_sign = pos_next < 0 ? -1 : 1;
         if (j + 1 < n_kv) {
           const int idx = (j + 1) * kPagesPerTile + pg;
           page_next = idx < num_pages ? bt[idx] : 0;
           pos_next = idx < num_pages ? ppos[idx] : 0;
+          if (KM == LAZY_K_STORED_POS) pos_next -= a.stored_pos[page_next];
         }
         const int npv = min(kPagesPerTile, num_pages - j * kPagesPerTile);
         const int row0 = (page * sh.Hkv + hk) * kPageSize;
         const uint32_t dst = s * C::TILE_BYTES + half * kHalfBytes + pg * (kPageSize * 128);
         ptx::mbar_wait_sleep(bar(B_KEMPTY + s), ph ^ 1);
+        if (KM == LAZY_K_STORED_POS && lane < kPagesPerTile) s_sign[s * kPagesPerTile + pg] = p0_sign;
+        __syncwarp();
         if (lane == 0)
-          ptx::mbar_arrive_expect_tx(bar(B_KFULL + s), npv * (C::NH * kPageSize * 128 + C::CS_ROW_BYTES));
+          ptx::mbar_arrive_expect_tx(bar(B_KFULL + s), npv * (C::NH * kPageSize * 128 +
+                                                              (KM == LAZY_K_ABSOLUTE ? 0 : C::CS_ROW_BYTES)));
         __syncwarp();
         if (kvsel == 0 && lane_on && pg < npv) {
           ptx::tma_load_2d(sK + dst, &tmap_k, bar(B_KFULL + s), half * 64, row0);
-          if (half == 0)
+          if (half == 0 && KM != LAZY_K_ABSOLUTE)
             ptx::bulk_load_1d(sCS + s * C::CS_STAGE_BYTES + pg * C::CS_ROW_BYTES, a.cs + (size_t)p0 * (D / 2),
                               C::CS_ROW_BYTES, bar(B_KFULL + s));
         }
@@ -326,7 +340,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     const int wtid = tid - 256;
     const int pp_ = wtid / TPP, t = (wtid % TPP) / C::CPR, c = wtid % C::CPR;
     float uc[8], us[8];                             // e^{i t theta_j}: in-page offset, fixed per thread
-    load_cs8<D>(a.cs + (size_t)t * (D / 2), c, uc, us);
+    if (KM == LAZY_K_UNROTATED) load_cs8<D>(a.cs + (size_t)t * (D / 2), c, uc, us);
+    const int* s_sign = reinterpret_cast<const int*>(smem + C::OFF_SIGN);
     for (int j = 0; j < n_kv; ++j) {
       const int s = j & 1;
       const int npv = min(kPagesPerTile, num_pages - j * kPagesPerTile);
@@ -336,16 +351,22 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 #pragma unroll
       for (int ps = 0; ps < PASSES; ++ps) {
         const int i = ps * PPP + pp_;
-        if (i < npv) {
+        if (KM != LAZY_K_ABSOLUTE && i < npv) {
           float wc[8], ws[8], zc[8], zs[8];         // e^{i p0 theta_j} of the page, then e^{i (p0+t) theta_j}
           load_cs8_smem<D>(cb + i * C::CS_ROW_BYTES, c, wc, ws);
           const int row = i * kPageSize + t;
           const uint32_t pa = kb + chunk_off(row, c), pb = kb + chunk_off(row, c + C::CPR);
           uint4 va = ptx::lds128(pa), vb = ptx::lds128(pb);
+          if (KM == LAZY_K_UNROTATED) {
 #pragma unroll
-          for (int e = 0; e < 8; ++e) {
-            zc[e] = wc[e] * uc[e] - ws[e] * us[e];
-            zs[e] = ws[e] * uc[e] + wc[e] * us[e];
+            for (int e = 0; e < 8; ++e) {
+              zc[e] = wc[e] * uc[e] - ws[e] * us[e];
+              zs[e] = ws[e] * uc[e] + wc[e] * us[e];
+            }
+          } else {                                  // one relative rotation for the whole page (may be negative)
+            const float sgn = (float)s_sign[s * kPagesPerTile + i];
+#pragma unroll
+            for (int e = 0; e < 8; ++e) { zc[e] = wc[e]; zs[e] = ws[e] * sgn; }
           }
           rotate8(va, vb, zc, zs);
           ptx::sts128(pa, va);
@@ -494,11 +515,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 
 }  // namespace
 
-template <int D>
+template <int D, int KM>
 static int launch_prefill_t(const lazy_handle* h, const PrefillArgs& args, int grid, cudaStream_t stream) {
   using C = PrefillCfg<D>;
   static bool attr_set = false;
-  auto kern = prefill_umma_kernel<D>;
+  auto kern = prefill_umma_kernel<D, KM>;
   if (!attr_set) {
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
       return LAZY_ERR_CUDA;
@@ -539,14 +560,22 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   a.cu_q_lens = cu_q_lens;
   a.out = static_cast<__nv_bfloat16*>(out);
   a.cs = h->ws.cs;
+  a.stored_pos = h->page_stored_pos;
   a.num_reqs = num_reqs;
   a.mblocks = (max_q_len + 2 * tpt - 1) / (2 * tpt);
   a.tokens_per_tile = tpt;
   a.sh = h->shape;
   const long long grid = (long long)a.mblocks * c.num_kv_heads * num_reqs;
   if (grid <= 0 || grid > INT_MAX) return LAZY_ERR_INVALID;
-  return c.head_dim == 128 ? launch_prefill_t<128>(h, a, (int)grid, stream)
-                           : launch_prefill_t<64>(h, a, (int)grid, stream);
+  const int g = (int)grid;
+  if (c.head_dim == 128) {
+    if (c.k_storage == LAZY_K_STORED_POS) return launch_prefill_t<128, LAZY_K_STORED_POS>(h, a, g, stream);
+    if (c.k_storage == LAZY_K_ABSOLUTE) return launch_prefill_t<128, LAZY_K_ABSOLUTE>(h, a, g, stream);
+    return launch_prefill_t<128, LAZY_K_UNROTATED>(h, a, g, stream);
+  }
+  if (c.k_storage == LAZY_K_STORED_POS) return launch_prefill_t<64, LAZY_K_STORED_POS>(h, a, g, stream);
+  if (c.k_storage == LAZY_K_ABSOLUTE) return launch_prefill_t<64, LAZY_K_ABSOLUTE>(h, a, g, stream);
+  return launch_prefill_t<64, LAZY_K_UNROTATED>(h, a, g, stream);
 }
 
 }  // namespace lazy

@@ -12,19 +12,26 @@ from .workloads import LazyBatch, Step
 
 
 class DeviceBatch:
-    def __init__(self, batch: LazyBatch, device: str = "cuda", flags: int = 0, max_position: Optional[int] = None):
+    def __init__(self, batch: LazyBatch, device: str = "cuda", flags: int = 0, max_position: Optional[int] = None,
+                 k_storage: int = B.LAZY_K_UNROTATED, page_stored_pos: Optional[torch.Tensor] = None,
+                 k_pool: Optional[torch.Tensor] = None, v_pool: Optional[torch.Tensor] = None,
+                 block_table: Optional[torch.Tensor] = None):
+        """k_pool / v_pool / block_table override the batch's own (the stored-position and absolute layouts of
+        SURVEY 8.0 row f1 hold differently encoded K, the absolute one also private pages per request)."""
         self.batch = batch
         self.device = torch.device(device)
         sh = batch.shape
-        self.k_pool = batch.k_pool.to(self.device)
-        self.v_pool = batch.v_pool.to(self.device)
-        self.block_table = batch.block_table.to(self.device)
+        self.k_pool = (batch.k_pool if k_pool is None else k_pool).to(self.device)
+        self.v_pool = (batch.v_pool if v_pool is None else v_pool).to(self.device)
+        self.block_table = (batch.block_table if block_table is None else block_table).to(self.device)
         self.page_logical_pos = batch.page_logical_pos.to(self.device)
         R, pmax = batch.block_table.shape
-        self.handle = B.lazy_create(sh.num_q_heads, sh.num_kv_heads, sh.head_dim, num_pages=batch.num_pages,
+        self.handle = B.lazy_create(sh.num_q_heads, sh.num_kv_heads, sh.head_dim, num_pages=int(self.k_pool.shape[0]),
                                     max_position=max_position or batch.max_position, max_reqs=R,
                                     max_pages_per_req=pmax, rope_theta=sh.rope_theta, page_size=sh.page_size,
-                                    flags=flags, device=self.device)
+                                    flags=flags, k_storage=k_storage, device=self.device)
+        if page_stored_pos is not None:
+            B.lazy_set_page_stored_pos(self.handle, page_stored_pos.to(self.device, dtype=torch.int32).contiguous())
 
     def tables_for(self, step: Step):
         if step.req_ids is None:

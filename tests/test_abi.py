@@ -39,7 +39,7 @@ def test_status_strings(lib):
 
 def _cfg(**kw):
     base = dict(num_q_heads=32, num_kv_heads=8, head_dim=128, page_size=16, num_pages=1000, max_position=4096,
-                max_reqs=64, max_pages_per_req=256, rope_theta=5e5, rope_style=0, dtype=0, flags=0, reserved=0)
+                max_reqs=64, max_pages_per_req=256, rope_theta=5e5, rope_style=0, dtype=0, flags=0, k_storage=0)
     base.update(kw)
     return B.LazyConfig(**base)
 
