@@ -258,6 +258,89 @@ class GpuJob:
         return sum(e[0].elapsed_time(e[1]) for e in evs)
 
 
+def run_ablation(job, steps, warmup):
+    """SURVEY 8.0 rows f1 / f2 on the job's batch: every (request, slot) gets a PRIVATE page (same block tables
+    and same HBM traffic in every arm), holding K (a) un-rotated, (b) rotated at a document-local stored position
+    (the paper's layout: one relative rotation per page), (c) rotated at its final position (rotation compiled
+    out: PAPER.md Fig. 5 'without deferred rotation').  The copies are made by lazy_materialize_pages, whose own
+    time is the Block-Attention-style re-encoding cost the lazy path avoids."""
+    from paper_2606_04302_b200.runner import DeviceBatch
+    B, dev, batch = job.B, job.dev, job.batch
+    d, sh, P = dev.device, batch.shape, batch.shape.page_size
+    rec = job.timed[-1]                               # the attention call of the step (decode, or cfg3's prefill)
+    st = rec["step"]
+    bt_h = batch.block_table if st.req_ids is None else batch.block_table[st.req_ids]
+    pp_h = batch.page_logical_pos if st.req_ids is None else batch.page_logical_pos[st.req_ids]
+    R, pmax = bt_h.shape
+    need = (st.seq_lens.to(torch.int64) + P - 1) // P
+    mask = torch.arange(pmax)[None, :] < need[:, None]
+    src = bt_h[mask].to(torch.int32).contiguous()
+    starts = pp_h[mask].to(torch.int32).contiguous()
+    n = int(src.numel())
+    bt_priv = torch.zeros(R, pmax, dtype=torch.int32)
+    bt_priv[mask] = torch.arange(n, dtype=torch.int32)
+    doc_pages = max(1, int(batch.meta.get("doc_len", 256)) // P)
+    slot = torch.arange(pmax)[None, :].expand(R, pmax)[mask]
+    stored = ((slot % doc_pages) * P).to(torch.int32).contiguous()
+    src_d, dst_d = src.to(d), torch.arange(n, dtype=torch.int32, device=d)
+    shape = (n, sh.num_kv_heads, P, sh.head_dim)
+    v_priv = torch.empty(shape, dtype=torch.bfloat16, device=d)
+    pools = {}
+    mat_ms = None
+    for name, rot, per_token in (("unrotated", torch.zeros(n, dtype=torch.int32), False),
+                                 ("stored_pos", stored, True), ("absolute", starts, True)):
+        kp = torch.empty(shape, dtype=torch.bfloat16, device=d)
+        rot_d = rot.to(d)
+        run = lambda: B.lazy_materialize_pages(dev.handle, dev.k_pool, dev.v_pool, src_d, rot_d, per_token, kp, v_priv,
+                                               dst_d)
+        run()
+        if name == "absolute":                        # time the re-encoding itself (K rotate + V copy), L2 flushed
+            evs = []
+            for _ in range(5):
+                job.flush_l2()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); run(); e1.record()
+                evs.append((e0, e1))
+            torch.cuda.synchronize()
+            mat_ms = float(np.median([a.elapsed_time(b) for a, b in evs]))
+        pools[name] = kp
+    res = {"layout": f"private page per (request, slot): {n} pages", "pages": n}
+    modes = (("unrotated", B.LAZY_K_UNROTATED, None), ("stored_pos", B.LAZY_K_STORED_POS, stored),
+             ("absolute", B.LAZY_K_ABSOLUTE, None))
+    for name, km, sp in modes:
+        dv = DeviceBatch(batch, device=str(d), k_storage=km, page_stored_pos=sp, k_pool=pools[name], v_pool=v_priv,
+                         block_table=bt_priv if st.req_ids is None else None,
+                         max_position=batch.max_position + doc_pages * P + P)
+        bt_d = bt_priv.to(d)
+        pp_d = pp_h.to(d).contiguous()
+
+        def attend():
+            if st.kind == "decode":
+                B.lazy_attn_decode(dv.handle, rec["q"], dv.k_pool, dv.v_pool, bt_d, pp_d, rec["sl"], rec["out"])
+            else:
+                B.lazy_attn_prefill(dv.handle, rec["q"], dv.k_pool, dv.v_pool, bt_d, pp_d, rec["sl"], rec["cu"],
+                                    rec["max_q"], rec["out"])
+        for _ in range(warmup):
+            job.flush_l2(); attend()
+        evs = []
+        for _ in range(steps):
+            job.flush_l2()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); attend(); e1.record()
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+        res[name + "_ms"] = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        dv.close()
+    page_bytes = sh.num_kv_heads * P * sh.head_dim * 2
+    res["rotation_overhead_pct"] = (res["unrotated_ms"] / res["absolute_ms"] - 1.0) * 100.0
+    res["stored_pos_overhead_pct"] = (res["stored_pos_ms"] / res["absolute_ms"] - 1.0) * 100.0
+    res["unrotated_vs_stored_pos_pct"] = (res["unrotated_ms"] / res["stored_pos_ms"] - 1.0) * 100.0
+    res["materialize_ms"] = mat_ms
+    res["materialize_bytes"] = 4 * n * page_bytes                 # K read + K write + V read + V write
+    res["materialize_GBps"] = res["materialize_bytes"] / (mat_ms * 1e-3) / 1e9
+    return res
+
+
 def headline(workload, work, ms_step):
     s = ms_step * 1e-3
     if workload in ("cfg2", "cfg4"):
@@ -334,6 +417,8 @@ def main():
     ap.add_argument("--noshare", action="store_true", help="every drawn document distinct (logical == unique bytes)")
     ap.add_argument("--no-secondary", action="store_true", help="skip the prefill (cfg3) and noshare side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ablation", action="store_true",
+                    help="also time the stored-position / absolute K layouts and the materialising re-encoding (f1/f2)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -459,6 +544,12 @@ def main():
                 "d2h_bytes_per_step": int(sum(e["d2h"] for e in job.e2e))},
         "gpu_launches": int(launches), "clocks": clocks,
     }
+    if args.ablation and rank == 0 and world == 1 and args.workload != "cfg5":
+        abl = run_ablation(job, max(5, args.steps), 3)
+        abl["lazy_shared_ms"] = ms_attn
+        abl["materialise_then_attend_ms"] = abl["materialize_ms"] + abl["absolute_ms"]
+        abl["lazy_speedup_vs_materialising"] = abl["materialise_then_attend_ms"] / ms_attn
+        out["ablation"] = abl
     job.dev.close()
     del job
     torch.cuda.empty_cache()

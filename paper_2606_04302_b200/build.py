@@ -19,7 +19,7 @@ LIB = os.path.join(CSRC, "liblazyattn.so")
 SOURCES = ["lazy_api.cu", "basic_kernels.cu", "decode_splitkv.cu", "prefill_umma.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
-         "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]
+         "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC] + os.environ.get("LAZY_NVCC_EXTRA", "").split()
 
 
 def _deps_mtime() -> float:
