@@ -31,6 +31,15 @@ constexpr int kHalfBytes = kTileRows * 128;   // one 64-column (128-byte) slab o
 constexpr int kPagesPerTile = kTileRows / kPageSize;
 constexpr float kRescaleThreshold = 8.f;      // log2 units: O is rescaled only when the row max grew by > 2^8
 
+// Optional timeline probe (compile with -DLAZY_TRACE): one mid-grid CTA records clock64() at the hand-offs of 16
+// consecutive KV iterations into a device array read back by lazy_debug_trace().  Off in the product build.
+#ifdef LAZY_TRACE
+__device__ long long g_trace[16 * 16];
+#define LAZY_TR(slot) do { if (blockIdx.x == 300 && j >= 10 && j < 26) g_trace[(j - 10) * 16 + (slot)] = clock64(); } while (0)
+#else
+#define LAZY_TR(slot) do { } while (0)
+#endif
+
 template <int D>
 struct PrefillCfg {
   static constexpr int NH = D / 64;                 // 128-byte column slabs per row
@@ -100,6 +109,11 @@ __device__ __forceinline__ float f32(uint32_t x) { return __uint_as_float(x); }
 // the tensor pipe in this kernel): Cody-Waite split x = floor(x) + f with a round-down magic-number
 // add, degree-3 polynomial for 2^f on [0,1) (max relative error 8.8e-5, far inside P's bf16 rounding 2^-9), exponent
 // inserted with one integer shift-add.  x is clamped to >= -126 (covers -inf of masked columns: result 2^-126 ~ 0).
+// Softmax ping-pong (FA3-style named-barrier hand-off between the two softmax warpgroups): 0 = free running,
+// 1 = the whole softmax of a tile is exclusive, 2 = only the exponential phase is exclusive.
+#ifndef LAZY_PINGPONG
+#define LAZY_PINGPONG 2
+#endif
 #ifndef LAZY_POLY_EVERY
 #define LAZY_POLY_EVERY 0   // every LAZY_POLY_EVERY-th group of 4 columns takes this path (0 = never: measured slower)
 #endif
@@ -285,58 +299,68 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         if (kvsel == 1 && lane_on && pg < npv) ptx::tma_load_2d(sV + dst, &tmap_v, bar(B_VFULL + s), half * 64, row0);
       }
     } else if (warp == 13) {
-      // ================================ MMA issuer (one lane) ===============================================
-      if (lane == 0) {
-        constexpr uint32_t IDESC_QK = ptx::umma_idesc_bf16(128, 128, 0, 0);
-        constexpr uint32_t IDESC_PV = ptx::umma_idesc_bf16(128, D, 0, 1);     // B = V is MN-major
-        // descriptor bases are laundered through an empty asm so the 8+8 per-k descriptors are re-derived with a
-        // couple of uniform ops per MMA instead of being hoisted out of the KV loop and spilled
-        auto qk = [&](int t, int s) {
-          uint32_t qa = sQ + t * C::TILE_BYTES, ka = sK + s * C::TILE_BYTES;
-          asm volatile("" : "+r"(qa), "+r"(ka));
+      // ================================ MMA issuer ==========================================================
+      // The whole warp walks the loop convergently and ONE elected lane issues: every operand of tcgen05.mma /
+      // tcgen05.commit is then provably warp-uniform and lives in uniform registers.  (Issuing from inside
+      // `if (lane == 0)` with opaque operands made the compiler wrap each MMA in an ELECT / R2UR / BRA.U.ANY
+      // waterfall loop, ~16 dependent instructions per MMA: the issue thread, not the tensor pipe, set the pace.)
+      constexpr uint32_t IDESC_QK = ptx::umma_idesc_bf16(128, 128, 0, 0);
+      constexpr uint32_t IDESC_PV = ptx::umma_idesc_bf16(128, D, 0, 1);       // B = V is MN-major
+      const uint32_t tb = __shfl_sync(0xffffffffu, tbase, 0);
+      const int nkv = __shfl_sync(0xffffffffu, n_kv, 0);
+      const bool leader = ptx::elect_one();
+      auto qk = [&](int t, int s) {
+        if (leader) {
+          const uint32_t qa = sQ + t * C::TILE_BYTES, ka = sK + s * C::TILE_BYTES;
 #pragma unroll
           for (int k = 0; k < D / 16; ++k) {
             const uint32_t off = (k >> 2) * kHalfBytes + (k & 3) * 32;
-            ptx::umma_ss(tbase + t * 128, ptx::umma_desc_sw128(qa + off, 0, 1024),
+            ptx::umma_ss(tb + t * 128, ptx::umma_desc_sw128(qa + off, 0, 1024),
                          ptx::umma_desc_sw128(ka + off, 0, 1024), IDESC_QK, k > 0);
           }
-        };
-        auto pv = [&](int t, int s, uint32_t acc) {
-          uint32_t va = sV + s * C::TILE_BYTES;
-          asm volatile("" : "+r"(va));
+        }
+      };
+      auto pv = [&](int t, int s, uint32_t acc) {
+        if (leader) {
+          const uint32_t va = sV + s * C::TILE_BYTES;
 #pragma unroll
           for (int k = 0; k < kTileRows / 16; ++k)
-            ptx::umma_ts(tbase + 256 + t * 128, tbase + t * 128 + k * 8,
+            ptx::umma_ts(tb + 256 + t * 128, tb + t * 128 + k * 8,
                          ptx::umma_desc_sw128(va + k * 2048, kHalfBytes, 1024), IDESC_PV, acc | (uint32_t)(k > 0));
-        };
-        ptx::mbar_wait(bar(B_KREADY + 0), 0);
-        for (int t = 0; t < 2; ++t) {
-          ptx::mbar_wait(bar(B_QREADY + t), 0);
-          ptx::tc_fence_after();
-          qk(t, 0);
-          ptx::umma_commit(bar(B_SFULL + t));
         }
-        ptx::umma_commit(bar(B_KEMPTY + 0));
-        for (int j = 0; j < n_kv; ++j) {
-          const int s = j & 1;
-          ptx::mbar_wait(bar(B_VFULL + s), (j >> 1) & 1);
-          if (j == n_kv - 1) ptx::mbar_wait(bar(B_VFIXED), 0);
-          for (int t = 0; t < 2; ++t) {
-            ptx::mbar_wait(bar(B_PREADY + t), j & 1);
-            ptx::tc_fence_after();
-            pv(t, s, j > 0);
-            if (t == 1) ptx::umma_commit(bar(B_VEMPTY + s));
-            if (j + 1 < n_kv) {
-              if (t == 0) {
-                ptx::mbar_wait(bar(B_KREADY + (s ^ 1)), ((j + 1) >> 1) & 1);
-                ptx::tc_fence_after();
-              }
-              qk(t, s ^ 1);
-              ptx::umma_commit(bar(B_SFULL + t));
-              if (t == 1) ptx::umma_commit(bar(B_KEMPTY + (s ^ 1)));
-            } else {
-              ptx::umma_commit(bar(B_OFULL + t));
+      };
+      auto commit = [&](int idx) { if (leader) ptx::umma_commit(bar(idx)); };
+      ptx::mbar_wait(bar(B_KREADY + 0), 0);
+      for (int t = 0; t < 2; ++t) {
+        ptx::mbar_wait(bar(B_QREADY + t), 0);
+        ptx::tc_fence_after();
+        qk(t, 0);
+        commit(B_SFULL + t);
+      }
+      commit(B_KEMPTY + 0);
+      for (int j = 0; j < nkv; ++j) {
+        const int s = j & 1;
+        ptx::mbar_wait(bar(B_VFULL + s), (j >> 1) & 1);
+        if (j == nkv - 1) ptx::mbar_wait(bar(B_VFIXED), 0);
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+          ptx::mbar_wait(bar(B_PREADY + t), j & 1);
+          ptx::tc_fence_after();
+          if (leader) LAZY_TR(8 + 3 * t);
+          pv(t, s, j > 0);
+          if (t == 1) commit(B_VEMPTY + s);
+          if (j + 1 < nkv) {
+            if (t == 0) {
+              ptx::mbar_wait(bar(B_KREADY + (s ^ 1)), ((j + 1) >> 1) & 1);
+              ptx::tc_fence_after();
+              if (leader) LAZY_TR(9);
             }
+            qk(t, s ^ 1);
+            commit(B_SFULL + t);
+            if (leader) LAZY_TR(10 + 3 * t);
+            if (t == 1) commit(B_KEMPTY + (s ^ 1));
+          } else {
+            commit(B_OFULL + t);
           }
         }
       }
@@ -373,6 +397,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       const uint32_t kb = sK + s * C::TILE_BYTES;
       const uint32_t cb = sCS + s * C::CS_STAGE_BYTES;
       ptx::mbar_wait(bar(B_KFULL + s), (j >> 1) & 1);
+      if (wtid == 0) LAZY_TR(6);
 #pragma unroll
       for (int ps = 0; ps < PASSES; ++ps) {
         const int i = ps * PPP + pp_;
@@ -400,6 +425,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       }
       ptx::fence_proxy_async();
       __syncwarp();
+      if (wtid == 0) LAZY_TR(7);
       if (lane == 0) ptx::mbar_arrive(bar(B_KREADY + s));
     }
   } else {
@@ -445,10 +471,13 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     if (lane == 0) ptx::mbar_arrive(bar(B_QREADY + t));
 
     float m_used = -INFINITY, l_run = 0.f;
+    if (LAZY_PINGPONG && t == 1) ptx::named_bar_arrive(2, 256);          // tile 0 goes first
     for (int j = 0; j < n_kv; ++j) {
       uint32_t sreg[128];                                     // this row of S (fp32 bits), later packed P
       ptx::mbar_wait(bar(B_SFULL + t), j & 1);
+      if (LAZY_PINGPONG == 1) ptx::named_bar_sync(2 + t, 256);             // my turn
       ptx::tc_fence_after();
+      if (row == 0) LAZY_TR(3 * t);
 #pragma unroll
       for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
       ptx::tmem_wait_ld();
@@ -487,6 +516,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
           ptx::tmem_wait_st();
         }
       }
+      if (row == 0) LAZY_TR(3 * t + 1);
+      if (LAZY_PINGPONG == 2) ptx::named_bar_sync(2 + t, 256);             // my turn on the MUFU
       const float2 negm = make_float2(-m_used, -m_used);
       float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
 #pragma unroll
@@ -507,14 +538,17 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         sreg[x + 1] = ptx::pack_bf16(p1.x, p1.y);
       }
       l_run += (sum0.x + sum0.y) + (sum1.x + sum1.y);
+      if (LAZY_PINGPONG) ptx::named_bar_arrive(2 + (t ^ 1), 256);          // the other tile's turn
       ptx::tmem_st32(tS, sreg);                               // P (bf16 pairs) over the first 64 columns of S
       ptx::tmem_st32(tS + 32, sreg + 32);
       ptx::tmem_wait_st();
       ptx::tc_fence_before();
       __syncwarp();
+      if (row == 0) LAZY_TR(3 * t + 2);
       if (lane == 0) ptx::mbar_arrive(bar(B_PREADY + t));
     }
 
+    if (LAZY_PINGPONG && t == 0) ptx::named_bar_sync(2, 256);            // consume tile 1's last hand-off
     // ---- epilogue (a9): normalise, round to bf16, store the row -------------------------------------------
     ptx::mbar_wait(bar(B_OFULL + t), 0);
     ptx::tc_fence_after();
@@ -562,6 +596,12 @@ static int launch_prefill_t(const lazy_handle* h, const PrefillArgs& args, int g
   kern<<<grid, kPrefillThreads, C::SMEM_BYTES, stream>>>(*mq, *mk, *mv, args);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
+
+#ifdef LAZY_TRACE
+extern "C" int lazy_debug_trace(long long* host_out) {
+  return cudaMemcpyFromSymbol(host_out, g_trace, sizeof(long long) * 256) == cudaSuccess ? 0 : -1;
+}
+#endif
 
 int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                    const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
