@@ -21,7 +21,10 @@ __global__ void build_cs_table_kernel(float2* __restrict__ cs, int max_position,
   double inv_freq = pow(theta, -2.0 * (double)j / (double)D);
   double s, c;
   sincos((double)pos * inv_freq, &s, &c);
-  cs[pos * half + cs_index(j, D)] = make_float2((float)c, (float)s);
+  float* row = reinterpret_cast<float*>(cs + pos * half);
+  const int k = cs_cos_index(j, D);
+  row[k] = (float)c;
+  row[k + 2] = (float)s;
 }
 
 int launch_build_tables(lazy_handle* h, cudaStream_t stream) {
@@ -100,8 +103,8 @@ materialize_pages_kernel(const uint4* __restrict__ k_src, const uint4* __restric
   const float2* row_cs = cs + (size_t)pos * (D / 2);
 #pragma unroll
   for (int w = 0; w < 4; ++w) {
-    const float2 c0 = __ldg(row_cs + cs_index(8 * c + 2 * w, D));
-    const float2 c1 = __ldg(row_cs + cs_index(8 * c + 2 * w + 1, D));
+    const float2 c0 = cs_load(row_cs, 8 * c + 2 * w, D);
+    const float2 c1 = cs_load(row_cs, 8 * c + 2 * w + 1, D);
     const float a0 = ptx::bf16_lo(aw[w]), a1 = ptx::bf16_hi(aw[w]);
     const float b0 = ptx::bf16_lo(bw[w]), b1 = ptx::bf16_hi(bw[w]);
     const float s0 = c0.y * sgn, s1 = c1.y * sgn;
@@ -180,7 +183,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     for (int e = 0; e < PER; ++e) {
       int j = lane * PER + e;
       float a = __bfloat162float(qp[j]), b = __bfloat162float(qp[j + HALF]);
-      float2 t = cs[(size_t)pos_q * HALF + cs_index(j, D)];
+      float2 t = cs_load(cs + (size_t)pos_q * HALF, j, D);
       q1[e] = (a * t.x - b * t.y) * sh.scale_log2;
       q2[e] = (a * t.y + b * t.x) * sh.scale_log2;
     }
@@ -204,7 +207,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     for (int e = 0; e < PER; ++e) {
       int j = lane * PER + e;
       float a = __bfloat162float(k_cache[base + j]), b = __bfloat162float(k_cache[base + j + HALF]);
-      float2 tcs = cs[(size_t)pos * HALF + cs_index(j, D)];
+      float2 tcs = cs_load(cs + (size_t)pos * HALF, j, D);
       tcs.y *= sgn;
       dot += q1[e] * (a * tcs.x - b * tcs.y) + q2[e] * (a * tcs.y + b * tcs.x);
       v1[e] = __bfloat162float(v_cache[base + j]);

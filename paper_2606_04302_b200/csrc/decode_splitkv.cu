@@ -131,7 +131,7 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
     }
   }
   {
-    // ctab[k'][lane] (16 B each): (cos,sin) pairs of the in-page offsets, pre-multiplied by log2(e)/sqrt(D),
+    // ctab[k'][lane] (16 B each): (cos, cos, sin, sin) of two rotation pairs of the in-page offsets, pre-multiplied by log2(e)/sqrt(D),
     // in the order thread (g,tq) consumes them: row t = g + 8*(k'/NL), pairs j = JT*tq + 2*(k'%NL), +1.
     float4* ctab = reinterpret_cast<float4*>(smem + C::OFF_CTAB);
     const float4* cs4 = reinterpret_cast<const float4*>(a.cs);
@@ -258,12 +258,12 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
 #pragma unroll
       for (int w = 0; w < C::NL; ++w) {
         float4 c = load_cs(w);
-        c.x *= scale; c.z *= scale;
-        c.y *= sgn * scale; c.w *= sgn * scale;
+        c.x *= scale; c.y *= scale;                 // (cos lo, cos hi, sin lo, sin hi) of the word's two pairs
+        c.z *= sgn * scale; c.w *= sgn * scale;
         float a_lo = ptx::bf16_lo(qraw[0][w]), a_hi = ptx::bf16_hi(qraw[0][w]);
         float b_lo = ptx::bf16_lo(qraw[1][w]), b_hi = ptx::bf16_hi(qraw[1][w]);
-        qhat[0][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
-        qhat[1][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
+        qhat[0][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.z, a_hi * c.y - b_hi * c.w);
+        qhat[1][w] = ptx::pack_bf16(a_lo * c.z + b_lo * c.x, a_hi * c.w + b_hi * c.y);
       }
     };
     if (KM == LAZY_K_ABSOLUTE && L > 0) {           // once per request: rotate q by the query token's position
@@ -319,8 +319,8 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
               const float4 c = ptx::lds128f(ctab_u32 + (rw * C::NL + w) * 512);
               float a_lo = ptx::bf16_lo(kreg[0][rw][w]), a_hi = ptx::bf16_hi(kreg[0][rw][w]);
               float b_lo = ptx::bf16_lo(kreg[1][rw][w]), b_hi = ptx::bf16_hi(kreg[1][rw][w]);
-              kreg[0][rw][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.y, a_hi * c.z - b_hi * c.w);
-              kreg[1][rw][w] = ptx::pack_bf16(a_lo * c.y + b_lo * c.x, a_hi * c.w + b_hi * c.z);
+              kreg[0][rw][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.z, a_hi * c.y - b_hi * c.w);
+              kreg[1][rw][w] = ptx::pack_bf16(a_lo * c.z + b_lo * c.x, a_hi * c.w + b_hi * c.y);
             }
         }
         // ---- S = Khat Qhat^T : rows = tokens (g, g+8), cols = heads (2tq, 2tq+1)

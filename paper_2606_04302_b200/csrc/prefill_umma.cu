@@ -135,8 +135,8 @@ __device__ __forceinline__ float2 ex2_poly2(float2 v) {
                      __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
 }
 
-// Index (in 16-byte units) inside a table row of the chunk holding (cos j, sin j, cos j+1, sin j+1), j = 8c + 2x
-// (row layout: cs_index in ptx_util.cuh).
+// Index (in 16-byte units) inside a table row of the chunk holding (cos j, cos j+1, sin j, sin j+1), j = 8c + 2x
+// (row layout: cs_cos_index in ptx_util.cuh).
 template <int D>
 __device__ __forceinline__ int cs_f4_index(int c, int x) {
   constexpr int JT = D / 8;
@@ -150,7 +150,7 @@ __device__ __forceinline__ void load_cs8(const float2* __restrict__ cs_row, int 
 #pragma unroll
   for (int x = 0; x < 4; ++x) {
     float4 v = __ldg(p + cs_f4_index<D>(c, x));
-    co[2 * x] = v.x; si[2 * x] = v.y; co[2 * x + 1] = v.z; si[2 * x + 1] = v.w;
+    co[2 * x] = v.x; co[2 * x + 1] = v.y; si[2 * x] = v.z; si[2 * x + 1] = v.w;
   }
 }
 template <int D>
@@ -158,7 +158,7 @@ __device__ __forceinline__ void load_cs8_smem(uint32_t row_addr, int c, float (&
 #pragma unroll
   for (int x = 0; x < 4; ++x) {
     uint4 v = ptx::lds128(row_addr + 16 * cs_f4_index<D>(c, x));
-    co[2 * x] = f32(v.x); si[2 * x] = f32(v.y); co[2 * x + 1] = f32(v.z); si[2 * x + 1] = f32(v.w);
+    co[2 * x] = f32(v.x); co[2 * x + 1] = f32(v.y); si[2 * x] = f32(v.z); si[2 * x + 1] = f32(v.w);
   }
 }
 
@@ -184,6 +184,23 @@ __device__ __forceinline__ void rotate8(uint4& a, uint4& b, const float (&co)[8]
 // LAZY_K_STORED_POS (Eq. 5): K tile rotated once by the page's relative offset
 // D = p0 - stored[page] (one table row per page, no in-page composition).  LAZY_K_ABSOLUTE: the K tile goes to
 // the MMA as it landed (the "rotation compiled out" arm of the overhead ablation, Fig. 5).
+// Same rotation on packed f32x2 lanes (FMUL2 / FFMA2: half the FMA-pipe issue slots).  zc[w], zs[w] hold the
+// (cos, sin) of the two pairs whose x1 / x2 elements are the bf16 halves of word w of a / b.
+__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
+__device__ __forceinline__ void rotate8_packed(uint4& a, uint4& b, const float2 (&zc)[4], const float2 (&zs)[4]) {
+  uint32_t* aw = reinterpret_cast<uint32_t*>(&a);
+  uint32_t* bw = reinterpret_cast<uint32_t*>(&b);
+#pragma unroll
+  for (int w = 0; w < 4; ++w) {
+    const float2 x1 = make_float2(ptx::bf16_lo(aw[w]), ptx::bf16_hi(aw[w]));
+    const float2 x2 = make_float2(ptx::bf16_lo(bw[w]), ptx::bf16_hi(bw[w]));
+    const float2 y1 = __ffma2_rn(neg2(x2), zs[w], __fmul2_rn(x1, zc[w]));
+    const float2 y2 = __ffma2_rn(x2, zc[w], __fmul2_rn(x1, zs[w]));
+    aw[w] = ptx::pack_bf16(y1.x, y1.y);
+    bw[w] = ptx::pack_bf16(y2.x, y2.y);
+  }
+}
+
 template <int D, int KM>
 __global__ void __launch_bounds__(kPrefillThreads, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
@@ -262,21 +279,29 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       // lane -> (K or V, column slab, page of the tile); the K lanes of slab 0 also fetch the page's table row
       const int kvsel = lane >> 4, half = (lane >> 3) & 1, pg = lane & 7;
       const bool lane_on = half < C::NH;
-      int page_next = (pg < num_pages) ? bt[pg] : 0;
-      int pos_next = (pg < num_pages) ? ppos[pg] : 0;
-      if (KM == LAZY_K_STORED_POS) pos_next -= a.stored_pos[page_next];
+      // table entries travel through a 3-deep shift register (tile j+2 -> j+1 -> j), so neither the table loads nor
+      // the dependent stored-position lookup sit on the issue path.  (A cp.async.bulk.prefetch.tensor of the next
+      // tile's boxes into L2 was tried here and cost 25%: the TMA unit is better left to the real loads.)
+      auto entry = [&](int tile, int& page, int& pos) {
+        const int idx = tile * kPagesPerTile + pg;
+        page = 0; pos = 0;
+        if (tile < n_kv && idx < num_pages) {
+          page = bt[idx];
+          pos = ppos[idx];
+          if (KM == LAZY_K_STORED_POS) pos -= a.stored_pos[page];
+        }
+      };
+      int page_next, pos_next, page_n2, pos_n2;
+      entry(0, page_next, pos_next);
+      entry(1, page_n2, pos_n2);
       int* s_sign = reinterpret_cast<int*>(smem + C::OFF_SIGN);
       for (int j = 0; j < n_kv; ++j) {
         const int s = j & 1, ph = (j >> 1) & 1;
         const int page = page_next;
         const int p0 = pos_next < 0 ? -pos_next : pos_next;      // negative only for LAZY_K_STORED_POS
         const int p0_sign = pos_next < 0 ? -1 : 1;
-        if (j + 1 < n_kv) {
-          const int idx = (j + 1) * kPagesPerTile + pg;
-          page_next = idx < num_pages ? bt[idx] : 0;
-          pos_next = idx < num_pages ? ppos[idx] : 0;
-          if (KM == LAZY_K_STORED_POS) pos_next -= a.stored_pos[page_next];
-        }
+        page_next = page_n2; pos_next = pos_n2;
+        entry(j + 2, page_n2, pos_n2);
         const int npv = min(kPagesPerTile, num_pages - j * kPagesPerTile);
         const int row0 = (page * sh.Hkv + hk) * kPageSize;
         const uint32_t dst = s * C::TILE_BYTES + half * kHalfBytes + pg * (kPageSize * 128);
@@ -388,8 +413,16 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     constexpr int PASSES = kPagesPerTile / PPP;
     const int wtid = tid - 256;
     const int pp_ = wtid / TPP, t = (wtid % TPP) / C::CPR, c = wtid % C::CPR;
-    float uc[8], us[8];                             // e^{i t theta_j}: in-page offset, fixed per thread
-    if (KM == LAZY_K_UNROTATED) load_cs8<D>(a.cs + (size_t)t * (D / 2), c, uc, us);
+    float2 uc[4], us[4];                            // e^{i t theta_j}: in-page offset, fixed per thread
+    if (KM == LAZY_K_UNROTATED) {
+      const float4* urow = reinterpret_cast<const float4*>(a.cs + (size_t)t * (D / 2));
+#pragma unroll
+      for (int x = 0; x < 4; ++x) {
+        const float4 v = __ldg(urow + cs_f4_index<D>(c, x));
+        uc[x] = make_float2(v.x, v.y);
+        us[x] = make_float2(v.z, v.w);
+      }
+    }
     const int* s_sign = reinterpret_cast<const int*>(smem + C::OFF_SIGN);
     for (int j = 0; j < n_kv; ++j) {
       const int s = j & 1;
@@ -402,23 +435,29 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       for (int ps = 0; ps < PASSES; ++ps) {
         const int i = ps * PPP + pp_;
         if (KM != LAZY_K_ABSOLUTE && i < npv) {
-          float wc[8], ws[8], zc[8], zs[8];         // e^{i p0 theta_j} of the page, then e^{i (p0+t) theta_j}
-          load_cs8_smem<D>(cb + i * C::CS_ROW_BYTES, c, wc, ws);
+          float2 zc[4], zs[4];                      // e^{i (p0+t) theta_j}, or e^{i Delta theta_j} of the page
           const int row = i * kPageSize + t;
           const uint32_t pa = kb + chunk_off(row, c), pb = kb + chunk_off(row, c + C::CPR);
-          uint4 va = ptx::lds128(pa), vb = ptx::lds128(pb);
-          if (KM == LAZY_K_UNROTATED) {
 #pragma unroll
-            for (int e = 0; e < 8; ++e) {
-              zc[e] = wc[e] * uc[e] - ws[e] * us[e];
-              zs[e] = ws[e] * uc[e] + wc[e] * us[e];
+          for (int x = 0; x < 4; ++x) {
+            const uint4 v = ptx::lds128(cb + i * C::CS_ROW_BYTES + 16 * cs_f4_index<D>(c, x));
+            zc[x] = make_float2(f32(v.x), f32(v.y));
+            zs[x] = make_float2(f32(v.z), f32(v.w));
+          }
+          uint4 va = ptx::lds128(pa), vb = ptx::lds128(pb);
+          if (KM == LAZY_K_UNROTATED) {             // compose with the in-page offset: z = w * u
+#pragma unroll
+            for (int x = 0; x < 4; ++x) {
+              const float2 wc = zc[x], ws = zs[x];
+              zc[x] = __ffma2_rn(neg2(ws), us[x], __fmul2_rn(wc, uc[x]));
+              zs[x] = __ffma2_rn(wc, us[x], __fmul2_rn(ws, uc[x]));
             }
           } else {                                  // one relative rotation for the whole page (may be negative)
             const float sgn = (float)s_sign[s * kPagesPerTile + i];
 #pragma unroll
-            for (int e = 0; e < 8; ++e) { zc[e] = wc[e]; zs[e] = ws[e] * sgn; }
+            for (int x = 0; x < 4; ++x) zs[x] = __fmul2_rn(zs[x], make_float2(sgn, sgn));
           }
-          rotate8(va, vb, zc, zs);
+          rotate8_packed(va, vb, zc, zs);
           ptx::sts128(pa, va);
           ptx::sts128(pb, vb);
         }

@@ -268,13 +268,20 @@ __device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.
 
 }  // namespace ptx
 
-// Layout of one row of the cos/sin table (D/2 float2 entries): entries are permuted so that the 16-byte chunk
-// (k*4 + tq) holds (cos,sin) of j = JT*tq + 2k and j+1, JT = D/8: the decode kernel's thread (g, tq) then
-// reads its rotation pairs with conflict-free 16-byte loads.  Every kernel goes through this function.
-__host__ __device__ __forceinline__ int cs_index(int j, int D) {
+// Layout of one row of the cos/sin table (D floats = D/2 (cos, sin) entries, kept behind a float2* for its 8-byte
+// alignment): 16-byte chunk (k*4 + tq) holds (cos j, cos j+1, sin j, sin j+1) for j = JT*tq + 2k, JT = D/8.
+// Thread (g, tq) of the decode kernel reads its rotation pairs with conflict-free 16-byte loads, and the cos and
+// the sin of two neighbouring pairs sit in adjacent registers, ready for packed f32x2 arithmetic.
+// Every kernel goes through these functions.
+__host__ __device__ __forceinline__ int cs_cos_index(int j, int D) {   // float index of cos j; sin j is 2 further
   int JT = D / 8;
   int tq = j / JT, i = j % JT;
-  return ((i >> 1) * 4 + tq) * 2 + (i & 1);
+  return ((i >> 1) * 4 + tq) * 4 + (i & 1);
+}
+__device__ __forceinline__ float2 cs_load(const float2* __restrict__ row, int j, int D) {   // (cos j, sin j)
+  const float* f = reinterpret_cast<const float*>(row);
+  const int k = cs_cos_index(j, D);
+  return make_float2(__ldg(f + k), __ldg(f + k + 2));
 }
 
 }  // namespace lazy
