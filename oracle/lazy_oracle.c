@@ -61,6 +61,37 @@ void lazy_oracle_rope(const double* x, double pos, int D, double theta, double* 
     }
 }
 
+/* Positional variants (section 3.5).  NULL means the default above.
+ *   rope_style 0  half-split pairing (j, j + D/2)
+ *              1  interleaved pairing (2j, 2j + 1)                       (L215 "interleaved")
+ *   inv_freq      optional [D/2] rotation frequency of pair j, replacing theta^(-2j/D): frequency-scaled RoPE
+ *                 families (Llama-3.1 / NTK / YaRN, L213 "variant-specific scaling metadata"); a pair with
+ *                 frequency 0 is not rotated (partial rotary)
+ *   scale         softmax scale replacing 1/sqrt(D) when > 0 (YaRN's attention temperature folds in here)
+ *   alibi_slopes  optional [Hq]: ALiBi (L221): NO rotation at all; the score of query position m and key position
+ *                 n gets the bias  slope_h * (n - m)  added after scaling                                        */
+typedef struct lazy_oracle_variant {
+    int rope_style;
+    const double* inv_freq;
+    double scale;
+    const double* alibi_slopes;
+} lazy_oracle_variant;
+
+void lazy_oracle_rope_variant(const double* x, double pos, int D, double theta, const lazy_oracle_variant* var,
+                              double* y) {
+    int half = D / 2;
+    if (var && var->alibi_slopes) { for (int d = 0; d < D; ++d) y[d] = x[d]; return; }
+    for (int j = 0; j < half; ++j) {
+        double f = (var && var->inv_freq) ? var->inv_freq[j] : pow(theta, -2.0 * (double)j / (double)D);
+        double a = pos * f;
+        double c = cos(a), s = sin(a);
+        int i1 = (var && var->rope_style == 1) ? 2 * j : j;
+        int i2 = (var && var->rope_style == 1) ? 2 * j + 1 : j + half;
+        y[i1] = x[i1] * c - x[i2] * s;
+        y[i2] = x[i1] * s + x[i2] * c;
+    }
+}
+
 /* Core: attention of n_q query rows over L keys with explicit positions.
  *   q      [n_q][Hq][D]   un-rotated queries
  *   k, v   [L][Hkv][D]    un-rotated keys, values (already gathered)
@@ -73,12 +104,34 @@ void lazy_oracle_rope(const double* x, double pos, int D, double theta, double* 
  * Step 1 materialises Khat = R_{pos_k} K (the "duplicate + re-encode" copy),
  * step 2 is Eq. 4 on (R_{pos_q} q, Khat, V).
  */
+int lazy_oracle_attend_core_ex(const double* q, const double* k, const double* v,
+                               const double* pos_q, const double* pos_k, const int64_t* vis,
+                               int n_q, int64_t L, int Hq, int Hkv, int D, double theta,
+                               const lazy_oracle_variant* var, const double* bias_pos_k,
+                               const uint8_t* row_select,
+                               double* out, double* probs, double* khat_out, double* qhat_out);
+
 int lazy_oracle_attend_core(const double* q, const double* k, const double* v,
                             const double* pos_q, const double* pos_k, const int64_t* vis,
                             int n_q, int64_t L, int Hq, int Hkv, int D, double theta,
                             const uint8_t* row_select,
                             double* out, double* probs, double* khat_out, double* qhat_out) {
+    return lazy_oracle_attend_core_ex(q, k, v, pos_q, pos_k, vis, n_q, L, Hq, Hkv, D, theta, NULL, NULL,
+                                      row_select, out, probs, khat_out, qhat_out);
+}
+
+/* Same with a positional variant.  bias_pos_k (optional, [L]) are the key positions the ALiBi bias uses when they
+ * differ from pos_k (pos_k is the rotation still owed to a key, which a stored-position cache makes different from
+ * its logical position); NULL = pos_k. */
+int lazy_oracle_attend_core_ex(const double* q, const double* k, const double* v,
+                               const double* pos_q, const double* pos_k, const int64_t* vis,
+                               int n_q, int64_t L, int Hq, int Hkv, int D, double theta,
+                               const lazy_oracle_variant* var, const double* bias_pos_k,
+                               const uint8_t* row_select,
+                               double* out, double* probs, double* khat_out, double* qhat_out) {
     if (Hq % Hkv != 0 || D % 2 != 0) return -1;
+    const double sm_scale = (var && var->scale > 0.0) ? var->scale : 1.0 / sqrt((double)D);
+    if (!bias_pos_k) bias_pos_k = pos_k;
     int group = Hq / Hkv;
     double* khat = (double*)malloc(sizeof(double) * (size_t)(L > 0 ? L : 1) * Hkv * D);
     if (!khat) return -2;
@@ -86,8 +139,8 @@ int lazy_oracle_attend_core(const double* q, const double* k, const double* v,
 #pragma omp parallel for schedule(static)
     for (int64_t s = 0; s < L; ++s)
         for (int hk = 0; hk < Hkv; ++hk)
-            lazy_oracle_rope(k + ((size_t)s * Hkv + hk) * D, pos_k[s], D, theta,
-                             khat + ((size_t)s * Hkv + hk) * D);
+            lazy_oracle_rope_variant(k + ((size_t)s * Hkv + hk) * D, pos_k[s], D, theta, var,
+                                     khat + ((size_t)s * Hkv + hk) * D);
     if (khat_out) memcpy(khat_out, khat, sizeof(double) * (size_t)L * Hkv * D);
     /* 2. standard attention, one (query row, head) at a time */
     int64_t n_rows = (int64_t)n_q * Hq;
@@ -104,7 +157,7 @@ int lazy_oracle_attend_core(const double* q, const double* k, const double* v,
         double* qhat = (double*)malloc(sizeof(double) * D);
         double* sc = (double*)malloc(sizeof(double) * (size_t)(last >= 0 ? last + 1 : 1));
         if (!qhat || !sc) { err = 1; free(qhat); free(sc); continue; }
-        lazy_oracle_rope(q + ((size_t)i * Hq + hq) * D, pos_q[i], D, theta, qhat);
+        lazy_oracle_rope_variant(q + ((size_t)i * Hq + hq) * D, pos_q[i], D, theta, var, qhat);
         if (qhat_out) memcpy(qhat_out + ((size_t)i * Hq + hq) * D, qhat, sizeof(double) * D);
         if (probs) for (int64_t s = 0; s < L; ++s) probs[((size_t)i * Hq + hq) * L + s] = 0.0;
         if (last >= 0) {
@@ -113,7 +166,8 @@ int lazy_oracle_attend_core(const double* q, const double* k, const double* v,
                 const double* kr = khat + ((size_t)s * Hkv + hk) * D;
                 double acc = 0.0;
                 for (int d = 0; d < D; ++d) acc += qhat[d] * kr[d];
-                sc[s] = acc / sqrt((double)D);
+                sc[s] = acc * sm_scale;
+                if (var && var->alibi_slopes) sc[s] += var->alibi_slopes[hq] * (bias_pos_k[s] - pos_q[i]);
                 if (sc[s] > m) m = sc[s];
             }
             double l = 0.0;
@@ -166,12 +220,35 @@ int lazy_oracle_attend_paged(const void* q, int dtype_q, const void* k_pool, con
  *   k_storage 2  position-dependent cache (the standard-attention baseline of PAPER.md Fig. 5 / Table 12):
  *                K is stored already rotated at its final position, no rotation is left to do.
  * In every mode q is rotated by the logical position of its own token and the rest is Eq. 4. */
+int lazy_oracle_attend_paged_variant(const void* q, int dtype_q, const void* k_pool, const void* v_pool,
+                                     int dtype_kv, const int32_t* block_table, const int32_t* page_logical_pos,
+                                     int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
+                                     int num_reqs, int Hq, int Hkv, int D, int P, double theta,
+                                     int k_storage, const int32_t* page_stored_pos,
+                                     int rope_style, const double* inv_freq, double scale, const double* alibi_slopes,
+                                     const uint8_t* row_select, double* out);
+
 int lazy_oracle_attend_paged_stored(const void* q, int dtype_q, const void* k_pool, const void* v_pool,
                                     int dtype_kv, const int32_t* block_table, const int32_t* page_logical_pos,
                                     int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
                                     int num_reqs, int Hq, int Hkv, int D, int P, double theta,
                                     int k_storage, const int32_t* page_stored_pos,
                                     const uint8_t* row_select, double* out) {
+    return lazy_oracle_attend_paged_variant(q, dtype_q, k_pool, v_pool, dtype_kv, block_table, page_logical_pos,
+                                            table_stride, seq_lens, cu_q_lens, num_reqs, Hq, Hkv, D, P, theta,
+                                            k_storage, page_stored_pos, 0, NULL, 0.0, NULL, row_select, out);
+}
+
+/* ... and with a positional variant (lazy_oracle_variant above). */
+int lazy_oracle_attend_paged_variant(const void* q, int dtype_q, const void* k_pool, const void* v_pool,
+                                     int dtype_kv, const int32_t* block_table, const int32_t* page_logical_pos,
+                                     int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
+                                     int num_reqs, int Hq, int Hkv, int D, int P, double theta,
+                                     int k_storage, const int32_t* page_stored_pos,
+                                     int rope_style, const double* inv_freq, double scale, const double* alibi_slopes,
+                                     const uint8_t* row_select, double* out) {
+    lazy_oracle_variant var;
+    var.rope_style = rope_style; var.inv_freq = inv_freq; var.scale = scale; var.alibi_slopes = alibi_slopes;
     if (k_storage < 0 || k_storage > 2 || (k_storage == 1 && !page_stored_pos)) return -1;
     for (int r = 0; r < num_reqs; ++r) {
         int64_t L = seq_lens[r];
@@ -219,9 +296,9 @@ int lazy_oracle_attend_paged_stored(const void* q, int dtype_q, const void* k_po
             vis[i] = sq;
             pos_q[i] = pos[sq];
         }
-        int rc = lazy_oracle_attend_core(qd, kg, vg, pos_q, rot, vis, n_q, L, Hq, Hkv, D, theta,
-                                         row_select ? row_select + q0 : NULL,
-                                         out + (size_t)q0 * Hq * D, NULL, NULL, NULL);
+        int rc = lazy_oracle_attend_core_ex(qd, kg, vg, pos_q, rot, vis, n_q, L, Hq, Hkv, D, theta, &var, pos,
+                                            row_select ? row_select + q0 : NULL,
+                                            out + (size_t)q0 * Hq * D, NULL, NULL, NULL);
         free(kg); free(vg); free(pos); free(rot); free(qd); free(pos_q); free(vis);
         if (rc) return rc;
     }

@@ -66,7 +66,14 @@ def rope(x, pos: float, theta: float) -> np.ndarray:
     return y
 
 
-def attend_core(q, k, v, pos_q, pos_k, vis, theta: float, row_select=None, want_probs=False, want_hats=False):
+class Variant(ctypes.Structure):
+    """Mirror of lazy_oracle_variant (positional variants)."""
+    _fields_ = [("rope_style", ctypes.c_int), ("inv_freq", ctypes.c_void_p), ("scale", ctypes.c_double),
+                ("alibi_slopes", ctypes.c_void_p)]
+
+
+def attend_core(q, k, v, pos_q, pos_k, vis, theta: float, row_select=None, want_probs=False, want_hats=False,
+                rope_style: int = 0, inv_freq=None, scale: float = 0.0, alibi_slopes=None):
     """q [n_q,Hq,D], k/v [L,Hkv,D] float64; returns out (and probs [n_q,Hq,L], khat, qhat if asked)."""
     q = np.ascontiguousarray(np.asarray(q, dtype=np.float64))
     k = np.ascontiguousarray(np.asarray(k, dtype=np.float64))
@@ -81,11 +88,15 @@ def attend_core(q, k, v, pos_q, pos_k, vis, theta: float, row_select=None, want_
     khat = np.zeros((L, Hkv, D), dtype=np.float64) if want_hats else None
     qhat = np.zeros((n_q, Hq, D), dtype=np.float64) if want_hats else None
     rs = None if row_select is None else np.ascontiguousarray(np.asarray(row_select, dtype=np.uint8))
-    f = lib().lazy_oracle_attend_core
+    fr = None if inv_freq is None else np.ascontiguousarray(np.asarray(inv_freq, dtype=np.float64))
+    sl = None if alibi_slopes is None else np.ascontiguousarray(np.asarray(alibi_slopes, dtype=np.float64))
+    var = Variant(int(rope_style), None if fr is None else fr.ctypes.data, float(scale),
+                  None if sl is None else sl.ctypes.data)
+    f = lib().lazy_oracle_attend_core_ex
     f.restype = ctypes.c_int
     rc = f(_p(q), _p(k), _p(v), _p(pos_q), _p(pos_k), _p(vis), ctypes.c_int(n_q), ctypes.c_int64(L),
-           ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(D), ctypes.c_double(theta), _p(rs),
-           _p(out), _p(probs), _p(khat), _p(qhat))
+           ctypes.c_int(Hq), ctypes.c_int(Hkv), ctypes.c_int(D), ctypes.c_double(theta), ctypes.byref(var), None,
+           _p(rs), _p(out), _p(probs), _p(khat), _p(qhat))
     if rc != 0:
         raise RuntimeError(f"lazy_oracle_attend_core failed: {rc}")
     res = [out]
@@ -98,7 +109,8 @@ def attend_core(q, k, v, pos_q, pos_k, vis, theta: float, row_select=None, want_
 
 def attend_paged(q, k_pool, v_pool, block_table, page_logical_pos, seq_lens, cu_q_lens, *,
                  num_q_heads: int, num_kv_heads: int, head_dim: int, page_size: int, theta: float,
-                 row_select=None, k_storage: int = 0, page_stored_pos=None) -> np.ndarray:
+                 row_select=None, k_storage: int = 0, page_stored_pos=None, rope_style: int = 0, inv_freq=None,
+                 scale: float = 0.0, alibi_slopes=None) -> np.ndarray:
     """Paged interface.  q [total_q,Hq,D]; pools [num_pages,Hkv,P,D] (torch bf16 or float arrays).
     k_storage 0: pages hold un-rotated K; 1: page g holds K rotated at page_stored_pos[g] + t (the paper's
     document-local layout); 2: K already rotated at its final position.
@@ -117,14 +129,17 @@ def attend_paged(q, k_pool, v_pool, block_table, page_logical_pos, seq_lens, cu_
     out = np.zeros((total_q, num_q_heads, head_dim), dtype=np.float64)
     rs = None if row_select is None else np.ascontiguousarray(np.asarray(row_select, dtype=np.uint8))
     sp = None if page_stored_pos is None else np.ascontiguousarray(np.asarray(page_stored_pos, dtype=np.int32))
-    f = lib().lazy_oracle_attend_paged_stored
+    fr = None if inv_freq is None else np.ascontiguousarray(np.asarray(inv_freq, dtype=np.float64))
+    al = None if alibi_slopes is None else np.ascontiguousarray(np.asarray(alibi_slopes, dtype=np.float64))
+    f = lib().lazy_oracle_attend_paged_variant
     f.restype = ctypes.c_int
     rc = f(_p(qa), ctypes.c_int(dq), _p(ka), _p(va), ctypes.c_int(dk), _p(bt), _p(pp),
            ctypes.c_int64(bt.shape[1]), _p(sl), _p(cu), ctypes.c_int(R), ctypes.c_int(num_q_heads),
            ctypes.c_int(num_kv_heads), ctypes.c_int(head_dim), ctypes.c_int(page_size), ctypes.c_double(theta),
-           ctypes.c_int(k_storage), _p(sp), _p(rs), _p(out))
+           ctypes.c_int(k_storage), _p(sp), ctypes.c_int(rope_style), _p(fr), ctypes.c_double(scale), _p(al),
+           _p(rs), _p(out))
     if rc != 0:
-        raise RuntimeError(f"lazy_oracle_attend_paged_stored failed: {rc}")
+        raise RuntimeError(f"lazy_oracle_attend_paged_variant failed: {rc}")
     return out
 
 

@@ -451,3 +451,117 @@ def test_stored_position_layouts_equal_unrotated_cache():
     assert np.abs(got - base).max() < 1e-10
     # and the oracle's own materialiser builds exactly those copies
     assert np.abs(oracle.materialize_pages(kp, src, starts, True, theta) - kp_abs).max() < 1e-12
+
+
+# ---- positional variants (section 3.5) ----------------------------------
+def brute_force_variant(q, k, v, pos_q, pos_k, vis, theta, pairing="half", inv_freq=None, scale=None, slopes=None):
+    """Independent statement for the variants: explicit 2x2 rotation of the pair (i1, i2) by (n - m) * f_j, an
+    arbitrary frequency vector, an arbitrary softmax scale, or (ALiBi) no rotation and the bias slope * (n - m)."""
+    n_q, Hq, D = q.shape
+    L, Hkv, _ = k.shape
+    h = D // 2
+    f = np.asarray(inv_freq) if inv_freq is not None else theta ** (-2.0 * np.arange(h) / D)
+    sc = scale if scale else 1.0 / math.sqrt(D)
+    out = np.zeros((n_q, Hq, D))
+    for i in range(n_q):
+        for hq in range(Hq):
+            hk = hq // (Hq // Hkv)
+            w = np.zeros(L)
+            for s in range(L):
+                if s > vis[i]:
+                    continue
+                rel = pos_k[s] - pos_q[i]
+                if slopes is not None:
+                    acc = float(q[i, hq] @ k[s, hk]) * sc + slopes[hq] * rel
+                else:
+                    acc = 0.0
+                    for j in range(h):
+                        i1, i2 = (2 * j, 2 * j + 1) if pairing == "interleaved" else (j, j + h)
+                        a = rel * f[j]
+                        acc += q[i, hq, i1] * (math.cos(a) * k[s, hk, i1] - math.sin(a) * k[s, hk, i2])
+                        acc += q[i, hq, i2] * (math.sin(a) * k[s, hk, i1] + math.cos(a) * k[s, hk, i2])
+                    acc *= sc
+                w[s] = math.exp(acc)
+            w /= w.sum()
+            for s in range(L):
+                out[i, hq] += w[s] * v[s, hk]
+    return out
+
+
+def test_interleaved_pairing_brute_force_and_permutation():
+    """L215: interleaved pairing (2j, 2j+1).  Brute force; and the fact the CUDA path relies on: interleaved RoPE is
+    half-split RoPE on de-interleaved vectors (dims 0,2,4,... then 1,3,5,...), applied to q and k alike."""
+    q, k, v, pos_q, pos_k, vis = random_case(71, n_q=3, L=9, Hq=4, Hkv=2, D=8)
+    out = oracle.attend_core(q, k, v, pos_q, pos_k, vis, 1e4, rope_style=1)
+    ref = brute_force_variant(q, k, v, pos_q, pos_k, vis, 1e4, pairing="interleaved")
+    assert np.abs(out - ref).max() < 1e-12
+    half = oracle.attend_core(q, k, v, pos_q, pos_k, vis, 1e4)
+    assert np.abs(out - half).max() > 1e-3                      # the two pairings are different functions
+    perm = np.concatenate([np.arange(0, 8, 2), np.arange(1, 8, 2)])
+    via_perm = oracle.attend_core(q[..., perm], k[..., perm], v, pos_q, pos_k, vis, 1e4)
+    assert np.abs(out - via_perm).max() < 1e-12
+    # SURVEY 8.c worked example B, interleaved reading: D=4, K rows (0,1,0,0), q=(0,2,0,0), keys at 0/100/200,
+    # query at 200: index 1 pairs with index 0 at frequency 1 -> scores cos(200-n), n = 0, 100, 200
+    kk = np.zeros((3, 1, 4)); kk[:, 0, 1] = 1.0
+    vv = np.eye(3, 4).reshape(3, 1, 4)
+    qq = np.array([[[0.0, 2.0, 0.0, 0.0]]])
+    o = oracle.attend_core(qq, kk, vv, [200.0], [0.0, 100.0, 200.0], [2], 1e4, rope_style=1)
+    e = np.exp(np.cos(np.array([200.0, 100.0, 0.0])))
+    assert np.abs(o[0, 0, :3] - e / e.sum()).max() < 1e-12
+
+
+def test_custom_frequencies_scale_and_partial_rotary():
+    """L213: frequency-scaled RoPE families only change the per-pair frequency vector (and YaRN a scalar
+    temperature).  Default vector reproduces the default path bit for bit; an arbitrary vector and scale match
+    brute force; zero frequencies leave those pairs un-rotated (partial rotary)."""
+    q, k, v, pos_q, pos_k, vis = random_case(73, n_q=2, L=10, Hq=2, Hkv=1, D=8)
+    theta = 5e5
+    base = theta ** (-2.0 * np.arange(4) / 8)
+    a = oracle.attend_core(q, k, v, pos_q, pos_k, vis, theta)
+    b = oracle.attend_core(q, k, v, pos_q, pos_k, vis, theta, inv_freq=base)
+    assert np.array_equal(a, b)
+    # a Llama-3.1-style rescaling written out here: low frequencies divided by 8, high kept, middle blended
+    wavelen = 2 * math.pi / base
+    lo, hi, factor, orig = 1.0, 4.0, 8.0, 64.0
+    smooth = np.clip((orig / wavelen - lo) / (hi - lo), 0.0, 1.0)
+    scaled = np.where(wavelen > orig / lo, base / factor, np.where(wavelen < orig / hi, base,
+                                                                  (1 - smooth) * base / factor + smooth * base))
+    out = oracle.attend_core(q, k, v, pos_q, pos_k, vis, theta, inv_freq=scaled, scale=0.41)
+    ref = brute_force_variant(q, k, v, pos_q, pos_k, vis, theta, inv_freq=scaled, scale=0.41)
+    assert np.abs(out - ref).max() < 1e-12
+    # partial rotary: pairs 2, 3 carry frequency 0 -> those dims behave as with all positions 0
+    part = base.copy(); part[2:] = 0.0
+    out = oracle.attend_core(q, k, v, pos_q, pos_k, vis, theta, inv_freq=part)
+    ref = brute_force_variant(q, k, v, pos_q, pos_k, vis, theta, inv_freq=part)
+    assert np.abs(out - ref).max() < 1e-12
+
+
+def test_alibi_bias_brute_force_closed_form_and_paged():
+    """L221: ALiBi -- no rotation, score bias slope_h * (n - m).  Brute force; closed form with q = 0 (weights
+    proportional to exp(slope * n)); shift invariance; and through the paged wrapper, where the bias must use the
+    LOGICAL position of a page (same page at two positions -> different biases)."""
+    q, k, v, pos_q, pos_k, vis = random_case(79, n_q=3, L=12, Hq=4, Hkv=2, D=8)
+    slopes = np.array([0.5, 0.25, 0.125, 0.0625])
+    out = oracle.attend_core(q, k, v, pos_q, pos_k, vis, 1e4, alibi_slopes=slopes)
+    ref = brute_force_variant(q, k, v, pos_q, pos_k, vis, 1e4, slopes=slopes)
+    assert np.abs(out - ref).max() < 1e-12
+    out2 = oracle.attend_core(q, k, v, pos_q + 1000, pos_k + 1000, vis, 1e4, alibi_slopes=slopes)
+    assert np.abs(out - out2).max() < 1e-10
+    z = oracle.attend_core(np.zeros_like(q), k, v, pos_q, pos_k, vis, 1e4, alibi_slopes=slopes, want_probs=True)[1]
+    for i in range(3):
+        for hq in range(4):
+            w = np.exp(slopes[hq] * (pos_k[: vis[i] + 1] - pos_k[vis[i]]))
+            assert np.abs(z[i, hq, : vis[i] + 1] - w / w.sum()).max() < 1e-12
+    r = _rng(83)
+    Hq, Hkv, D, P = 2, 1, 8, 4
+    kp = r.standard_normal((3, Hkv, P, D)); vp = r.standard_normal((3, Hkv, P, D))
+    bt = np.array([[1, 0, 1, 2]], np.int32); pp = np.array([[0, 4, 30, 34]], np.int32)   # page 1 at 0 and at 30
+    sl = np.array([14], np.int32); cu = np.array([0, 2], np.int32)
+    qq = r.standard_normal((2, Hq, D)); s2 = np.array([0.3, 0.05])
+    got = oracle.attend_paged(qq, kp, vp, bt, pp, sl, cu, num_q_heads=Hq, num_kv_heads=Hkv, head_dim=D, page_size=P,
+                              theta=1e4, alibi_slopes=s2)
+    kk = np.stack([kp[bt[0, s // P], :, s % P] for s in range(14)])
+    vv = np.stack([vp[bt[0, s // P], :, s % P] for s in range(14)])
+    pos = np.array([pp[0, s // P] + s % P for s in range(14)], dtype=np.float64)
+    ref = brute_force_variant(qq, kk, vv, pos[12:], pos, np.array([12, 13]), 1e4, slopes=s2)
+    assert np.abs(got - ref).max() < 1e-12
