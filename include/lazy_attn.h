@@ -58,11 +58,22 @@ typedef struct lazy_config {
   int32_t max_reqs;          /* upper bound on num_reqs of any call                             */
   int32_t max_pages_per_req; /* row stride (in entries) of block_table and page_logical_pos     */
   double  rope_theta;        /* 1e4, 5e5, 1e6 ...                                               */
-  int32_t rope_style;        /* 0 = half-split (the only style)                                 */
+  int32_t rope_style;        /* LAZY_ROPE_* : pairing of the rotated dimensions (0 = half-split)  */
   int32_t dtype;             /* 0 = bf16 (the only dtype)                                       */
   int32_t flags;             /* LAZY_FLAG_* (0 for production)                                  */
   int32_t k_storage;         /* LAZY_K_* : how the pages hold K (0 = un-rotated, the product)    */
 } lazy_config;
+
+/* rope_style (section 3.5).
+ *   LAZY_ROPE_HALF_SPLIT  pair (j, j + D/2)  (the product path).
+ *   LAZY_ROPE_INTERLEAVED pair (2j, 2j + 1)  (L215).  q and k_new arrive in the model's own dimension order;
+ *                         lazy_cache_write stores K rows DE-INTERLEAVED (dims 0,2,4,... then 1,3,5,...), which is
+ *                         still position-free, and the attention kernels de-interleave q on load: interleaved RoPE
+ *                         on x equals half-split RoPE on de-interleaved x, and a dot product does not care about a
+ *                         permutation applied to both operands.  k_cache's last axis is therefore in that order
+ *                         (V and every output are untouched). */
+#define LAZY_ROPE_HALF_SPLIT  0
+#define LAZY_ROPE_INTERLEAVED 1
 
 /* k_storage: what a physical page's K rows carry (V is position-free in every mode).
  *   LAZY_K_UNROTATED  the product path (north_star): K is the projection output, the kernels
@@ -130,6 +141,14 @@ int lazy_attn_prefill(lazy_handle* h, const void* q, const void* k_cache, const 
 int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                      const int32_t* block_table, const int32_t* page_logical_pos,
                      const int32_t* seq_lens, int32_t num_reqs, void* out, void* stream);
+
+/* f3. Frequency-scaled RoPE families (Llama-3.1 / NTK / YaRN scaling only change "variant-specific
+ * scaling metadata").  Replaces the rotation frequency of pair j, theta_j = rope_theta^(-2j/D), by inv_freq[j]
+ * (HOST array of head_dim/2 doubles; NULL restores the default) and rebuilds the fp64-built cos/sin table on `stream`
+ * (one launch; attention calls enqueued later on the same stream see the new table).  A pair with frequency 0 is
+ * not rotated (partial rotary).  softmax_scale > 0 replaces 1/sqrt(head_dim) (YaRN's attention temperature);
+ * 0 keeps the current one. */
+int lazy_set_rope_frequencies(lazy_handle* h, const double* inv_freq, double softmax_scale, void* stream);
 
 /* LAZY_K_STORED_POS only: device array [num_pages] int32, position at which token 0 of each physical page
  * was rotated when it was stored.  The pointer is kept (not copied) and read by every later attention call;

@@ -179,7 +179,7 @@ def cache_write(k_new, v_new, slot_mapping, k_pool, v_pool, page_size: int) -> N
         raise RuntimeError(f"lazy_oracle_cache_write failed: {rc}")
 
 
-def run_step(batch, step, k_pool, v_pool, row_select=None) -> Optional[np.ndarray]:
+def run_step(batch, step, k_pool, v_pool, row_select=None, **variant) -> Optional[np.ndarray]:
     """Apply one workloads.Step with the oracle: cache write (in place on the given pool copies),
     then the attention call.  Returns the fp64 output or None for write-only steps."""
     sh = batch.shape
@@ -192,4 +192,5 @@ def run_step(batch, step, k_pool, v_pool, row_select=None) -> Optional[np.ndarra
         bt, pp = bt[step.req_ids], pp[step.req_ids]
     return attend_paged(step.q, k_pool, v_pool, bt.numpy(), pp.numpy(), step.seq_lens.numpy(),
                         step.cu_q_lens.numpy(), num_q_heads=sh.num_q_heads, num_kv_heads=sh.num_kv_heads,
-                        head_dim=sh.head_dim, page_size=sh.page_size, theta=sh.rope_theta, row_select=row_select)
+                        head_dim=sh.head_dim, page_size=sh.page_size, theta=sh.rope_theta, row_select=row_select,
+                        **variant)

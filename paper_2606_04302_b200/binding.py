@@ -16,9 +16,11 @@ LIB_PATH = os.path.join(_HERE, "csrc", "liblazyattn.so")
 LAZY_OK, LAZY_ERR_INVALID, LAZY_ERR_UNSUPPORTED, LAZY_ERR_WORKSPACE, LAZY_ERR_CUDA = 0, -1, -2, -3, -4
 LAZY_FLAG_ROWWISE_KERNELS = 1
 LAZY_K_UNROTATED, LAZY_K_STORED_POS, LAZY_K_ABSOLUTE = 0, 1, 2
+LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED = 0, 1
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
-           "lazy_attn_decode", "lazy_set_page_stored_pos", "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step"]
+           "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_page_stored_pos",
+           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step"]
 
 
 class LazyConfig(ctypes.Structure):
@@ -53,6 +55,8 @@ def lib() -> ctypes.CDLL:
         L.lazy_attn_prefill.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, vp]
         L.lazy_attn_decode.restype = ctypes.c_int
         L.lazy_attn_decode.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, vp, vp]
+        L.lazy_set_rope_frequencies.restype = ctypes.c_int
+        L.lazy_set_rope_frequencies.argtypes = [vp, vp, ctypes.c_double, vp]
         L.lazy_set_page_stored_pos.restype = ctypes.c_int
         L.lazy_set_page_stored_pos.argtypes = [vp, vp]
         L.lazy_materialize_pages.restype = ctypes.c_int
@@ -132,9 +136,10 @@ class LazyHandle:
 
 def lazy_create(num_q_heads: int, num_kv_heads: int, head_dim: int, *, num_pages: int, max_position: int,
                 max_reqs: int, max_pages_per_req: int, rope_theta: float, page_size: int = 16, flags: int = 0,
-                k_storage: int = LAZY_K_UNROTATED, device="cuda", stream=None) -> LazyHandle:
+                k_storage: int = LAZY_K_UNROTATED, rope_style: int = LAZY_ROPE_HALF_SPLIT, device="cuda",
+                stream=None) -> LazyHandle:
     cfg = LazyConfig(num_q_heads, num_kv_heads, head_dim, page_size, num_pages, max_position, max_reqs,
-                     max_pages_per_req, float(rope_theta), 0, 0, flags, k_storage)
+                     max_pages_per_req, float(rope_theta), rope_style, 0, flags, k_storage)
     return LazyHandle(cfg, device=device, stream=stream)
 
 
@@ -168,6 +173,19 @@ def lazy_attn_decode(h: LazyHandle, q, k_cache, v_cache, block_table, page_logic
                                 _ptr(page_logical_pos), _ptr(seq_lens), num_reqs, _ptr(out), _stream(stream))
     if rc != 0:
         raise LazyError("lazy_attn_decode", rc)
+
+
+def lazy_set_rope_frequencies(h: LazyHandle, inv_freq=None, softmax_scale: float = 0.0, stream=None) -> None:
+    """inv_freq: sequence of head_dim/2 floats (host) or None for the default theta^(-2j/D)."""
+    arr = None
+    if inv_freq is not None:
+        vals = [float(x) for x in inv_freq]
+        if len(vals) != h.cfg.head_dim // 2:
+            raise LazyError("lazy_set_rope_frequencies", LAZY_ERR_INVALID)
+        arr = (ctypes.c_double * len(vals))(*vals)
+    rc = lib().lazy_set_rope_frequencies(h.ptr, arr, float(softmax_scale), _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_set_rope_frequencies", rc)
 
 
 def lazy_set_page_stored_pos(h: LazyHandle, page_stored_pos) -> None:

@@ -7,33 +7,42 @@
 //  * rowwise_attn   : one CTA per (query row, q head), keys strided over 4 warps, K rotated by its absolute
 //    angle from the table, online softmax.  It follows PAPER.md Eq. 4 (L94-106) directly and is kept as the
 //    LAZY_FLAG_ROWWISE_KERNELS debugging path; the production kernels are decode_splitkv.cu / prefill_umma.cu.
+#include <cmath>
+
 #include "lazy_internal.h"
 #include "ptx_util.cuh"
 
 namespace lazy {
 
-__global__ void build_cs_table_kernel(float2* __restrict__ cs, int max_position, int half, double theta, int D) {
+struct FreqTable { double f[64]; };   // rotation frequency of pair j (head_dim / 2 <= 64 entries), by value
+
+__global__ void build_cs_table_kernel(float2* __restrict__ cs, int max_position, int half, FreqTable freq, int D) {
   long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   long long total = (long long)max_position * half;
   if (idx >= total) return;
   int j = (int)(idx % half);
   long long pos = idx / half;
-  double inv_freq = pow(theta, -2.0 * (double)j / (double)D);
   double s, c;
-  sincos((double)pos * inv_freq, &s, &c);
+  sincos((double)pos * freq.f[j], &s, &c);
   float* row = reinterpret_cast<float*>(cs + pos * half);
   const int k = cs_cos_index(j, D);
   row[k] = (float)c;
   row[k + 2] = (float)s;
 }
 
-int launch_build_tables(lazy_handle* h, cudaStream_t stream) {
+// inv_freq_host == nullptr: theta_j = rope_theta^(-2j/D) (RoPE), computed here in fp64
+int launch_build_tables(lazy_handle* h, const double* inv_freq_host, cudaStream_t stream) {
   int half = h->cfg.head_dim / 2;
+  FreqTable ft;
+  for (int j = 0; j < 64; ++j)
+    ft.f[j] = j >= half ? 0.0
+              : inv_freq_host ? inv_freq_host[j]
+                              : pow(h->cfg.rope_theta, -2.0 * (double)j / (double)h->cfg.head_dim);
   long long total = (long long)h->cfg.max_position * half;
   int threads = 256;
   long long blocks = (total + threads - 1) / threads;
-  build_cs_table_kernel<<<(unsigned)blocks, threads, 0, stream>>>(h->ws.cs, h->cfg.max_position, half,
-                                                                 h->cfg.rope_theta, h->cfg.head_dim);
+  build_cs_table_kernel<<<(unsigned)blocks, threads, 0, stream>>>(h->ws.cs, h->cfg.max_position, half, ft,
+                                                                 h->cfg.head_dim);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
 
@@ -42,7 +51,7 @@ int launch_build_tables(lazy_handle* h, cudaStream_t stream) {
 // chunk index c in [0, T*Hkv*D/8): token = c / (Hkv*D/8), head = (c / (D/8)) % Hkv, part = c % (D/8).
 __global__ void cache_write_kernel(const uint4* __restrict__ k_new, const uint4* __restrict__ v_new,
                                    const long long* __restrict__ slot_mapping, long long num_chunks,
-                                   int Hkv, int chunks_per_row, uint4* __restrict__ k_cache,
+                                   int Hkv, int chunks_per_row, int deinterleave, uint4* __restrict__ k_cache,
                                    uint4* __restrict__ v_cache) {
   long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= num_chunks) return;
@@ -55,7 +64,21 @@ __global__ void cache_write_kernel(const uint4* __restrict__ k_new, const uint4*
   long long page = slot / kPageSize;
   int off = (int)(slot % kPageSize);
   long long dst = (((page * Hkv + head) * kPageSize) + off) * chunks_per_row + part;
-  k_cache[dst] = k_new[c];
+  if (!deinterleave) {
+    k_cache[dst] = k_new[c];
+  } else {
+    // LAZY_ROPE_INTERLEAVED: stored dim d' < D/2 is model dim 2d', stored dim D/2 + d' is model dim 2d' + 1
+    // (still position-free; only the order of the dimensions changes, include/lazy_attn.h)
+    const int half_chunks = chunks_per_row / 2;
+    const int hi = part >= half_chunks;                          // this chunk holds the odd (x2) elements
+    const uint4* src = k_new + (c - part) + 2 * (part - hi * half_chunks);   // 16 model dims = two chunks
+    const uint4 s0 = src[0], s1 = src[1];
+    const uint32_t sel = hi ? 0x7632u : 0x5410u;
+    uint4 o;
+    o.x = __byte_perm(s0.x, s0.y, sel); o.y = __byte_perm(s0.z, s0.w, sel);
+    o.z = __byte_perm(s1.x, s1.y, sel); o.w = __byte_perm(s1.z, s1.w, sel);
+    k_cache[dst] = o;
+  }
   v_cache[dst] = v_new[c];
 }
 
@@ -68,7 +91,7 @@ int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, con
   cache_write_kernel<<<(unsigned)blocks, threads, 0, stream>>>(
       static_cast<const uint4*>(k_new), static_cast<const uint4*>(v_new),
       reinterpret_cast<const long long*>(slot_mapping), num_chunks, h->cfg.num_kv_heads, chunks_per_row,
-      static_cast<uint4*>(k_cache), static_cast<uint4*>(v_cache));
+      h->cfg.rope_style == LAZY_ROPE_INTERLEAVED, static_cast<uint4*>(k_cache), static_cast<uint4*>(v_cache));
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
 
@@ -147,7 +170,8 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
                     const __nv_bfloat16* __restrict__ v_cache, const int* __restrict__ block_table,
                     const int* __restrict__ page_pos, const int* __restrict__ seq_lens,
                     const int* __restrict__ cu_q_lens, int num_reqs, Shape sh, const float2* __restrict__ cs,
-                    int k_storage, const int* __restrict__ stored_pos, __nv_bfloat16* __restrict__ out) {
+                    int k_storage, const int* __restrict__ stored_pos, int q_interleaved,
+                    __nv_bfloat16* __restrict__ out) {
   constexpr int HALF = D / 2;
   constexpr int PER = D / 64;
   const int row = blockIdx.x;
@@ -182,7 +206,8 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
 #pragma unroll
     for (int e = 0; e < PER; ++e) {
       int j = lane * PER + e;
-      float a = __bfloat162float(qp[j]), b = __bfloat162float(qp[j + HALF]);
+      float a = __bfloat162float(qp[q_interleaved ? 2 * j : j]);
+      float b = __bfloat162float(qp[q_interleaved ? 2 * j + 1 : j + HALF]);
       float2 t = cs_load(cs + (size_t)pos_q * HALF, j, D);
       q1[e] = (a * t.x - b * t.y) * sh.scale_log2;
       q2[e] = (a * t.y + b * t.x) * sh.scale_log2;
@@ -253,11 +278,13 @@ int launch_rowwise(lazy_handle* h, const void* q, const void* k_cache, const voi
   if (h->cfg.head_dim == 128)
     rowwise_attn_kernel<128><<<grid, 128, 0, stream>>>(qp, kp, vp, block_table, page_logical_pos, seq_lens,
                                                        cu_q_lens, num_reqs, h->shape, h->ws.cs, h->cfg.k_storage,
-                                                       h->page_stored_pos, op);
+                                                       h->page_stored_pos,
+                                                       h->cfg.rope_style == LAZY_ROPE_INTERLEAVED, op);
   else
     rowwise_attn_kernel<64><<<grid, 128, 0, stream>>>(qp, kp, vp, block_table, page_logical_pos, seq_lens,
                                                       cu_q_lens, num_reqs, h->shape, h->ws.cs, h->cfg.k_storage,
-                                                      h->page_stored_pos, op);
+                                                      h->page_stored_pos,
+                                                      h->cfg.rope_style == LAZY_ROPE_INTERLEAVED, op);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
 

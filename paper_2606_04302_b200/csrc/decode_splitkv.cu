@@ -70,6 +70,7 @@ struct DecodeArgs {
   float2* part_ml;
   int* req_counter;
   int num_reqs;
+  int q_interleaved;       // LAZY_ROPE_INTERLEAVED: q arrives with pairs (2j, 2j+1); de-interleaved on load
   Shape sh;
 };
 
@@ -243,13 +244,28 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
       for (int w = 0; w < C::NL; ++w) qraw[h][w] = 0u;
     if (g < group) {
       const uint4* qp = reinterpret_cast<const uint4*>(a.q + ((size_t)r * sh.Hq + hk * group + g) * D);
+      if (!a.q_interleaved) {
 #pragma unroll
-      for (int h = 0; h < 2; ++h)
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+          for (int x = 0; x < C::NLK; ++x) {
+            uint4 v = qp[(h * (D / 2) + C::JT * tq) / 8 + x];
+            qraw[h][4 * x + 0] = v.x; qraw[h][4 * x + 1] = v.y; qraw[h][4 * x + 2] = v.z; qraw[h][4 * x + 3] = v.w;
+          }
+      } else {
+        // model order (x1_j, x2_j) per word -> this thread's x1 words and x2 words (same pairs j as above)
 #pragma unroll
         for (int x = 0; x < C::NLK; ++x) {
-          uint4 v = qp[(h * (D / 2) + C::JT * tq) / 8 + x];
-          qraw[h][4 * x + 0] = v.x; qraw[h][4 * x + 1] = v.y; qraw[h][4 * x + 2] = v.z; qraw[h][4 * x + 3] = v.w;
+          const int j0 = C::JT * tq + 8 * x;
+          const uint4 s0 = qp[j0 / 4], s1 = qp[j0 / 4 + 1];
+          const uint32_t sw[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
+#pragma unroll
+          for (int wi = 0; wi < 4; ++wi) {
+            qraw[0][4 * x + wi] = __byte_perm(sw[2 * wi], sw[2 * wi + 1], 0x5410u);
+            qraw[1][4 * x + wi] = __byte_perm(sw[2 * wi], sw[2 * wi + 1], 0x7632u);
+          }
         }
+      }
     }
 
     // Qhat = scale * R_angle q from one cos/sin row (a3/a4); `scale` is 1 when the K side carries the scale
@@ -562,6 +578,7 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
     a.part_ml = h->ws.part_ml;
     a.req_counter = h->ws.req_counter;
     a.num_reqs = n;
+    a.q_interleaved = c.rope_style == LAZY_ROPE_INTERLEAVED;
     a.sh = h->shape;
     int gx = h->num_sms / HG;
     if (gx < 1) gx = 1;

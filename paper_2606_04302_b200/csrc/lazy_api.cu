@@ -20,7 +20,8 @@ bool config_supported(const lazy_config* c) {
   if (c->num_q_heads / c->num_kv_heads > 8) return false;
   int hkv = c->num_kv_heads;
   if (!(hkv == 1 || hkv == 2 || hkv == 4 || hkv % 8 == 0)) return false;
-  if (c->dtype != 0 || c->rope_style != 0) return false;
+  if (c->dtype != 0) return false;
+  if (c->rope_style != LAZY_ROPE_HALF_SPLIT && c->rope_style != LAZY_ROPE_INTERLEAVED) return false;
   if (c->k_storage < LAZY_K_UNROTATED || c->k_storage > LAZY_K_ABSOLUTE) return false;
   return true;
 }
@@ -101,7 +102,7 @@ int lazy_create(const lazy_config* cfg, void* workspace, size_t workspace_bytes,
     delete h;
     return LAZY_ERR_CUDA;
   }
-  int n = lazy::launch_build_tables(h, s);
+  int n = lazy::launch_build_tables(h, nullptr, s);
   if (n < 0) { delete h; return n; }
   h->launches += n;
   *out = h;
@@ -122,6 +123,18 @@ int lazy_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const
                                    static_cast<cudaStream_t>(stream));
   if (n < 0) return n;
   h->launches += n;
+  return LAZY_OK;
+}
+
+int lazy_set_rope_frequencies(lazy_handle* h, const double* inv_freq, double softmax_scale, void* stream) {
+  if (!h || softmax_scale < 0.0) return LAZY_ERR_INVALID;
+  if (inv_freq)
+    for (int j = 0; j < h->cfg.head_dim / 2; ++j)
+      if (!(inv_freq[j] >= 0.0) || !std::isfinite(inv_freq[j])) return LAZY_ERR_INVALID;
+  int n = lazy::launch_build_tables(h, inv_freq, static_cast<cudaStream_t>(stream));
+  if (n < 0) return n;
+  h->launches += n;
+  if (softmax_scale > 0.0) h->shape.scale_log2 = (float)(1.4426950408889634 * softmax_scale);
   return LAZY_OK;
 }
 

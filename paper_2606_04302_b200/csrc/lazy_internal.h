@@ -61,7 +61,7 @@ bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, in
 bool encode_q_tmap(void* out_map, const void* q, int total_q, int Hq, int Hkv, int D, int tokens_per_tile);
 
 // Each launcher enqueues on `stream` and returns the number of kernels launched (<0: LAZY_ERR_*).
-int launch_build_tables(lazy_handle* h, cudaStream_t stream);
+int launch_build_tables(lazy_handle* h, const double* inv_freq_host, cudaStream_t stream);
 int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
                        int num_tokens, void* k_cache, void* v_cache, cudaStream_t stream);
 int launch_materialize(lazy_handle* h, const void* k_src, const void* v_src, const int32_t* src_pages,

@@ -85,6 +85,7 @@ struct PrefillArgs {
   const float2* cs;
   const int* stored_pos;   // LAZY_K_STORED_POS: [num_pages] position each physical page was stored at
   int num_reqs;
+  int q_interleaved;    // LAZY_ROPE_INTERLEAVED: q arrives with pairs (2j, 2j+1); de-interleaved while it is rotated
   int mblocks;          // CTAs per (request, kv head)
   int tokens_per_tile;  // 128 / group
   Shape sh;
@@ -488,6 +489,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       if (valid) {
         const int pos = ppos[sq / kPageSize] + sq % kPageSize;
         const float2* cs_row = a.cs + (size_t)pos * (D / 2);
+        uint4 src[2 * C::CPR];                      // LAZY_ROPE_INTERLEAVED: the whole row first (in-place hazard)
+        if (a.q_interleaved) {
+#pragma unroll
+          for (int c = 0; c < 2 * C::CPR; ++c) src[c] = ptx::lds128(qb + chunk_off(row, c));
+        }
 #pragma unroll
         for (int c = 0; c < C::CPR; ++c) {
           float co[8], si[8];
@@ -495,7 +501,16 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 #pragma unroll
           for (int e = 0; e < 8; ++e) { co[e] *= sh.scale_log2; si[e] *= sh.scale_log2; }
           const uint32_t pa = qb + chunk_off(row, c), pb = qb + chunk_off(row, c + C::CPR);
-          uint4 va = ptx::lds128(pa), vb = ptx::lds128(pb);
+          uint4 va, vb;
+          if (!a.q_interleaved) {
+            va = ptx::lds128(pa); vb = ptx::lds128(pb);
+          } else {                                  // model words (x1_j, x2_j) -> x1 chunk and x2 chunk of pairs 8c..8c+7
+            const uint4 s0 = src[2 * c], s1 = src[2 * c + 1];
+            va.x = __byte_perm(s0.x, s0.y, 0x5410u); va.y = __byte_perm(s0.z, s0.w, 0x5410u);
+            va.z = __byte_perm(s1.x, s1.y, 0x5410u); va.w = __byte_perm(s1.z, s1.w, 0x5410u);
+            vb.x = __byte_perm(s0.x, s0.y, 0x7632u); vb.y = __byte_perm(s0.z, s0.w, 0x7632u);
+            vb.z = __byte_perm(s1.x, s1.y, 0x7632u); vb.w = __byte_perm(s1.z, s1.w, 0x7632u);
+          }
           rotate8(va, vb, co, si);
           ptx::sts128(pa, va);
           ptx::sts128(pb, vb);
@@ -672,6 +687,7 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   a.cs = h->ws.cs;
   a.stored_pos = h->page_stored_pos;
   a.num_reqs = num_reqs;
+  a.q_interleaved = c.rope_style == LAZY_ROPE_INTERLEAVED;
   a.mblocks = (max_q_len + 2 * tpt - 1) / (2 * tpt);
   a.tokens_per_tile = tpt;
   a.sh = h->shape;

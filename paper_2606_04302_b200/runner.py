@@ -15,7 +15,8 @@ class DeviceBatch:
     def __init__(self, batch: LazyBatch, device: str = "cuda", flags: int = 0, max_position: Optional[int] = None,
                  k_storage: int = B.LAZY_K_UNROTATED, page_stored_pos: Optional[torch.Tensor] = None,
                  k_pool: Optional[torch.Tensor] = None, v_pool: Optional[torch.Tensor] = None,
-                 block_table: Optional[torch.Tensor] = None):
+                 block_table: Optional[torch.Tensor] = None, rope_style: int = B.LAZY_ROPE_HALF_SPLIT,
+                 inv_freq=None, softmax_scale: float = 0.0):
         """k_pool / v_pool / block_table override the batch's own (the stored-position and absolute layouts of
         SURVEY 8.0 row f1 hold differently encoded K, the absolute one also private pages per request)."""
         self.batch = batch
@@ -29,7 +30,9 @@ class DeviceBatch:
         self.handle = B.lazy_create(sh.num_q_heads, sh.num_kv_heads, sh.head_dim, num_pages=int(self.k_pool.shape[0]),
                                     max_position=max_position or batch.max_position, max_reqs=R,
                                     max_pages_per_req=pmax, rope_theta=sh.rope_theta, page_size=sh.page_size,
-                                    flags=flags, k_storage=k_storage, device=self.device)
+                                    flags=flags, k_storage=k_storage, rope_style=rope_style, device=self.device)
+        if inv_freq is not None or softmax_scale:
+            B.lazy_set_rope_frequencies(self.handle, inv_freq, softmax_scale)
         if page_stored_pos is not None:
             B.lazy_set_page_stored_pos(self.handle, page_stored_pos.to(self.device, dtype=torch.int32).contiguous())
 

@@ -32,10 +32,13 @@ def compare(got: torch.Tensor, ref: np.ndarray, what: str = "", rows=None, abs_s
 
 
 def run_and_compare(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, max_position=None,
-                    scale_abs_by_output: bool = False):
+                    scale_abs_by_output: bool = False, dev_kw=None, oracle_kw=None, k_perm=None):
     """Runs every step on the GPU and on the oracle (oracle pools are separate CPU copies).  With
     sample_rows > 0 the oracle computes only that many seeded query rows per attention step."""
-    dev = DeviceBatch(batch, flags=flags, max_position=max_position)
+    """dev_kw / oracle_kw: the same positional variant handed to the CUDA handle and to the oracle; k_perm: order
+    in which the library stores K's last axis (LAZY_ROPE_INTERLEAVED de-interleaves on write; pre-loaded pages must be
+    uploaded in that order, dev_kw["k_pool"])."""
+    dev = DeviceBatch(batch, flags=flags, max_position=max_position, **(dev_kw or {}))
     k_ref, v_ref = batch.k_pool.clone(), batch.v_pool.clone()
     rng = np.random.default_rng(seed)
     all_stats = []
@@ -48,9 +51,10 @@ def run_and_compare(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, 
                 rows = np.sort(rng.choice(step.q.shape[0], size=sample_rows, replace=False))
                 sel = np.zeros(step.q.shape[0], dtype=np.uint8)
                 sel[rows] = 1
-            ref = O.run_step(batch, step, k_ref, v_ref, row_select=sel)
+            ref = O.run_step(batch, step, k_ref, v_ref, row_select=sel, **(oracle_kw or {}))
             # pools must agree bit for bit after the step's cache write, and stay so after the read path
-            assert torch.equal(dev.k_pool.cpu().view(torch.int16), k_ref.view(torch.int16)), f"step {si}: K pool"
+            k_expect = k_ref if k_perm is None else k_ref[..., k_perm]
+            assert torch.equal(dev.k_pool.cpu().view(torch.int16), k_expect.view(torch.int16)), f"step {si}: K pool"
             assert torch.equal(dev.v_pool.cpu().view(torch.int16), v_ref.view(torch.int16)), f"step {si}: V pool"
             if got is not None:
                 sc = max(1.0, float(np.abs(ref).max())) if scale_abs_by_output else 1.0
