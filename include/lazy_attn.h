@@ -71,9 +71,15 @@ typedef struct lazy_config {
  *                         still position-free, and the attention kernels de-interleave q on load: interleaved RoPE
  *                         on x equals half-split RoPE on de-interleaved x, and a dot product does not care about a
  *                         permutation applied to both operands.  k_cache's last axis is therefore in that order
- *                         (V and every output are untouched). */
+ *                         (V and every output are untouched).
+ *   LAZY_POS_ALIBI        no rotation at all: ALiBi.  K and q are used as they are and the score of
+ *                         the query at logical position m with the key at logical position n gets the bias
+ *                         slope[hq] * (n - m) added after scaling (lazy_set_alibi_slopes; slopes start as 0).
+ *                         The positions are the same per-page logical positions RoPE would use, so a cached page
+ *                         is reusable at any offset exactly as with RoPE.  k_storage must be LAZY_K_UNROTATED. */
 #define LAZY_ROPE_HALF_SPLIT  0
 #define LAZY_ROPE_INTERLEAVED 1
+#define LAZY_POS_ALIBI        2
 
 /* k_storage: what a physical page's K rows carry (V is position-free in every mode).
  *   LAZY_K_UNROTATED  the product path (north_star): K is the projection output, the kernels
@@ -149,6 +155,10 @@ int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const v
  * not rotated (partial rotary).  softmax_scale > 0 replaces 1/sqrt(head_dim) (YaRN's attention temperature);
  * 0 keeps the current one. */
 int lazy_set_rope_frequencies(lazy_handle* h, const double* inv_freq, double softmax_scale, void* stream);
+
+/* LAZY_POS_ALIBI only: per-q-head slopes (HOST array of num_q_heads floats, natural-log domain as in the ALiBi
+ * definition: bias = slope * (n - m)).  Copied into the workspace on `stream`. */
+int lazy_set_alibi_slopes(lazy_handle* h, const float* slopes, void* stream);
 
 /* LAZY_K_STORED_POS only: device array [num_pages] int32, position at which token 0 of each physical page
  * was rotated when it was stored.  The pointer is kept (not copied) and read by every later attention call;

@@ -16,10 +16,10 @@ LIB_PATH = os.path.join(_HERE, "csrc", "liblazyattn.so")
 LAZY_OK, LAZY_ERR_INVALID, LAZY_ERR_UNSUPPORTED, LAZY_ERR_WORKSPACE, LAZY_ERR_CUDA = 0, -1, -2, -3, -4
 LAZY_FLAG_ROWWISE_KERNELS = 1
 LAZY_K_UNROTATED, LAZY_K_STORED_POS, LAZY_K_ABSOLUTE = 0, 1, 2
-LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED = 0, 1
+LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
-           "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_page_stored_pos",
+           "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_alibi_slopes", "lazy_set_page_stored_pos",
            "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step"]
 
 
@@ -57,6 +57,8 @@ def lib() -> ctypes.CDLL:
         L.lazy_attn_decode.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, vp, vp]
         L.lazy_set_rope_frequencies.restype = ctypes.c_int
         L.lazy_set_rope_frequencies.argtypes = [vp, vp, ctypes.c_double, vp]
+        L.lazy_set_alibi_slopes.restype = ctypes.c_int
+        L.lazy_set_alibi_slopes.argtypes = [vp, vp, vp]
         L.lazy_set_page_stored_pos.restype = ctypes.c_int
         L.lazy_set_page_stored_pos.argtypes = [vp, vp]
         L.lazy_materialize_pages.restype = ctypes.c_int
@@ -186,6 +188,17 @@ def lazy_set_rope_frequencies(h: LazyHandle, inv_freq=None, softmax_scale: float
     rc = lib().lazy_set_rope_frequencies(h.ptr, arr, float(softmax_scale), _stream(stream))
     if rc != 0:
         raise LazyError("lazy_set_rope_frequencies", rc)
+
+
+def lazy_set_alibi_slopes(h: LazyHandle, slopes, stream=None) -> None:
+    """slopes: sequence of num_q_heads floats (host)."""
+    vals = [float(x) for x in slopes]
+    if len(vals) != h.cfg.num_q_heads:
+        raise LazyError("lazy_set_alibi_slopes", LAZY_ERR_INVALID)
+    arr = (ctypes.c_float * len(vals))(*vals)
+    rc = lib().lazy_set_alibi_slopes(h.ptr, arr, _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_set_alibi_slopes", rc)
 
 
 def lazy_set_page_stored_pos(h: LazyHandle, page_stored_pos) -> None:

@@ -171,7 +171,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
                     const int* __restrict__ page_pos, const int* __restrict__ seq_lens,
                     const int* __restrict__ cu_q_lens, int num_reqs, Shape sh, const float2* __restrict__ cs,
                     int k_storage, const int* __restrict__ stored_pos, int q_interleaved,
-                    __nv_bfloat16* __restrict__ out) {
+                    const float* __restrict__ alibi, __nv_bfloat16* __restrict__ out) {
   constexpr int HALF = D / 2;
   constexpr int PER = D / 64;
   const int row = blockIdx.x;
@@ -208,7 +208,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
       int j = lane * PER + e;
       float a = __bfloat162float(qp[q_interleaved ? 2 * j : j]);
       float b = __bfloat162float(qp[q_interleaved ? 2 * j + 1 : j + HALF]);
-      float2 t = cs_load(cs + (size_t)pos_q * HALF, j, D);
+      float2 t = cs_load(cs + (size_t)(alibi ? 0 : pos_q) * HALF, j, D);   // table row 0 is the identity
       q1[e] = (a * t.x - b * t.y) * sh.scale_log2;
       q2[e] = (a * t.y + b * t.x) * sh.scale_log2;
     }
@@ -222,7 +222,8 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     int page = bt[slot];
     // rotation still owed to this key: its logical position (un-rotated pages), one relative offset per page
     // (stored-position pages), nothing (absolute pages; table row 0 is the identity)
-    int pos = k_storage == LAZY_K_UNROTATED ? pp[slot] + t
+    int pos = alibi ? 0
+              : k_storage == LAZY_K_UNROTATED ? pp[slot] + t
               : k_storage == LAZY_K_STORED_POS ? pp[slot] - stored_pos[page] : 0;
     const float sgn = pos < 0 ? -1.f : 1.f;
     pos = pos < 0 ? -pos : pos;
@@ -240,6 +241,7 @@ rowwise_attn_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) dot += __shfl_xor_sync(0xffffffffu, dot, off);
+    if (alibi) dot += alibi[hq] * (float)(pp[slot] + t - pos_q);          // ALiBi bias (log2 units)
     float m_new = fmaxf(m, dot);
     float corr = exp2f(m - m_new);       // m = -inf on the first key -> 0
     float p = exp2f(dot - m_new);
@@ -279,12 +281,14 @@ int launch_rowwise(lazy_handle* h, const void* q, const void* k_cache, const voi
     rowwise_attn_kernel<128><<<grid, 128, 0, stream>>>(qp, kp, vp, block_table, page_logical_pos, seq_lens,
                                                        cu_q_lens, num_reqs, h->shape, h->ws.cs, h->cfg.k_storage,
                                                        h->page_stored_pos,
-                                                       h->cfg.rope_style == LAZY_ROPE_INTERLEAVED, op);
+                                                       h->cfg.rope_style == LAZY_ROPE_INTERLEAVED,
+                                                       h->cfg.rope_style == LAZY_POS_ALIBI ? h->ws.alibi : nullptr, op);
   else
     rowwise_attn_kernel<64><<<grid, 128, 0, stream>>>(qp, kp, vp, block_table, page_logical_pos, seq_lens,
                                                       cu_q_lens, num_reqs, h->shape, h->ws.cs, h->cfg.k_storage,
                                                       h->page_stored_pos,
-                                                      h->cfg.rope_style == LAZY_ROPE_INTERLEAVED, op);
+                                                      h->cfg.rope_style == LAZY_ROPE_INTERLEAVED,
+                                                      h->cfg.rope_style == LAZY_POS_ALIBI ? h->ws.alibi : nullptr, op);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
 

@@ -66,6 +66,7 @@ struct DecodeArgs {
   __nv_bfloat16* out;
   const float2* cs;
   const int* stored_pos;   // LAZY_K_STORED_POS: [num_pages] position each physical page was stored at
+  const float* alibi;      // kKmAlibi: [Hq] slopes * log2(e)
   float* part_o;
   float2* part_ml;
   int* req_counter;
@@ -78,11 +79,14 @@ struct DecodeArgs {
 // L175-182: "rotate Q" by the page's relative offset): K is consumed as stored, q is re-rotated once per page
 // by m - (p0 - stored[page]).  LAZY_K_ABSOLUTE: K as stored, q rotated once per request by m (no table rows
 // travel with the pages): the "rotation compiled out" arm of the overhead ablation (Fig. 5).
+// kKmAlibi: nothing is rotated; the score of token t of a page starting at p0 gets the bias
+// slope[head] * (p0 + t - m) -- the same per-page relative offset m - p0 the rotation would use.
 template <int D, int HKV_CTA, int KM>
 __global__ void __launch_bounds__(kDecodeThreads, 1)
 decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
                       const DecodeArgs a) {
   using C = DecodeCfg<D, HKV_CTA>;
+  constexpr bool kNoRows = KM == LAZY_K_ABSOLUTE || KM == kKmAlibi;   // no cos/sin row travels with a page
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const uint32_t smem_base = ptx::smem_u32(smem);
@@ -201,7 +205,7 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
       if (pl < C::PPS) reinterpret_cast<int*>(st + C::OFF_META)[pl] = delta;
       __syncwarp();
       if (lane == 0)
-        ptx::mbar_arrive_expect_tx(full, nvalid * (2 * C::PAGE_BYTES + (KM == LAZY_K_ABSOLUTE ? 0 : C::CS_ROW_BYTES)));
+        ptx::mbar_arrive_expect_tx(full, nvalid * (2 * C::PAGE_BYTES + (kNoRows ? 0 : C::CS_ROW_BYTES)));
       __syncwarp();
       if (active) {
         const int row0 = (pg * sh.Hkv + hg * HKV_CTA) * kPageSize;
@@ -210,7 +214,7 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
           ptx::tma_load_2d(st_u32 + pl * C::PAGE_BYTES + h * C::BOX_BYTES, &tmap_k, full, h * 64, row0);
           ptx::tma_load_2d(st_u32 + C::OFF_V + pl * C::PAGE_BYTES + h * C::BOX_BYTES, &tmap_v, full, h * 64, row0);
         }
-        if (KM != LAZY_K_ABSOLUTE) {
+        if (!kNoRows) {
           int ad = delta < 0 ? -delta : delta;
           ptx::bulk_load_1d(st_u32 + C::OFF_CS + pl * C::CS_ROW_BYTES, a.cs + (size_t)ad * (D / 2),
                             C::CS_ROW_BYTES, full);
@@ -282,6 +286,16 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
         qhat[1][w] = ptx::pack_bf16(a_lo * c.z + b_lo * c.x, a_hi * c.w + b_hi * c.y);
       }
     };
+    float slope0 = 0.f, slope1 = 0.f;               // kKmAlibi: slopes (log2 units) of heads 2tq, 2tq+1
+    if (KM == kKmAlibi) {
+#pragma unroll
+      for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int w = 0; w < C::NL; ++w)
+          qhat[h][w] = ptx::pack_bf16(ptx::bf16_lo(qraw[h][w]) * sh.scale_log2, ptx::bf16_hi(qraw[h][w]) * sh.scale_log2);
+      if (2 * tq < group) slope0 = a.alibi[hk * group + 2 * tq];
+      if (2 * tq + 1 < group) slope1 = a.alibi[hk * group + 2 * tq + 1];
+    }
     if (KM == LAZY_K_ABSOLUTE && L > 0) {           // once per request: rotate q by the query token's position
       const int* pp = a.page_pos + (size_t)r * sh.table_stride;
       const int mq = pp[(L - 1) / kPageSize] + (L - 1) % kPageSize;
@@ -321,7 +335,7 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
               kreg[h][rw][4 * x + 2] = v.z; kreg[h][rw][4 * x + 3] = v.w;
             }
         // ---- q re-rotated for this page: Qhat = R_{m - p0} q   (a3/a4; one cos/sin row per page)
-        if (KM != LAZY_K_ABSOLUTE) {
+        if (!kNoRows) {
           const uint32_t qcs = st + C::OFF_CS + pl * C::CS_ROW_BYTES + tq * 16;
           rotate_q([&](int w) { return ptx::lds128f(qcs + w * 64); }, delta < 0 ? -1.f : 1.f,
                    KM == LAZY_K_UNROTATED ? 1.f : sh.scale_log2);
@@ -350,6 +364,11 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
         }
 #pragma unroll
         for (int x = 0; x < 4; ++x) s[x] += s_b[x];
+        if (KM == kKmAlibi) {                        // bias slope * (n - m), n - m = t - delta
+          const float rel0 = (float)(g - delta), rel1 = (float)(g + 8 - delta);
+          s[0] += slope0 * rel0; s[1] += slope1 * rel0;
+          s[2] += slope0 * rel1; s[3] += slope1 * rel1;
+        }
         if (g >= nv) { s[0] = -INFINITY; s[1] = -INFINITY; }
         if (g + 8 >= nv) { s[2] = -INFINITY; s[3] = -INFINITY; }
         // ---- online softmax over the 16 tokens (a6): max across the 8 row-lanes with shuffles
@@ -541,6 +560,7 @@ static int launch_decode_km(lazy_handle* h, const DecodeArgs& args, int grid_x, 
 
 template <int D, int HKV_CTA>
 static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, int grid_y, cudaStream_t stream) {
+  if (h->cfg.rope_style == LAZY_POS_ALIBI) return launch_decode_km<D, HKV_CTA, kKmAlibi>(h, args, grid_x, grid_y, stream);
   switch (h->cfg.k_storage) {
     case LAZY_K_STORED_POS: return launch_decode_km<D, HKV_CTA, LAZY_K_STORED_POS>(h, args, grid_x, grid_y, stream);
     case LAZY_K_ABSOLUTE:   return launch_decode_km<D, HKV_CTA, LAZY_K_ABSOLUTE>(h, args, grid_x, grid_y, stream);
@@ -574,6 +594,7 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
     a.seq_lens = seq_lens + r0;
     a.cs = h->ws.cs;
     a.stored_pos = h->page_stored_pos;
+    a.alibi = h->ws.alibi;
     a.part_o = h->ws.part_o;
     a.part_ml = h->ws.part_ml;
     a.req_counter = h->ws.req_counter;

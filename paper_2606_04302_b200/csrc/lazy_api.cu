@@ -21,7 +21,9 @@ bool config_supported(const lazy_config* c) {
   int hkv = c->num_kv_heads;
   if (!(hkv == 1 || hkv == 2 || hkv == 4 || hkv % 8 == 0)) return false;
   if (c->dtype != 0) return false;
-  if (c->rope_style != LAZY_ROPE_HALF_SPLIT && c->rope_style != LAZY_ROPE_INTERLEAVED) return false;
+  if (c->rope_style < LAZY_ROPE_HALF_SPLIT || c->rope_style > LAZY_POS_ALIBI) return false;
+  if (c->rope_style == LAZY_POS_ALIBI && (c->k_storage != LAZY_K_UNROTATED || c->num_q_heads > lazy::kMaxAlibiHeads))
+    return false;
   if (c->k_storage < LAZY_K_UNROTATED || c->k_storage > LAZY_K_ABSOLUTE) return false;
   return true;
 }
@@ -32,7 +34,7 @@ bool config_valid(const lazy_config* c) {
 }
 
 struct Layout {
-  size_t cs, part_o, part_ml, req_counter, sched, total;
+  size_t cs, part_o, part_ml, req_counter, sched, alibi, total;
 };
 
 Layout workspace_layout(const lazy_config* c) {
@@ -47,6 +49,7 @@ Layout workspace_layout(const lazy_config* c) {
   l.part_ml = off;     off = align_up(off + parts * c->num_q_heads * sizeof(float2), 256);
   l.req_counter = off; off = align_up(off + (size_t)c->max_reqs * head_groups * sizeof(int), 256);
   l.sched = off;       off = align_up(off + 1024 * sizeof(int), 256);
+  l.alibi = off;       off = align_up(off + lazy::kMaxAlibiHeads * sizeof(float), 256);
   l.total = off;
   return l;
 }
@@ -89,6 +92,7 @@ int lazy_create(const lazy_config* cfg, void* workspace, size_t workspace_bytes,
   h->ws.part_ml = reinterpret_cast<float2*>(base + l.part_ml);
   h->ws.req_counter = reinterpret_cast<int*>(base + l.req_counter);
   h->ws.sched = reinterpret_cast<int*>(base + l.sched);
+  h->ws.alibi = reinterpret_cast<float*>(base + l.alibi);
 
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess ||
@@ -98,7 +102,8 @@ int lazy_create(const lazy_config* cfg, void* workspace, size_t workspace_bytes,
   }
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (cudaMemsetAsync(h->ws.req_counter, 0, l.sched - l.req_counter, s) != cudaSuccess ||
-      cudaMemsetAsync(h->ws.sched, 0, 1024 * sizeof(int), s) != cudaSuccess) {
+      cudaMemsetAsync(h->ws.sched, 0, 1024 * sizeof(int), s) != cudaSuccess ||
+      cudaMemsetAsync(h->ws.alibi, 0, lazy::kMaxAlibiHeads * sizeof(float), s) != cudaSuccess) {
     delete h;
     return LAZY_ERR_CUDA;
   }
@@ -135,6 +140,20 @@ int lazy_set_rope_frequencies(lazy_handle* h, const double* inv_freq, double sof
   if (n < 0) return n;
   h->launches += n;
   if (softmax_scale > 0.0) h->shape.scale_log2 = (float)(1.4426950408889634 * softmax_scale);
+  return LAZY_OK;
+}
+
+int lazy_set_alibi_slopes(lazy_handle* h, const float* slopes, void* stream) {
+  if (!h || !slopes) return LAZY_ERR_INVALID;
+  if (h->cfg.rope_style != LAZY_POS_ALIBI) return LAZY_ERR_UNSUPPORTED;
+  for (int i = 0; i < h->cfg.num_q_heads; ++i) {
+    if (!std::isfinite(slopes[i])) return LAZY_ERR_INVALID;
+    h->alibi_host[i] = slopes[i] * 1.4426950408889634f;       // the kernels work in log2 units
+  }
+  // pageable source: the runtime stages it before returning, so later changes of alibi_host are harmless
+  if (cudaMemcpyAsync(h->ws.alibi, h->alibi_host, h->cfg.num_q_heads * sizeof(float), cudaMemcpyHostToDevice,
+                      static_cast<cudaStream_t>(stream)) != cudaSuccess)
+    return LAZY_ERR_CUDA;
   return LAZY_OK;
 }
 

@@ -11,6 +11,8 @@ namespace lazy {
 
 constexpr int kPageSize = 16;
 constexpr int kMaxDecodeCtas = 1024;   // upper bound on the decode grid (sizes the partial buffers)
+constexpr int kKmAlibi = 3;            // kernel template value next to LAZY_K_*: no rotation, ALiBi score bias
+constexpr int kMaxAlibiHeads = 256;
 
 // Device-side views the kernels take by value.
 struct Shape {
@@ -26,6 +28,7 @@ struct Workspace {
   float2* part_ml;       // [max_reqs + kMaxDecodeCtas][Hq] (running max in log2 units, sum)
   int*    req_counter;   // [max_reqs] arrival counters for the in-kernel combine (self-resetting)
   int*    sched;         // small scratch for device-side scheduling
+  float*  alibi;         // [kMaxAlibiHeads] slopes * log2(e) (LAZY_POS_ALIBI)
 };
 
 }  // namespace lazy
@@ -37,6 +40,7 @@ struct lazy_handle {
   int num_sms;
   int64_t launches;
   const int32_t* page_stored_pos;   // LAZY_K_STORED_POS: device [num_pages], caller-owned
+  float alibi_host[lazy::kMaxAlibiHeads];   // staging copy of the slopes (source of the async H2D copy)
   // cached TMA descriptors (128 bytes each), keyed by the pool pointer they were encoded for
   alignas(64) unsigned char tmap_k[128];
   alignas(64) unsigned char tmap_v[128];

@@ -54,8 +54,9 @@ struct PrefillCfg {
   static constexpr int OFF_BAR = OFF_CS + 2 * CS_STAGE_BYTES;
   static constexpr int NUM_BARS = 24;
   static constexpr int OFF_TMEM = OFF_BAR + NUM_BARS * 8;
-  static constexpr int OFF_SIGN = OFF_TMEM + 16;    // 2 stages x 8 pages: sign of the page's relative offset
-  static constexpr int SMEM_BYTES = OFF_SIGN + 2 * kPagesPerTile * 4 + 1024;   // + alignment slack
+  static constexpr int OFF_SIGN = OFF_TMEM + 16;    // ring of 4 tiles x 8 pages: sign of the page's relative offset
+                                                    // (LAZY_K_STORED_POS) or its logical start (ALiBi)
+  static constexpr int SMEM_BYTES = OFF_SIGN + 4 * kPagesPerTile * 4 + 1024;   // + alignment slack
 };
 
 // register budgets per warpgroup (setmaxnreg; 2*128*184 + 128*104 + 128*40 = 65536)
@@ -84,6 +85,7 @@ struct PrefillArgs {
   __nv_bfloat16* out;
   const float2* cs;
   const int* stored_pos;   // LAZY_K_STORED_POS: [num_pages] position each physical page was stored at
+  const float* alibi;      // kKmAlibi: [Hq] slopes * log2(e)
   int num_reqs;
   int q_interleaved;    // LAZY_ROPE_INTERLEAVED: q arrives with pairs (2j, 2j+1); de-interleaved while it is rotated
   int mblocks;          // CTAs per (request, kv head)
@@ -184,7 +186,9 @@ __device__ __forceinline__ void rotate8(uint4& a, uint4& b, const float (&co)[8]
 // KM = lazy_config.k_storage.  LAZY_K_UNROTATED: K tile rotated by the absolute angle of its tokens.
 // LAZY_K_STORED_POS (Eq. 5): K tile rotated once by the page's relative offset
 // D = p0 - stored[page] (one table row per page, no in-page composition).  LAZY_K_ABSOLUTE: the K tile goes to
-// the MMA as it landed (the "rotation compiled out" arm of the overhead ablation, Fig. 5).
+// the MMA as it landed (the "rotation compiled out" arm of the overhead ablation, Fig. 5).  kKmAlibi
+// (PAPER.md L221): nothing is rotated; the softmax warpgroups add slope[head] * (n - m) to S, with the key position
+// n = page start + t taken from a small per-tile ring the producer fills.
 // Same rotation on packed f32x2 lanes (FMUL2 / FFMA2: half the FMA-pipe issue slots).  zc[w], zs[w] hold the
 // (cos, sin) of the two pairs whose x1 / x2 elements are the bf16 halves of word w of a / b.
 __device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
@@ -207,6 +211,7 @@ __global__ void __launch_bounds__(kPrefillThreads, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
                     const __grid_constant__ CUtensorMap tmap_v, const PrefillArgs a) {
   using C = PrefillCfg<D>;
+  constexpr bool kNoRotate = KM == LAZY_K_ABSOLUTE || KM == kKmAlibi;   // the K tile goes to the MMA as it landed
   extern __shared__ unsigned char smem_raw[];
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const uint32_t smem_base = ptx::smem_u32(smem);
@@ -307,15 +312,16 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         const int row0 = (page * sh.Hkv + hk) * kPageSize;
         const uint32_t dst = s * C::TILE_BYTES + half * kHalfBytes + pg * (kPageSize * 128);
         ptx::mbar_wait_sleep(bar(B_KEMPTY + s), ph ^ 1);
-        if (KM == LAZY_K_STORED_POS && lane < kPagesPerTile) s_sign[s * kPagesPerTile + pg] = p0_sign;
+        if (KM == LAZY_K_STORED_POS && lane < kPagesPerTile) s_sign[(j & 3) * kPagesPerTile + pg] = p0_sign;
+        if (KM == kKmAlibi && lane < kPagesPerTile) s_sign[(j & 3) * kPagesPerTile + pg] = p0;
         __syncwarp();
         if (lane == 0)
           ptx::mbar_arrive_expect_tx(bar(B_KFULL + s), npv * (C::NH * kPageSize * 128 +
-                                                              (KM == LAZY_K_ABSOLUTE ? 0 : C::CS_ROW_BYTES)));
+                                                              (kNoRotate ? 0 : C::CS_ROW_BYTES)));
         __syncwarp();
         if (kvsel == 0 && lane_on && pg < npv) {
           ptx::tma_load_2d(sK + dst, &tmap_k, bar(B_KFULL + s), half * 64, row0);
-          if (half == 0 && KM != LAZY_K_ABSOLUTE)
+          if (half == 0 && !kNoRotate)
             ptx::bulk_load_1d(sCS + s * C::CS_STAGE_BYTES + pg * C::CS_ROW_BYTES, a.cs + (size_t)p0 * (D / 2),
                               C::CS_ROW_BYTES, bar(B_KFULL + s));
         }
@@ -435,7 +441,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 #pragma unroll
       for (int ps = 0; ps < PASSES; ++ps) {
         const int i = ps * PPP + pp_;
-        if (KM != LAZY_K_ABSOLUTE && i < npv) {
+        if (!kNoRotate && i < npv) {
           float2 zc[4], zs[4];                      // e^{i (p0+t) theta_j}, or e^{i Delta theta_j} of the page
           const int row = i * kPageSize + t;
           const uint32_t pa = kb + chunk_off(row, c), pb = kb + chunk_off(row, c + C::CPR);
@@ -454,7 +460,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
               zs[x] = __ffma2_rn(wc, us[x], __fmul2_rn(ws, uc[x]));
             }
           } else {                                  // one relative rotation for the whole page (may be negative)
-            const float sgn = (float)s_sign[s * kPagesPerTile + i];
+            const float sgn = (float)s_sign[(j & 3) * kPagesPerTile + i];
 #pragma unroll
             for (int x = 0; x < 4; ++x) zs[x] = __fmul2_rn(zs[x], make_float2(sgn, sgn));
           }
@@ -497,9 +503,14 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 #pragma unroll
         for (int c = 0; c < C::CPR; ++c) {
           float co[8], si[8];
-          load_cs8<D>(cs_row, c, co, si);
+          if (KM == kKmAlibi) {                     // no rotation: scale only
 #pragma unroll
-          for (int e = 0; e < 8; ++e) { co[e] *= sh.scale_log2; si[e] *= sh.scale_log2; }
+            for (int e = 0; e < 8; ++e) { co[e] = sh.scale_log2; si[e] = 0.f; }
+          } else {
+            load_cs8<D>(cs_row, c, co, si);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) { co[e] *= sh.scale_log2; si[e] *= sh.scale_log2; }
+          }
           const uint32_t pa = qb + chunk_off(row, c), pb = qb + chunk_off(row, c + C::CPR);
           uint4 va, vb;
           if (!a.q_interleaved) {
@@ -524,6 +535,12 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     __syncwarp();
     if (lane == 0) ptx::mbar_arrive(bar(B_QREADY + t));
 
+    float alibi_slope = 0.f;                                   // kKmAlibi: this row's slope (log2 units), position
+    int alibi_pos_q = 0;
+    if (KM == kKmAlibi && valid) {
+      alibi_slope = a.alibi[hk * group + g];
+      alibi_pos_q = ppos[sq / kPageSize] + sq % kPageSize;
+    }
     float m_used = -INFINITY, l_run = 0.f;
     if (LAZY_PINGPONG && t == 1) ptx::named_bar_arrive(2, 256);          // tile 0 goes first
     for (int j = 0; j < n_kv; ++j) {
@@ -535,6 +552,21 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 #pragma unroll
       for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
       ptx::tmem_wait_ld();
+      if (KM == kKmAlibi) {                                   // S += slope * (n - m), n = page start + t
+        const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 3) * kPagesPerTile;
+#pragma unroll
+        for (int pg = 0; pg < kPagesPerTile; ++pg) {
+          const float base = alibi_slope * (float)(pstart[pg] - alibi_pos_q);
+#pragma unroll
+          for (int x = 0; x < kPageSize; x += 2) {
+            const float2 b = __ffma2_rn(make_float2(alibi_slope, alibi_slope), make_float2((float)x, (float)(x + 1)),
+                                        make_float2(base, base));
+            const float2 v = __fadd2_rn(make_float2(f32(sreg[16 * pg + x]), f32(sreg[16 * pg + x + 1])), b);
+            sreg[16 * pg + x] = __float_as_uint(v.x);
+            sreg[16 * pg + x + 1] = __float_as_uint(v.y);
+          }
+        }
+      }
       if (j * kTileRows + kTileRows - 1 > lim_min) {          // tile touches the causal edge / the tail: rare
         const int lim_col = lim_row - j * kTileRows;          // column visible iff col <= lim_col
 #pragma unroll
@@ -686,6 +718,7 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   a.out = static_cast<__nv_bfloat16*>(out);
   a.cs = h->ws.cs;
   a.stored_pos = h->page_stored_pos;
+  a.alibi = h->ws.alibi;
   a.num_reqs = num_reqs;
   a.q_interleaved = c.rope_style == LAZY_ROPE_INTERLEAVED;
   a.mblocks = (max_q_len + 2 * tpt - 1) / (2 * tpt);
@@ -694,6 +727,9 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   const long long grid = (long long)a.mblocks * c.num_kv_heads * num_reqs;
   if (grid <= 0 || grid > INT_MAX) return LAZY_ERR_INVALID;
   const int g = (int)grid;
+  if (c.rope_style == LAZY_POS_ALIBI)
+    return c.head_dim == 128 ? launch_prefill_t<128, kKmAlibi>(h, a, g, stream)
+                             : launch_prefill_t<64, kKmAlibi>(h, a, g, stream);
   if (c.head_dim == 128) {
     if (c.k_storage == LAZY_K_STORED_POS) return launch_prefill_t<128, LAZY_K_STORED_POS>(h, a, g, stream);
     if (c.k_storage == LAZY_K_ABSOLUTE) return launch_prefill_t<128, LAZY_K_ABSOLUTE>(h, a, g, stream);

@@ -16,7 +16,7 @@ class DeviceBatch:
                  k_storage: int = B.LAZY_K_UNROTATED, page_stored_pos: Optional[torch.Tensor] = None,
                  k_pool: Optional[torch.Tensor] = None, v_pool: Optional[torch.Tensor] = None,
                  block_table: Optional[torch.Tensor] = None, rope_style: int = B.LAZY_ROPE_HALF_SPLIT,
-                 inv_freq=None, softmax_scale: float = 0.0):
+                 inv_freq=None, softmax_scale: float = 0.0, alibi_slopes=None):
         """k_pool / v_pool / block_table override the batch's own (the stored-position and absolute layouts of
         SURVEY 8.0 row f1 hold differently encoded K, the absolute one also private pages per request)."""
         self.batch = batch
@@ -31,6 +31,8 @@ class DeviceBatch:
                                     max_position=max_position or batch.max_position, max_reqs=R,
                                     max_pages_per_req=pmax, rope_theta=sh.rope_theta, page_size=sh.page_size,
                                     flags=flags, k_storage=k_storage, rope_style=rope_style, device=self.device)
+        if alibi_slopes is not None:
+            B.lazy_set_alibi_slopes(self.handle, alibi_slopes)
         if inv_freq is not None or softmax_scale:
             B.lazy_set_rope_frequencies(self.handle, inv_freq, softmax_scale)
         if page_stored_pos is not None:

@@ -86,3 +86,48 @@ def test_partial_rotary_and_restore_default(cfg, scale):
             B.lazy_set_rope_frequencies(dev.handle, [-1.0] * (sh.head_dim // 2))
     finally:
         dev.close(); ref.close()
+
+
+def _alibi_slopes(n_heads):
+    return np.array([2.0 ** (-8.0 * (h + 1) / n_heads) for h in range(n_heads)])
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+@pytest.mark.parametrize("cfg,scale", [(1, None), (2, 0.1), (3, 0.05), (4, 0.1), (5, 0.15)])
+def test_alibi_bias(cfg, scale, flags):
+    """ALiBi with deferred positions -- the bias uses the per-page logical positions, nothing is
+    rotated, cached pages stay reusable at any offset (the configs share pages across requests and positions)."""
+    batch = _batch(cfg, scale)
+    slopes = _alibi_slopes(batch.shape.num_q_heads)
+    run_and_compare(batch, flags=flags, dev_kw=dict(rope_style=B.LAZY_POS_ALIBI, alibi_slopes=slopes),
+                    oracle_kw=dict(alibi_slopes=slopes))
+
+
+def test_alibi_strong_slopes_and_shift_invariance():
+    """Large slopes make the bias decide the softmax (a wrong sign or a wrong page position cannot hide);
+    shifting every logical position leaves the outputs unchanged."""
+    slopes = None
+    outs = []
+    for shift in (0, 4096):
+        batch = W.config2(scale=0.1, pos_shift=shift)
+        slopes = np.linspace(0.5, 0.01, batch.shape.num_q_heads)
+        if shift == 0:
+            run_and_compare(batch, dev_kw=dict(rope_style=B.LAZY_POS_ALIBI, alibi_slopes=slopes),
+                            oracle_kw=dict(alibi_slopes=slopes), scale_abs_by_output=True)
+        from paper_2606_04302_b200.runner import DeviceBatch
+        dev = DeviceBatch(batch, rope_style=B.LAZY_POS_ALIBI, alibi_slopes=slopes)
+        outs.append([o.float().cpu() for o in dev.run_all() if o is not None])
+        dev.close()
+    for a, b in zip(*outs):
+        assert (a - b).abs().max().item() < 2e-3
+
+
+def test_alibi_rejects_rotated_storage_and_wrong_style():
+    cfg = B.LazyConfig(32, 8, 128, 16, 64, 4096, 4, 16, 5e5, B.LAZY_POS_ALIBI, 0, 0, B.LAZY_K_ABSOLUTE)
+    assert B.lazy_workspace_bytes(cfg) == 0
+    h = B.lazy_create(4, 1, 64, num_pages=8, max_position=256, max_reqs=1, max_pages_per_req=4, rope_theta=1e4)
+    try:
+        with pytest.raises(B.LazyError):
+            B.lazy_set_alibi_slopes(h, [0.1, 0.2, 0.3, 0.4])
+    finally:
+        h.close()
