@@ -331,6 +331,29 @@ def run_ablation(job, steps, warmup):
         torch.cuda.synchronize()
         res[name + "_ms"] = float(np.mean([a.elapsed_time(b) for a, b in evs]))
         dv.close()
+    # f3: ALiBi on the batch's own (shared) pool -- same pages, same traffic as the headline RoPE run
+    if sh.num_q_heads <= 256:
+        slopes = [2.0 ** (-8.0 * (i + 1) / sh.num_q_heads) for i in range(sh.num_q_heads)]
+        dv = DeviceBatch(batch, device=str(d), rope_style=B.LAZY_POS_ALIBI, alibi_slopes=slopes, k_pool=dev.k_pool,
+                         v_pool=dev.v_pool)
+
+        def attend_alibi():
+            if st.kind == "decode":
+                B.lazy_attn_decode(dv.handle, rec["q"], dv.k_pool, dv.v_pool, rec["bt"], rec["pp"], rec["sl"], rec["out"])
+            else:
+                B.lazy_attn_prefill(dv.handle, rec["q"], dv.k_pool, dv.v_pool, rec["bt"], rec["pp"], rec["sl"],
+                                    rec["cu"], rec["max_q"], rec["out"])
+        for _ in range(warmup):
+            job.flush_l2(); attend_alibi()
+        evs = []
+        for _ in range(steps):
+            job.flush_l2()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); attend_alibi(); e1.record()
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+        res["alibi_shared_ms"] = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        dv.close()
     page_bytes = sh.num_kv_heads * P * sh.head_dim * 2
     res["rotation_overhead_pct"] = (res["unrotated_ms"] / res["absolute_ms"] - 1.0) * 100.0
     res["stored_pos_overhead_pct"] = (res["stored_pos_ms"] / res["absolute_ms"] - 1.0) * 100.0
