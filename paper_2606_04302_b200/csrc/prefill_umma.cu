@@ -75,6 +75,7 @@ enum : int {
   B_SFULL = 16,   // +t   MMA commit -> softmax WG t
   B_PREADY = 18,  // +t   softmax WG t (4 warps) -> MMA
   B_OFULL = 20,   // +t   MMA commit -> softmax WG t (epilogue)
+  B_PHALF = 22,   // +t   softmax WG t (4 warps) -> MMA: first half of P (keys 0..63) is in TMEM
 };
 
 struct PrefillArgs {
@@ -256,6 +257,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       ptx::mbar_init(bar(B_KEMPTY + x), 1); ptx::mbar_init(bar(B_VFULL + x), 1);
       ptx::mbar_init(bar(B_VEMPTY + x), 1); ptx::mbar_init(bar(B_SFULL + x), 1);
       ptx::mbar_init(bar(B_PREADY + x), 4); ptx::mbar_init(bar(B_OFULL + x), 1);
+      ptx::mbar_init(bar(B_PHALF + x), 4);
     }
     ptx::mbar_init(bar(B_VFIXED), 1);
     ptx::fence_mbar_init();
@@ -352,11 +354,11 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
           }
         }
       };
-      auto pv = [&](int t, int s, uint32_t acc) {
+      auto pv = [&](int t, int s, uint32_t acc, int k0, int k1) {
         if (leader) {
           const uint32_t va = sV + s * C::TILE_BYTES;
 #pragma unroll
-          for (int k = 0; k < kTileRows / 16; ++k)
+          for (int k = k0; k < k1; ++k)
             ptx::umma_ts(tb + 256 + t * 128, tb + t * 128 + k * 8,
                          ptx::umma_desc_sw128(va + k * 2048, kHalfBytes, 1024), IDESC_PV, acc | (uint32_t)(k > 0));
         }
@@ -376,10 +378,14 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         if (j == nkv - 1) ptx::mbar_wait(bar(B_VFIXED), 0);
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
+          // PV starts on the first 64 keys while the softmax warpgroup is still exponentiating the other 64
+          ptx::mbar_wait(bar(B_PHALF + t), j & 1);
+          ptx::tc_fence_after();
+          pv(t, s, j > 0, 0, kTileRows / 32);
           ptx::mbar_wait(bar(B_PREADY + t), j & 1);
           ptx::tc_fence_after();
           if (leader) LAZY_TR(8 + 3 * t);
-          pv(t, s, j > 0);
+          pv(t, s, 1u, kTileRows / 32, kTileRows / 16);
           if (t == 1) commit(B_VEMPTY + s);
           if (j + 1 < nkv) {
             if (t == 0) {
@@ -549,37 +555,53 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       if (LAZY_PINGPONG == 1) ptx::named_bar_sync(2 + t, 256);             // my turn
       ptx::tc_fence_after();
       if (row == 0) LAZY_TR(3 * t);
+      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+      auto max_chunk = [&](int c) {                           // running row max over columns 32c .. 32c+31
 #pragma unroll
-      for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
-      ptx::tmem_wait_ld();
-      if (KM == kKmAlibi) {                                   // S += slope * (n - m), n = page start + t
-        const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 3) * kPagesPerTile;
+        for (int x = 32 * c; x < 32 * c + 32; x += 8) {
+          mx0 = fmaxf(fmaxf(mx0, f32(sreg[x + 0])), f32(sreg[x + 1]));
+          mx1 = fmaxf(fmaxf(mx1, f32(sreg[x + 2])), f32(sreg[x + 3]));
+          mx2 = fmaxf(fmaxf(mx2, f32(sreg[x + 4])), f32(sreg[x + 5]));
+          mx3 = fmaxf(fmaxf(mx3, f32(sreg[x + 6])), f32(sreg[x + 7]));
+        }
+      };
+      const bool edge = j * kTileRows + kTileRows - 1 > lim_min;   // tile touches the causal edge / the tail: rare
+      if (KM != kKmAlibi && !edge) {
+        // interior tile: the TMEM load of chunk c+1 is in flight while the max of chunk c is taken
+        ptx::tmem_ld32(tS, sreg);
 #pragma unroll
-        for (int pg = 0; pg < kPagesPerTile; ++pg) {
-          const float base = alibi_slope * (float)(pstart[pg] - alibi_pos_q);
+        for (int c = 0; c < 4; ++c) {
+          ptx::tmem_wait_ld();
+          if (c + 1 < 4) ptx::tmem_ld32(tS + (c + 1) * 32, sreg + (c + 1) * 32);
+          max_chunk(c);
+        }
+      } else {
 #pragma unroll
-          for (int x = 0; x < kPageSize; x += 2) {
-            const float2 b = __ffma2_rn(make_float2(alibi_slope, alibi_slope), make_float2((float)x, (float)(x + 1)),
-                                        make_float2(base, base));
-            const float2 v = __fadd2_rn(make_float2(f32(sreg[16 * pg + x]), f32(sreg[16 * pg + x + 1])), b);
-            sreg[16 * pg + x] = __float_as_uint(v.x);
-            sreg[16 * pg + x + 1] = __float_as_uint(v.y);
+        for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
+        ptx::tmem_wait_ld();
+        if (KM == kKmAlibi) {                                 // S += slope * (n - m), n = page start + t
+          const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 3) * kPagesPerTile;
+#pragma unroll
+          for (int pg = 0; pg < kPagesPerTile; ++pg) {
+            const float base = alibi_slope * (float)(pstart[pg] - alibi_pos_q);
+#pragma unroll
+            for (int x = 0; x < kPageSize; x += 2) {
+              const float2 b = __ffma2_rn(make_float2(alibi_slope, alibi_slope),
+                                          make_float2((float)x, (float)(x + 1)), make_float2(base, base));
+              const float2 v = __fadd2_rn(make_float2(f32(sreg[16 * pg + x]), f32(sreg[16 * pg + x + 1])), b);
+              sreg[16 * pg + x] = __float_as_uint(v.x);
+              sreg[16 * pg + x + 1] = __float_as_uint(v.y);
+            }
           }
         }
-      }
-      if (j * kTileRows + kTileRows - 1 > lim_min) {          // tile touches the causal edge / the tail: rare
-        const int lim_col = lim_row - j * kTileRows;          // column visible iff col <= lim_col
+        if (edge) {
+          const int lim_col = lim_row - j * kTileRows;        // column visible iff col <= lim_col
 #pragma unroll
-        for (int x = 0; x < 128; ++x)
-          if (x > lim_col) sreg[x] = 0xff800000u;             // -inf replaces the value (NaN-safe)
-      }
-      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+          for (int x = 0; x < 128; ++x)
+            if (x > lim_col) sreg[x] = 0xff800000u;           // -inf replaces the value (NaN-safe)
+        }
 #pragma unroll
-      for (int x = 0; x < 128; x += 8) {
-        mx0 = fmaxf(fmaxf(mx0, f32(sreg[x + 0])), f32(sreg[x + 1]));
-        mx1 = fmaxf(fmaxf(mx1, f32(sreg[x + 2])), f32(sreg[x + 3]));
-        mx2 = fmaxf(fmaxf(mx2, f32(sreg[x + 4])), f32(sreg[x + 5]));
-        mx3 = fmaxf(fmaxf(mx3, f32(sreg[x + 6])), f32(sreg[x + 7]));
+        for (int c = 0; c < 4; ++c) max_chunk(c);
       }
       const float m_new = fmaxf(m_used, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
       if (j == 0) {
@@ -607,29 +629,32 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       const float2 negm = make_float2(-m_used, -m_used);
       float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
 #pragma unroll
-      for (int x = 0; x < 64; x += 2) {
-        const float2 v0 = __fadd2_rn(make_float2(f32(sreg[2 * x]), f32(sreg[2 * x + 1])), negm);
-        const float2 v1 = __fadd2_rn(make_float2(f32(sreg[2 * x + 2]), f32(sreg[2 * x + 3])), negm);
-        float2 p0, p1;
-        if (LAZY_POLY_EVERY > 0 && (x / 2) % (LAZY_POLY_EVERY > 0 ? LAZY_POLY_EVERY : 1) == LAZY_POLY_EVERY - 1) {
-          p0 = ex2_poly2(v0);
-          p1 = ex2_poly2(v1);
-        } else {
-          p0 = make_float2(ex2(v0.x), ex2(v0.y));
-          p1 = make_float2(ex2(v1.x), ex2(v1.y));
+      for (int hf = 0; hf < 2; ++hf) {
+#pragma unroll
+        for (int x = 32 * hf; x < 32 * hf + 32; x += 2) {
+          const float2 v0 = __fadd2_rn(make_float2(f32(sreg[2 * x]), f32(sreg[2 * x + 1])), negm);
+          const float2 v1 = __fadd2_rn(make_float2(f32(sreg[2 * x + 2]), f32(sreg[2 * x + 3])), negm);
+          float2 p0, p1;
+          if (LAZY_POLY_EVERY > 0 && (x / 2) % (LAZY_POLY_EVERY > 0 ? LAZY_POLY_EVERY : 1) == LAZY_POLY_EVERY - 1) {
+            p0 = ex2_poly2(v0);
+            p1 = ex2_poly2(v1);
+          } else {
+            p0 = make_float2(ex2(v0.x), ex2(v0.y));
+            p1 = make_float2(ex2(v1.x), ex2(v1.y));
+          }
+          sum0 = __fadd2_rn(sum0, p0);
+          sum1 = __fadd2_rn(sum1, p1);
+          sreg[x] = ptx::pack_bf16(p0.x, p0.y);
+          sreg[x + 1] = ptx::pack_bf16(p1.x, p1.y);
         }
-        sum0 = __fadd2_rn(sum0, p0);
-        sum1 = __fadd2_rn(sum1, p1);
-        sreg[x] = ptx::pack_bf16(p0.x, p0.y);
-        sreg[x + 1] = ptx::pack_bf16(p1.x, p1.y);
+        if (hf == 1 && LAZY_PINGPONG) ptx::named_bar_arrive(2 + (t ^ 1), 256);   // the other tile's turn
+        ptx::tmem_st32(tS + 32 * hf, sreg + 32 * hf);         // P (bf16 pairs) over the first 64 columns of S
+        ptx::tmem_wait_st();
+        ptx::tc_fence_before();
+        __syncwarp();
+        if (hf == 0 && lane == 0) ptx::mbar_arrive(bar(B_PHALF + t));
       }
       l_run += (sum0.x + sum0.y) + (sum1.x + sum1.y);
-      if (LAZY_PINGPONG) ptx::named_bar_arrive(2 + (t ^ 1), 256);          // the other tile's turn
-      ptx::tmem_st32(tS, sreg);                               // P (bf16 pairs) over the first 64 columns of S
-      ptx::tmem_st32(tS + 32, sreg + 32);
-      ptx::tmem_wait_st();
-      ptx::tc_fence_before();
-      __syncwarp();
       if (row == 0) LAZY_TR(3 * t + 2);
       if (lane == 0) ptx::mbar_arrive(bar(B_PREADY + t));
     }
