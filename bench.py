@@ -440,6 +440,8 @@ def main():
     ap.add_argument("--noshare", action="store_true", help="every drawn document distinct (logical == unique bytes)")
     ap.add_argument("--no-secondary", action="store_true", help="skip the prefill (cfg3) and noshare side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--graph", action="store_true",
+                    help="also replay the step from a CUDA graph (f4) and report its time next to the eager one")
     ap.add_argument("--ablation", action="store_true",
                     help="also time the stored-position / absolute K layouts and the materialising re-encoding (f1/f2)")
     args = ap.parse_args()
@@ -567,6 +569,27 @@ def main():
                 "d2h_bytes_per_step": int(sum(e["d2h"] for e in job.e2e))},
         "gpu_launches": int(launches), "clocks": clocks,
     }
+    if args.graph and rank == 0 and world == 1:
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            job.run()
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g):
+            job.run()
+        evs = []
+        for i in range(args.warmup + args.steps):
+            job.flush_l2()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); g.replay(); e1.record()
+            if i >= args.warmup:
+                evs.append((e0, e1))
+        torch.cuda.synchronize()
+        g_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        out["graph"] = {"ms_per_step": g_ms, "eager_ms_per_step": ms_step,
+                        "launches_per_step": int(launches) // max(1, args.steps)}
     if args.ablation and rank == 0 and world == 1 and args.workload != "cfg5":
         abl = run_ablation(job, max(5, args.steps), 3)
         abl["lazy_shared_ms"] = ms_attn
