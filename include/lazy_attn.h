@@ -221,6 +221,30 @@ size_t lazy_host_step_staging_bytes(const lazy_handle* h, int32_t num_reqs, int3
                                     int32_t num_new_tokens);
 int lazy_host_step(lazy_handle* h, const lazy_host_step_args* a, void* stream);
 
+/* ---- f4 (host side): document-granular page pool with reference counts and LRU eviction ----------------------
+ * Pure host code, no CUDA call: it hands out PHYSICAL PAGE IDS of the caller's k_cache / v_cache.  One physical copy
+ * per document, reusable at any logical position with LAZY_POOL_AGNOSTIC; with
+ * LAZY_POOL_POSITION_AWARE the key is (document, logical position), i.e. the position-coupled behaviour the paper
+ * compares against (L56-58).  Not thread-safe. */
+typedef struct lazy_pool lazy_pool;
+#define LAZY_POOL_AGNOSTIC        0
+#define LAZY_POOL_POSITION_AWARE  1
+lazy_pool* lazy_pool_create(int32_t num_pages, int32_t page_size, int32_t keying);   /* NULL on bad arguments */
+void lazy_pool_destroy(lazy_pool* p);
+/* Looks a document up for a request that places it at logical_pos and pins it (refcount + 1).
+ * Returns 1 = hit (pages_out filled, KV is valid), 0 = miss (pages_out filled with freshly allocated pages: the
+ * caller prefills the document block-locally and lazy_cache_write's it), LAZY_ERR_WORKSPACE = does not fit even after
+ * evicting every unpinned document, LAZY_ERR_INVALID = bad arguments or a length different from the cached one.
+ * pages_out has room for ceil(doc_tokens / page_size) entries (HOST). Eviction is LRU over unpinned documents. */
+int lazy_pool_acquire(lazy_pool* p, int64_t doc_id, int32_t doc_tokens, int32_t logical_pos, int32_t* pages_out);
+/* Unpins (refcount - 1); at 0 the document becomes evictable (most recently used). */
+int lazy_pool_release(lazy_pool* p, int64_t doc_id, int32_t logical_pos);
+void lazy_pool_stats(const lazy_pool* p, int64_t* lookups, int64_t* hits, int64_t* evictions, int32_t* pages_in_use);
+/* PAPER.md Eq. 1 / Eq. 2 (L60-70): hit ratio of a cache of `capacity_entries` entries over `num_docs` documents with
+ * Zipf(alpha) popularity when every document needs `positions` position-specific copies (1 = position-agnostic).
+ * Eq. 3 is the ratio of two calls.  Returns -1 on bad arguments. */
+double lazy_hit_ratio_model(double alpha, int64_t num_docs, int64_t capacity_entries, int32_t positions);
+
 #ifdef __cplusplus
 }
 #endif

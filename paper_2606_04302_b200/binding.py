@@ -20,7 +20,10 @@ LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
            "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_alibi_slopes", "lazy_set_page_stored_pos",
-           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step"]
+           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step",
+           "lazy_pool_create", "lazy_pool_destroy", "lazy_pool_acquire", "lazy_pool_release", "lazy_pool_stats",
+           "lazy_hit_ratio_model"]
+LAZY_POOL_AGNOSTIC, LAZY_POOL_POSITION_AWARE = 0, 1
 
 
 class LazyConfig(ctypes.Structure):
@@ -71,6 +74,19 @@ def lib() -> ctypes.CDLL:
         L.lazy_host_step_staging_bytes.argtypes = [vp, i32, i32, i32]
         L.lazy_host_step.restype = ctypes.c_int
         L.lazy_host_step.argtypes = [vp, ctypes.POINTER(HostStep), vp]
+        L.lazy_pool_create.restype = vp
+        L.lazy_pool_create.argtypes = [i32, i32, i32]
+        L.lazy_pool_destroy.restype = None
+        L.lazy_pool_destroy.argtypes = [vp]
+        L.lazy_pool_acquire.restype = ctypes.c_int
+        L.lazy_pool_acquire.argtypes = [vp, i64, i32, i32, ctypes.POINTER(i32)]
+        L.lazy_pool_release.restype = ctypes.c_int
+        L.lazy_pool_release.argtypes = [vp, i64, i32]
+        L.lazy_pool_stats.restype = None
+        L.lazy_pool_stats.argtypes = [vp, ctypes.POINTER(i64), ctypes.POINTER(i64), ctypes.POINTER(i64),
+                                      ctypes.POINTER(i32)]
+        L.lazy_hit_ratio_model.restype = ctypes.c_double
+        L.lazy_hit_ratio_model.argtypes = [ctypes.c_double, i64, i64, i32]
         _lib = L
     return _lib
 
@@ -238,3 +254,47 @@ def lazy_host_step(h: LazyHandle, args: HostStep, stream=None) -> None:
     rc = lib().lazy_host_step(h.ptr, ctypes.byref(args), _stream(stream))
     if rc != 0:
         raise LazyError("lazy_host_step", rc)
+
+
+class LazyPool:
+    """Host page pool (lazy_pool_*): marshalling only."""
+
+    def __init__(self, num_pages: int, page_size: int = 16, keying: int = LAZY_POOL_AGNOSTIC):
+        self.page_size = page_size
+        self._p = lib().lazy_pool_create(num_pages, page_size, keying)
+        if not self._p:
+            raise LazyError("lazy_pool_create", LAZY_ERR_INVALID)
+
+    def acquire(self, doc_id: int, doc_tokens: int, logical_pos: int = 0):
+        """Returns (hit: bool, pages: list[int]); raises LazyError when the document cannot be placed."""
+        n = (doc_tokens + self.page_size - 1) // self.page_size
+        buf = (ctypes.c_int32 * n)()
+        rc = lib().lazy_pool_acquire(self._p, doc_id, doc_tokens, logical_pos, buf)
+        if rc < 0:
+            raise LazyError("lazy_pool_acquire", rc)
+        return rc == 1, list(buf)
+
+    def release(self, doc_id: int, logical_pos: int = 0) -> None:
+        rc = lib().lazy_pool_release(self._p, doc_id, logical_pos)
+        if rc != 0:
+            raise LazyError("lazy_pool_release", rc)
+
+    def stats(self) -> dict:
+        a, b, c, d = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int32()
+        lib().lazy_pool_stats(self._p, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c), ctypes.byref(d))
+        return dict(lookups=a.value, hits=b.value, evictions=c.value, pages_in_use=d.value)
+
+    def close(self):
+        if getattr(self, "_p", None):
+            lib().lazy_pool_destroy(self._p)
+            self._p = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def lazy_hit_ratio_model(alpha: float, num_docs: int, capacity_entries: int, positions: int = 1) -> float:
+    return float(lib().lazy_hit_ratio_model(alpha, num_docs, capacity_entries, positions))

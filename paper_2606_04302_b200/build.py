@@ -16,20 +16,20 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(CSRC, "liblazyattn.so")
-SOURCES = ["lazy_api.cu", "basic_kernels.cu", "decode_splitkv.cu", "prefill_umma.cu"]
+SOURCES = ["lazy_api.cu", "basic_kernels.cu", "decode_splitkv.cu", "prefill_umma.cu", "page_pool.cpp"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
          "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC] + os.environ.get("LAZY_NVCC_EXTRA", "").split()
 
 
 def _deps_mtime() -> float:
-    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h"))]
+    files = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cu", ".cuh", ".h", ".cpp"))]
     files += [os.path.join(INCLUDE, f) for f in os.listdir(INCLUDE)]
     return max(os.path.getmtime(f) for f in files)
 
 
 def _compile(src: str, verbose: bool) -> str:
-    obj = os.path.join(CSRC, src.replace(".cu", ".o"))
+    obj = os.path.join(CSRC, os.path.splitext(src)[0] + ".o")
     cmd = [NVCC, *FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")

@@ -1,0 +1,102 @@
+"""Host page pool and hit-ratio model (Eq. 1-3, Table 1): CPU only."""
+import numpy as np
+import pytest
+
+from oracle import cache_model as M
+from paper_2606_04302_b200 import binding as B
+from paper_2606_04302_b200 import build as lazy_build
+from paper_2606_04302_b200.workloads import zipf_probs
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    lazy_build.build()
+    B.lib()
+
+
+def test_hit_ratio_model_matches_equations():
+    """Eq. 1 / Eq. 2 against the plain sums; Eq. 3's printed example: D = 20, C = 100 gives 2.86x for a 'moderately
+    skewed' Zipf -- the exponent is not printed; the equation gives 2.86 at alpha = 0.853 (2.27 at 1.0, 3.13 at 0.8)."""
+    for alpha, n, c, d in [(1.0, 1000, 100, 1), (1.1, 5000, 300, 10), (2.1, 100, 50, 7), (0.0, 10, 4, 2)]:
+        want = M.hit_ratio_aware(alpha, n, c, d) if d > 1 else M.hit_ratio_agnostic(alpha, n, c)
+        assert abs(B.lazy_hit_ratio_model(alpha, n, c, d) - want) < 1e-12
+    # closed forms: alpha = 0 is uniform -> C/N; capacity >= N -> 1
+    assert abs(B.lazy_hit_ratio_model(0.0, 200, 50, 1) - 0.25) < 1e-15
+    assert B.lazy_hit_ratio_model(1.3, 40, 40, 1) == 1.0
+    ratio = lambda a: B.lazy_hit_ratio_model(a, 10 ** 4, 100, 1) / B.lazy_hit_ratio_model(a, 10 ** 4, 100, 20)
+    assert abs(ratio(0.853) - 2.86) < 0.01 and abs(ratio(0.853) - M.advantage(0.853, 100, 20)) < 1e-12
+    assert abs(ratio(1.0) - 2.27) < 0.01 and abs(ratio(0.8) - 3.13) < 0.01
+    assert B.lazy_hit_ratio_model(1.0, 0, 1, 1) == -1.0
+
+
+def _trace(seed, n_requests, docs_per_req, pool_docs, alpha, n_positions):
+    rng = np.random.default_rng(seed)
+    p = zipf_probs(pool_docs, alpha)
+    for _ in range(n_requests):
+        docs = rng.choice(pool_docs, size=docs_per_req, replace=False, p=p)
+        yield [(int(d), int(k)) for k, d in enumerate(rng.permutation(docs))]      # (doc, slot in the prompt)
+
+
+@pytest.mark.parametrize("keying", [B.LAZY_POOL_AGNOSTIC, B.LAZY_POOL_POSITION_AWARE])
+def test_pool_matches_brute_force_lru(keying):
+    """Same seeded Zipf request trace through the C++ pool and the brute-force pool: identical hit/miss decisions,
+    identical page ids, identical eviction counts; pinned documents are never evicted."""
+    doc_tokens, page = 64, 16
+    pool = B.LazyPool(num_pages=4 * 30, page_size=page, keying=keying)
+    ref = M.BruteForcePool(4 * 30, page, keying == B.LAZY_POOL_POSITION_AWARE)
+    try:
+        for req in _trace(11, 400, 5, 200, 1.1, 5):
+            got = [pool.acquire(d, doc_tokens, k * doc_tokens) for d, k in req]
+            want = [ref.acquire(d, doc_tokens, k * doc_tokens) for d, k in req]
+            assert got == want
+            pages = [pg for _, ps in got for pg in ps]
+            assert len(set(pages)) == len(pages)                    # pinned documents of one request never overlap
+            for d, k in req:
+                pool.release(d, k * doc_tokens); ref.release(d, k * doc_tokens)
+        st = pool.stats()
+        assert (st["lookups"], st["hits"], st["evictions"]) == (ref.lookups, ref.hits, ref.evictions)
+        assert st["hits"] > 0 and st["evictions"] > 0
+    finally:
+        pool.close()
+
+
+def test_position_agnostic_pool_hits_more_under_the_same_budget():
+    """The cache-level claim (Table 1): same page budget, same trace -- keying by document alone hits
+    more often than keying by (document, position), and tracks Eq. 1 for an LRU cache under Zipf popularity."""
+    res = {}
+    for keying in (B.LAZY_POOL_AGNOSTIC, B.LAZY_POOL_POSITION_AWARE):
+        pool = B.LazyPool(num_pages=4 * 100, page_size=16, keying=keying)
+        for req in _trace(5, 3000, 10, 2000, 1.1, 10):
+            for d, k in req:
+                pool.acquire(d, 64, k * 64)
+            for d, k in req:
+                pool.release(d, k * 64)
+        st = pool.stats()
+        res[keying] = st["hits"] / st["lookups"]
+        pool.close()
+    assert res[B.LAZY_POOL_AGNOSTIC] > 1.5 * res[B.LAZY_POOL_POSITION_AWARE]
+    model = B.lazy_hit_ratio_model(1.1, 2000, 100, 1)               # ideal top-C cache; LRU sits a little below it
+    assert 0.6 * model < res[B.LAZY_POOL_AGNOSTIC] <= model + 0.02
+
+
+def test_pool_pins_and_errors():
+    pool = B.LazyPool(num_pages=8, page_size=16)
+    try:
+        hit, a = pool.acquire(1, 64, 0)
+        hit2, b = pool.acquire(2, 64, 64)
+        assert (hit, hit2) == (False, False) and sorted(a + b) == list(range(8))
+        with pytest.raises(B.LazyError):                            # both pinned: nothing can be evicted
+            pool.acquire(3, 16, 0)
+        pool.release(1, 0)
+        hit3, c = pool.acquire(3, 16, 128)                          # evicts document 1, reuses one of its pages
+        assert not hit3 and c[0] in a
+        assert pool.acquire(2, 64, 999) == (True, b)                # position-agnostic: any offset hits
+        with pytest.raises(B.LazyError):
+            pool.acquire(2, 32, 0)                                  # a different length is a different document
+        with pytest.raises(B.LazyError):
+            pool.release(7, 0)
+        assert pool.stats()["evictions"] == 1
+    finally:
+        pool.close()
+    with pytest.raises(B.LazyError):
+        B.LazyPool(0)
