@@ -189,3 +189,25 @@ def test_host_step_matches_device_calls():
     torch.cuda.synchronize()
     assert torch.equal(hout.view(torch.int16), want.cpu().view(torch.int16))
     dev.close(); dev2.close()
+
+
+def test_many_requests_cross_the_per_launch_limit():
+    """Maximum sizes: more requests than one decode launch keeps in shared memory (2048) -> lazy_attn_decode splits
+    the batch into several launches; many short prefill chunks -> one CTA per (request, kv head)."""
+    rng = np.random.default_rng(3)
+    R = 2300
+    lens = rng.integers(0, 40, size=R).tolist()
+    lens[5] = 0
+    lens[2047] = 33; lens[2048] = 17; lens[2299] = 1
+    _check(_custom(SH64, lens, [1] * R, seed=21, kind="decode"))
+    R = 300
+    lens = rng.integers(1, 50, size=R).tolist()
+    qs = [int(min(L, rng.integers(1, 20))) for L in lens]
+    _check(_custom(SH64, lens, qs, seed=22))
+
+
+def test_long_chunk_prefill_and_single_key():
+    """A 2 000-token chunk over a short prefix (many m-blocks per request, mostly causal tiles) next to a request
+    whose query sees exactly one key."""
+    _check(_custom(SH128, [2100, 1, 130], [2000, 1, 130], seed=23))
+    _check(_custom(SH7, [1500, 1], [1500, 1], seed=24))
