@@ -408,7 +408,7 @@ def oracle_sample(workload, batch, budget_s=20.0):
         else:
             nq = int(st.cu_q_lens[1] - st.cu_q_lens[0])
             L = int(st.seq_lens[0])
-            rows = min(nq, 16)
+            rows = min(nq, 128)
             sel = np.zeros(nq, dtype=np.uint8)
             pick = np.sort(np.random.default_rng(0).choice(nq, size=rows, replace=False))
             sel[pick] = 1
