@@ -440,6 +440,8 @@ def main():
     ap.add_argument("--noshare", action="store_true", help="every drawn document distinct (logical == unique bytes)")
     ap.add_argument("--no-secondary", action="store_true", help="skip the prefill (cfg3) and noshare side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mixed", action="store_true",
+                    help="cfg5: also time the step with lazy_attn_mixed (prefill and decode concurrently, f4)")
     ap.add_argument("--graph", action="store_true",
                     help="also replay the step from a CUDA graph (f4) and report its time next to the eager one")
     ap.add_argument("--ablation", action="store_true",
@@ -569,6 +571,32 @@ def main():
                 "d2h_bytes_per_step": int(sum(e["d2h"] for e in job.e2e))},
         "gpu_launches": int(launches), "clocks": clocks,
     }
+    if args.mixed and rank == 0 and world == 1 and args.workload == "cfg5":
+        B, dev = job.B, job.dev
+        rp = [r for r in job.timed if r["step"].kind == "prefill"][0]
+        rd = [r for r in job.timed if r["step"].kind == "decode"][0]
+
+        def mixed_step(sms):
+            for rec in job.timed:
+                B.lazy_cache_write(dev.handle, rec["k_new"], rec["v_new"], rec["slots"], dev.k_pool, dev.v_pool)
+            B.lazy_attn_mixed(dev.handle, dev.k_pool, dev.v_pool, q_prefill=rp["q"], block_table_prefill=rp["bt"],
+                              page_logical_pos_prefill=rp["pp"], seq_lens_prefill=rp["sl"], cu_q_lens=rp["cu"],
+                              max_q_len=rp["max_q"], out_prefill=rp["out"], q_decode=rd["q"], block_table_decode=rd["bt"],
+                              page_logical_pos_decode=rd["pp"], seq_lens_decode=rd["sl"], out_decode=rd["out"],
+                              decode_sms=sms)
+        res = {}
+        for sms in (0, 64, 96, 128):
+            for _ in range(3):
+                job.flush_l2(); mixed_step(sms)
+            evs = []
+            for _ in range(args.steps):
+                job.flush_l2()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(); mixed_step(sms); e1.record()
+                evs.append((e0, e1))
+            torch.cuda.synchronize()
+            res[f"decode_sms_{sms if sms else 'default'}"] = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        out["mixed"] = {"ms_per_step": res, "separate_calls_ms_per_step": ms_step}
     if args.graph and rank == 0 and world == 1:
         g = torch.cuda.CUDAGraph()
         side = torch.cuda.Stream()

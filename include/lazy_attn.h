@@ -221,6 +221,27 @@ size_t lazy_host_step_staging_bytes(const lazy_handle* h, int32_t num_reqs, int3
                                     int32_t num_new_tokens);
 int lazy_host_step(lazy_handle* h, const lazy_host_step_args* a, void* stream);
 
+/* f4. One serving step's attention for a MIXED batch: the block-local prefill of cache-miss documents (or any
+ * prefill chunk) and the decode of the running requests, issued together (Fig. 5 phases 1-3 happen in one
+ * engine step).  Same results as lazy_attn_prefill followed by lazy_attn_decode; the two
+ * kernels run CONCURRENTLY: the decode kernel (HBM-bound) is confined to `decode_sms` SMs on a library-owned side
+ * stream forked from and joined back into `stream` with events, the prefill kernel (tensor-bound) takes the other
+ * SMs and, as decode CTAs retire, theirs too.  No host synchronisation; capturable in a CUDA graph.  The side stream
+ * and two events are host-side resources created at the first call and released by lazy_destroy.
+ * Field meanings are those of the two calls above; the two request sets use separate tables. */
+typedef struct lazy_mixed_args {
+  const void* q_prefill;  const int32_t* block_table_prefill;  const int32_t* page_logical_pos_prefill;
+  const int32_t* seq_lens_prefill;  const int32_t* cu_q_lens;
+  int32_t num_reqs_prefill, total_q, max_q_len, reserved0;
+  void* out_prefill;
+  const void* q_decode;  const int32_t* block_table_decode;  const int32_t* page_logical_pos_decode;
+  const int32_t* seq_lens_decode;
+  int32_t num_reqs_decode;
+  int32_t decode_sms;     /* SMs the decode kernel may occupy while both run; 0 = three quarters of the device     */
+  void* out_decode;
+} lazy_mixed_args;
+int lazy_attn_mixed(lazy_handle* h, const lazy_mixed_args* a, const void* k_cache, const void* v_cache, void* stream);
+
 /* ---- f4 (host side): document-granular page pool with reference counts and LRU eviction ----------------------
  * Pure host code, no CUDA call: it hands out PHYSICAL PAGE IDS of the caller's k_cache / v_cache.  One physical copy
  * per document, reusable at any logical position with LAZY_POOL_AGNOSTIC; with

@@ -20,7 +20,7 @@ LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
            "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_alibi_slopes", "lazy_set_page_stored_pos",
-           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step",
+           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step", "lazy_attn_mixed",
            "lazy_pool_create", "lazy_pool_destroy", "lazy_pool_acquire", "lazy_pool_release", "lazy_pool_stats",
            "lazy_hit_ratio_model"]
 LAZY_POOL_AGNOSTIC, LAZY_POOL_POSITION_AWARE = 0, 1
@@ -74,6 +74,8 @@ def lib() -> ctypes.CDLL:
         L.lazy_host_step_staging_bytes.argtypes = [vp, i32, i32, i32]
         L.lazy_host_step.restype = ctypes.c_int
         L.lazy_host_step.argtypes = [vp, ctypes.POINTER(HostStep), vp]
+        L.lazy_attn_mixed.restype = ctypes.c_int
+        L.lazy_attn_mixed.argtypes = [vp, ctypes.POINTER(MixedArgs), vp, vp, vp]
         L.lazy_pool_create.restype = vp
         L.lazy_pool_create.argtypes = [i32, i32, i32]
         L.lazy_pool_destroy.restype = None
@@ -232,6 +234,30 @@ def lazy_materialize_pages(h: LazyHandle, k_src, v_src, src_pages, rot_pos, per_
                                       _stream(stream))
     if rc != 0:
         raise LazyError("lazy_materialize_pages", rc)
+
+
+class MixedArgs(ctypes.Structure):
+    """Mirror of lazy_mixed_args (include/lazy_attn.h)."""
+    _fields_ = [("q_prefill", ctypes.c_void_p), ("block_table_prefill", ctypes.c_void_p),
+                ("page_logical_pos_prefill", ctypes.c_void_p), ("seq_lens_prefill", ctypes.c_void_p),
+                ("cu_q_lens", ctypes.c_void_p), ("num_reqs_prefill", ctypes.c_int32), ("total_q", ctypes.c_int32),
+                ("max_q_len", ctypes.c_int32), ("reserved0", ctypes.c_int32), ("out_prefill", ctypes.c_void_p),
+                ("q_decode", ctypes.c_void_p), ("block_table_decode", ctypes.c_void_p),
+                ("page_logical_pos_decode", ctypes.c_void_p), ("seq_lens_decode", ctypes.c_void_p),
+                ("num_reqs_decode", ctypes.c_int32), ("decode_sms", ctypes.c_int32), ("out_decode", ctypes.c_void_p)]
+
+
+def lazy_attn_mixed(h: LazyHandle, k_cache, v_cache, *, q_prefill, block_table_prefill, page_logical_pos_prefill,
+                    seq_lens_prefill, cu_q_lens, max_q_len: int, out_prefill, q_decode, block_table_decode,
+                    page_logical_pos_decode, seq_lens_decode, out_decode, decode_sms: int = 0, stream=None) -> None:
+    args = MixedArgs(_ptr(q_prefill), _ptr(block_table_prefill), _ptr(page_logical_pos_prefill),
+                     _ptr(seq_lens_prefill), _ptr(cu_q_lens), int(seq_lens_prefill.shape[0]), int(q_prefill.shape[0]),
+                     int(max_q_len), 0, _ptr(out_prefill), _ptr(q_decode), _ptr(block_table_decode),
+                     _ptr(page_logical_pos_decode), _ptr(seq_lens_decode), int(seq_lens_decode.shape[0]),
+                     int(decode_sms), _ptr(out_decode))
+    rc = lib().lazy_attn_mixed(h.ptr, ctypes.byref(args), _ptr(k_cache), _ptr(v_cache), _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_attn_mixed", rc)
 
 
 class HostStep(ctypes.Structure):

@@ -623,7 +623,7 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
     a.num_reqs = n;
     a.q_interleaved = c.rope_style == LAZY_ROPE_INTERLEAVED;
     a.sh = h->shape;
-    int gx = h->num_sms / HG;
+    int gx = (h->decode_cta_limit > 0 ? h->decode_cta_limit : h->num_sms) / HG;
     if (gx < 1) gx = 1;
     if (gx > kMaxDecodeCtas) gx = kMaxDecodeCtas;
     int rc;

@@ -114,7 +114,15 @@ int lazy_create(const lazy_config* cfg, void* workspace, size_t workspace_bytes,
   return LAZY_OK;
 }
 
-void lazy_destroy(lazy_handle* h) { delete h; }
+void lazy_destroy(lazy_handle* h) {
+  if (!h) return;
+  if (h->side_stream) {
+    cudaStreamDestroy(h->side_stream);
+    cudaEventDestroy(h->ev_fork);
+    cudaEventDestroy(h->ev_join);
+  }
+  delete h;
+}
 
 int lazy_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
                      int32_t num_tokens, void* k_cache, void* v_cache, void* stream) {
@@ -235,6 +243,46 @@ int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const v
   if (n < 0) return n;
   h->launches += n;
   return LAZY_OK;
+}
+
+int lazy_attn_mixed(lazy_handle* h, const lazy_mixed_args* a, const void* k_cache, const void* v_cache, void* stream) {
+  if (!h || !a) return LAZY_ERR_INVALID;
+  if (a->num_reqs_prefill < 0 || a->num_reqs_decode < 0 || a->decode_sms < 0) return LAZY_ERR_INVALID;
+  if (h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS) return LAZY_ERR_UNSUPPORTED;
+  const bool has_p = a->num_reqs_prefill > 0 && a->total_q > 0, has_d = a->num_reqs_decode > 0;
+  if (!has_p || !has_d) {                       // nothing to overlap: plain calls
+    int rc = LAZY_OK;
+    if (has_p)
+      rc = lazy_attn_prefill(h, a->q_prefill, k_cache, v_cache, a->block_table_prefill, a->page_logical_pos_prefill,
+                             a->seq_lens_prefill, a->cu_q_lens, a->num_reqs_prefill, a->total_q, a->max_q_len,
+                             a->out_prefill, stream);
+    if (rc == LAZY_OK && has_d)
+      rc = lazy_attn_decode(h, a->q_decode, k_cache, v_cache, a->block_table_decode, a->page_logical_pos_decode,
+                            a->seq_lens_decode, a->num_reqs_decode, a->out_decode, stream);
+    return rc;
+  }
+  if (!h->side_stream) {
+    if (cudaStreamCreateWithFlags(&h->side_stream, cudaStreamNonBlocking) != cudaSuccess) return LAZY_ERR_CUDA;
+    if (cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess)
+      return LAZY_ERR_CUDA;
+  }
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  if (cudaEventRecord(h->ev_fork, s) != cudaSuccess || cudaStreamWaitEvent(h->side_stream, h->ev_fork, 0) != cudaSuccess)
+    return LAZY_ERR_CUDA;
+  // decode first, on the side stream, confined to a subset of the SMs (one persistent CTA per SM)
+  h->decode_cta_limit = a->decode_sms > 0 ? (a->decode_sms < h->num_sms ? a->decode_sms : h->num_sms) : h->num_sms * 3 / 4;
+  int rc = lazy_attn_decode(h, a->q_decode, k_cache, v_cache, a->block_table_decode, a->page_logical_pos_decode,
+                            a->seq_lens_decode, a->num_reqs_decode, a->out_decode, h->side_stream);
+  h->decode_cta_limit = 0;
+  if (rc == LAZY_OK)
+    rc = lazy_attn_prefill(h, a->q_prefill, k_cache, v_cache, a->block_table_prefill, a->page_logical_pos_prefill,
+                           a->seq_lens_prefill, a->cu_q_lens, a->num_reqs_prefill, a->total_q, a->max_q_len,
+                           a->out_prefill, stream);
+  // join even on error so the caller's stream never outruns the side stream
+  if (cudaEventRecord(h->ev_join, h->side_stream) != cudaSuccess || cudaStreamWaitEvent(s, h->ev_join, 0) != cudaSuccess)
+    return LAZY_ERR_CUDA;
+  return rc;
 }
 
 const char* lazy_status_string(int status) {

@@ -40,6 +40,9 @@ struct lazy_handle {
   int num_sms;
   int64_t launches;
   const int32_t* page_stored_pos;   // LAZY_K_STORED_POS: device [num_pages], caller-owned
+  int decode_cta_limit;             // > 0: lazy_attn_mixed confines the decode kernel to this many CTAs (= SMs)
+  cudaStream_t side_stream;         // lazy_attn_mixed: library-owned fork stream and its two events (host resources)
+  cudaEvent_t ev_fork, ev_join;
   float alibi_host[lazy::kMaxAlibiHeads];   // staging copy of the slopes (source of the async H2D copy)
   // cached TMA descriptors (128 bytes each), keyed by the pool pointer they were encoded for
   alignas(64) unsigned char tmap_k[128];
