@@ -475,23 +475,36 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
         const int hq = hg * heads_cta + hh;
         const int n_slots = n_parts * C::PPS;
         const int slot0 = (r + b_first) * C::PPS;
-        float mstar = -INFINITY;
-        for (int sidx = 0; sidx < n_slots; ++sidx)
-          mstar = fmaxf(mstar, __ldcg(&a.part_ml[(size_t)(slot0 + sidx) * sh.Hq + hq]).x);
+        // single pass with a running max; the loads of four partials are issued together so that their L2
+        // latencies overlap (the partials were written by other SMs)
+        float mstar = -INFINITY, lsum = 0.f;
         float acc[D / 32];
 #pragma unroll
         for (int x = 0; x < D / 32; ++x) acc[x] = 0.f;
-        float lsum = 0.f;
-        for (int sidx = 0; sidx < n_slots; ++sidx) {
-          float2 ml = __ldcg(&a.part_ml[(size_t)(slot0 + sidx) * sh.Hq + hq]);
-          if (ml.x == -INFINITY) continue;
-          float w = exp2f(ml.x - mstar);
-          lsum += w * ml.y;
-          const float* po = a.part_o + ((size_t)(slot0 + sidx) * sh.Hq + hq) * D + lane * (D / 32);
+        for (int base = 0; base < n_slots; base += 4) {
+          float2 ml[4];
+          float2 pv[4][D / 64];
 #pragma unroll
-          for (int x = 0; x < D / 32; x += 2) {
-            float2 v = __ldcg(reinterpret_cast<const float2*>(po + x));
-            acc[x] += w * v.x; acc[x + 1] += w * v.y;
+          for (int i = 0; i < 4; ++i) {
+            const int sidx = min(base + i, n_slots - 1);
+            ml[i] = __ldcg(&a.part_ml[(size_t)(slot0 + sidx) * sh.Hq + hq]);
+            const float2* po = reinterpret_cast<const float2*>(a.part_o + ((size_t)(slot0 + sidx) * sh.Hq + hq) * D +
+                                                               lane * (D / 32));
+#pragma unroll
+            for (int x = 0; x < D / 64; ++x) pv[i][x] = __ldcg(po + x);
+          }
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            if (base + i >= n_slots || ml[i].x == -INFINITY) continue;
+            const float mnew = fmaxf(mstar, ml[i].x);
+            const float f = exp2f(mstar - mnew), w = exp2f(ml[i].x - mnew);   // mstar = -inf on the first: f = 0
+            mstar = mnew;
+            lsum = lsum * f + w * ml[i].y;
+#pragma unroll
+            for (int x = 0; x < D / 64; ++x) {
+              acc[2 * x] = acc[2 * x] * f + w * pv[i][x].x;
+              acc[2 * x + 1] = acc[2 * x + 1] * f + w * pv[i][x].y;
+            }
           }
         }
         const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
