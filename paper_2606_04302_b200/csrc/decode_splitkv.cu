@@ -453,14 +453,14 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
         if (g == 0) a.part_ml[(size_t)slot * sh.Hq + hq] = make_float2(m_run[e], l_run[e]);
       }
     }
-    __threadfence();
-    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    ptx::named_bar_sync(1, kConsumerWarps * 32);    // all partials of this CTA are written (CTA-scope order) ...
     // number of CTAs that hold a piece of request r: those containing units cum[r] .. cum[r+1]-1
     const long long c0 = s_cum[r], c1 = s_cum[r + 1];
     const int b_first = (int)(((c0 + 1) * G + U - 1) / U) - 1;
     const int b_last = (int)((c1 * G + U - 1) / U) - 1;
     const int n_parts = b_last - b_first + 1;
     if (tid == 0) {
+      __threadfence();                              // ... and one cumulative gpu-scope release publishes them
       int old = atomicAdd(&a.req_counter[r * HG + hg], 1);
       int last = (old == n_parts - 1);
       if (last) a.req_counter[r * HG + hg] = 0;     // self-resetting: ready for the next call
