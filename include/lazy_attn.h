@@ -184,6 +184,14 @@ int lazy_materialize_pages(lazy_handle* h, const void* k_src, const void* v_src,
 /* Static description of a status code (host string, never NULL). */
 const char* lazy_status_string(int status);
 
+/* Debug aid (the ONLY synchronising call; never on the serving path): checks the CONTENTS of the device tables
+ * that the attention calls trust -- for every request r < num_reqs and every slot below ceil(seq_len / page_size):
+ * 0 <= block_table < num_pages, 0 <= page_logical_pos and page_logical_pos + page_size <= max_position; and
+ * 0 <= seq_len <= max_pages_per_req * page_size.  Returns the number of violations (>= 0) after synchronising
+ * `stream`, or a negative status.  Uses 4 bytes of the workspace. */
+int64_t lazy_debug_validate(lazy_handle* h, const int32_t* block_table, const int32_t* page_logical_pos,
+                            const int32_t* seq_lens, int32_t num_reqs, void* stream);
+
 /* Introspection for tests and bench.py: number of kernel launches this handle has enqueued so far. */
 int64_t lazy_launch_count(const lazy_handle* h);
 

@@ -20,7 +20,7 @@ LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
            "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_alibi_slopes", "lazy_set_page_stored_pos",
-           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step", "lazy_attn_mixed",
+           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step", "lazy_attn_mixed", "lazy_debug_validate",
            "lazy_pool_create", "lazy_pool_destroy", "lazy_pool_acquire", "lazy_pool_release", "lazy_pool_stats",
            "lazy_hit_ratio_model"]
 LAZY_POOL_AGNOSTIC, LAZY_POOL_POSITION_AWARE = 0, 1
@@ -76,6 +76,8 @@ def lib() -> ctypes.CDLL:
         L.lazy_host_step.argtypes = [vp, ctypes.POINTER(HostStep), vp]
         L.lazy_attn_mixed.restype = ctypes.c_int
         L.lazy_attn_mixed.argtypes = [vp, ctypes.POINTER(MixedArgs), vp, vp, vp]
+        L.lazy_debug_validate.restype = i64
+        L.lazy_debug_validate.argtypes = [vp, vp, vp, vp, i32, vp]
         L.lazy_pool_create.restype = vp
         L.lazy_pool_create.argtypes = [i32, i32, i32]
         L.lazy_pool_destroy.restype = None
@@ -236,6 +238,15 @@ def lazy_materialize_pages(h: LazyHandle, k_src, v_src, src_pages, rot_pos, per_
         raise LazyError("lazy_materialize_pages", rc)
 
 
+def lazy_debug_validate(h: LazyHandle, block_table, page_logical_pos, seq_lens, stream=None) -> int:
+    """Synchronising debug call: number of table entries the attention kernels would misuse."""
+    rc = int(lib().lazy_debug_validate(h.ptr, _ptr(block_table), _ptr(page_logical_pos), _ptr(seq_lens),
+                                       int(seq_lens.shape[0]), _stream(stream)))
+    if rc < 0:
+        raise LazyError("lazy_debug_validate", rc)
+    return rc
+
+
 class MixedArgs(ctypes.Structure):
     """Mirror of lazy_mixed_args (include/lazy_attn.h)."""
     _fields_ = [("q_prefill", ctypes.c_void_p), ("block_table_prefill", ctypes.c_void_p),
@@ -257,7 +268,7 @@ def lazy_attn_mixed(h: LazyHandle, k_cache, v_cache, *, q_prefill, block_table_p
                      int(decode_sms), _ptr(out_decode))
     rc = lib().lazy_attn_mixed(h.ptr, ctypes.byref(args), _ptr(k_cache), _ptr(v_cache), _stream(stream))
     if rc != 0:
-        raise LazyError("lazy_attn_mixed", rc)
+        raise LazyError("lazy_attn_mixed", "lazy_debug_validate", rc)
 
 
 class HostStep(ctypes.Structure):

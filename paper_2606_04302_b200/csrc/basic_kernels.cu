@@ -96,6 +96,32 @@ int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, con
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// lazy_debug_validate: one CTA per request counts table entries the attention kernels would misuse.
+__global__ void validate_tables_kernel(const int* __restrict__ block_table, const int* __restrict__ page_pos,
+                                       const int* __restrict__ seq_lens, int table_stride, int num_pages,
+                                       int max_position, int* __restrict__ counter) {
+  const int r = blockIdx.x;
+  const int L = seq_lens[r];
+  int bad = 0;
+  if (threadIdx.x == 0 && (L < 0 || L > table_stride * kPageSize)) bad++;
+  const int np = L < 0 ? 0 : min((L + kPageSize - 1) / kPageSize, table_stride);
+  for (int s = threadIdx.x; s < np; s += blockDim.x) {
+    const int pg = block_table[(size_t)r * table_stride + s], pos = page_pos[(size_t)r * table_stride + s];
+    if (pg < 0 || pg >= num_pages) bad++;
+    if (pos < 0 || pos > max_position - kPageSize) bad++;
+  }
+  if (bad) atomicAdd(counter, bad);
+}
+
+int launch_validate(lazy_handle* h, const int32_t* block_table, const int32_t* page_logical_pos,
+                    const int32_t* seq_lens, int num_reqs, int* counter, cudaStream_t stream) {
+  validate_tables_kernel<<<num_reqs, 128, 0, stream>>>(block_table, page_logical_pos, seq_lens,
+                                                       h->cfg.max_pages_per_req, h->cfg.num_pages, h->cfg.max_position,
+                                                       counter);
+  return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
+}
+
+// ---------------------------------------------------------------------------------------------------------
 // Materialising re-encoding ("allocate + copy + rotate", L447).  HBM-bound:
 // per page it reads Hkv*16*D*2 B of K (and of V) and writes the same.  One thread owns one 8-pair chunk of one
 // row: two 16-byte loads (dims 8c.. and D/2+8c..), fp32 rotation from the fp64-built table, two 16-byte stores.

@@ -285,6 +285,24 @@ int lazy_attn_mixed(lazy_handle* h, const lazy_mixed_args* a, const void* k_cach
   return rc;
 }
 
+int64_t lazy_debug_validate(lazy_handle* h, const int32_t* block_table, const int32_t* page_logical_pos,
+                            const int32_t* seq_lens, int32_t num_reqs, void* stream) {
+  if (!h || num_reqs < 0 || num_reqs > h->cfg.max_reqs) return LAZY_ERR_INVALID;
+  if (num_reqs == 0) return 0;
+  if (!block_table || !page_logical_pos || !seq_lens) return LAZY_ERR_INVALID;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  int* counter = h->ws.sched + 512;               // a word of the scheduling scratch no kernel uses
+  if (cudaMemsetAsync(counter, 0, sizeof(int), s) != cudaSuccess) return LAZY_ERR_CUDA;
+  int n = lazy::launch_validate(h, block_table, page_logical_pos, seq_lens, num_reqs, counter, s);
+  if (n < 0) return n;
+  h->launches += n;
+  int host = 0;
+  if (cudaMemcpyAsync(&host, counter, sizeof(int), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+      cudaStreamSynchronize(s) != cudaSuccess)
+    return LAZY_ERR_CUDA;
+  return host;
+}
+
 const char* lazy_status_string(int status) {
   switch (status) {
     case LAZY_OK: return "ok";

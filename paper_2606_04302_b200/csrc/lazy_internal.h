@@ -74,6 +74,8 @@ int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, con
 int launch_materialize(lazy_handle* h, const void* k_src, const void* v_src, const int32_t* src_pages,
                        const int32_t* rot_pos, int per_token, void* k_dst, void* v_dst, const int32_t* dst_pages,
                        int num, cudaStream_t stream);
+int launch_validate(lazy_handle* h, const int32_t* block_table, const int32_t* page_logical_pos,
+                    const int32_t* seq_lens, int num_reqs, int* counter, cudaStream_t stream);
 int launch_rowwise(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                    const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                    const int32_t* cu_q_lens, int num_reqs, int total_q, int max_q_len, void* out,

@@ -211,3 +211,25 @@ def test_long_chunk_prefill_and_single_key():
     whose query sees exactly one key."""
     _check(_custom(SH128, [2100, 1, 130], [2000, 1, 130], seed=23))
     _check(_custom(SH7, [1500, 1], [1500, 1], seed=24))
+
+
+def test_debug_validate_counts_bad_table_entries():
+    batch = W.config2(scale=0.05)
+    dev = DeviceBatch(batch)
+    try:
+        st = [s for s in batch.steps if s.kind == "decode"][0]
+        bt, pp = dev.tables_for(st)
+        sl = st.seq_lens.cuda()
+        assert B.lazy_debug_validate(dev.handle, bt, pp, sl) == 0
+        bt2, pp2, sl2 = bt.clone(), pp.clone(), sl.clone()
+        bt2[0, 0] = batch.num_pages            # page id out of range
+        bt2[1, 3] = -1
+        pp2[0, 1] = batch.max_position         # position beyond the table
+        sl2[2] = bt.shape[1] * 16 + 1          # longer than the table row
+        assert B.lazy_debug_validate(dev.handle, bt2, pp2, sl2) == 4
+        bt2[0, bt.shape[1] - 1] = -7           # beyond ceil(seq_len / 16): ignored, as the attention calls do
+        sl3 = sl.clone()
+        sl3[0] = 100
+        assert B.lazy_debug_validate(dev.handle, bt2, pp2, sl3) == 3
+    finally:
+        dev.close()
