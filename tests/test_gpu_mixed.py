@@ -54,3 +54,34 @@ def test_mixed_step_matches_oracle_and_separate_calls(decode_sms):
         assert torch.equal(dev.k_pool.cpu().view(torch.int16), k_ref.view(torch.int16))
     finally:
         dev.close()
+
+
+def test_mixed_step_full_size_cfg5_sampled():
+    """BASELINE.json configs[4] at full size through the call bench.py times for it (lazy_attn_mixed, default SM
+    share): all decode rows and 64 seeded prefill rows against the oracle."""
+    batch = W.config5()
+    pre, dec = batch.steps[0], batch.steps[1]
+    dev = DeviceBatch(batch)
+    d = dev.device
+    k_ref, v_ref = batch.k_pool.clone(), batch.v_pool.clone()
+    try:
+        dev.write(pre); dev.write(dec)
+        rows = np.sort(np.random.default_rng(5).choice(pre.q.shape[0], size=64, replace=False))
+        sel = np.zeros(pre.q.shape[0], dtype=np.uint8); sel[rows] = 1
+        ref_p = O.run_step(batch, pre, k_ref, v_ref, row_select=sel)
+        ref_d = O.run_step(batch, dec, k_ref, v_ref)
+        bt_p, pp_p = dev.tables_for(pre)
+        bt_d, pp_d = dev.tables_for(dec)
+        out_p = torch.zeros_like(pre.q, device=d)
+        out_d = torch.zeros_like(dec.q, device=d)
+        max_q = int((pre.cu_q_lens[1:] - pre.cu_q_lens[:-1]).max())
+        B.lazy_attn_mixed(dev.handle, dev.k_pool, dev.v_pool, q_prefill=pre.q.to(d), block_table_prefill=bt_p,
+                          page_logical_pos_prefill=pp_p, seq_lens_prefill=pre.seq_lens.to(d),
+                          cu_q_lens=pre.cu_q_lens.to(d), max_q_len=max_q, out_prefill=out_p, q_decode=dec.q.to(d),
+                          block_table_decode=bt_d, page_logical_pos_decode=pp_d, seq_lens_decode=dec.seq_lens.to(d),
+                          out_decode=out_d)
+        torch.cuda.synchronize()
+        compare(out_p, ref_p, "cfg5 mixed prefill", rows=rows)
+        compare(out_d, ref_d, "cfg5 mixed decode")
+    finally:
+        dev.close()
