@@ -566,9 +566,15 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 
     float alibi_slope = 0.f;                                   // kKmAlibi: this row's slope (log2 units), position
     int alibi_pos_q = 0;
+    float2 alibi_d2[kPageSize / 2];                            // slope * t for the in-page offsets, as pairs
     if (KM == kKmAlibi && valid) {
       alibi_slope = a.alibi[hk * group + g];
       alibi_pos_q = ppos[sq / kPageSize] + sq % kPageSize;
+    }
+    if (KM == kKmAlibi) {
+#pragma unroll
+      for (int x = 0; x < kPageSize / 2; ++x)
+        alibi_d2[x] = make_float2(alibi_slope * (float)(2 * x), alibi_slope * (float)(2 * x + 1));
     }
     float m_used = -INFINITY, l_run = 0.f;
     if (LAZY_PINGPONG && t == 1) ptx::named_bar_arrive(2, 256);          // tile 0 goes first
@@ -578,6 +584,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       if (LAZY_PINGPONG == 1) ptx::named_bar_sync(2 + t, 256);             // my turn
       ptx::tc_fence_after();
       if (row == 0) LAZY_TR(3 * t);
+      float abase[kPagesPerTile];                             // kKmAlibi: slope * (page start - m) of the tile's pages
       float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
       auto max_chunk = [&](int c) {                           // running row max over columns 32c .. 32c+31
 #pragma unroll
@@ -602,16 +609,18 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 #pragma unroll
         for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
         ptx::tmem_wait_ld();
-        if (KM == kKmAlibi) {                                 // S += slope * (n - m), n = page start + t
+        if (KM == kKmAlibi) {
+          // S += slope * (n - m), n = page start + t: only the in-page part slope * t is added to the elements
+          // (one packed add per pair); the per-page part abase[page] = slope * (page start - m) is folded into the
+          // page maxima below and into the constant of the exponential
           const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 3) * kPagesPerTile;
 #pragma unroll
           for (int pg = 0; pg < kPagesPerTile; ++pg) {
-            const float base = alibi_slope * (float)(pstart[pg] - alibi_pos_q);
+            abase[pg] = alibi_slope * (float)(pstart[pg] - alibi_pos_q);
 #pragma unroll
             for (int x = 0; x < kPageSize; x += 2) {
-              const float2 b = __ffma2_rn(make_float2(alibi_slope, alibi_slope),
-                                          make_float2((float)x, (float)(x + 1)), make_float2(base, base));
-              const float2 v = __fadd2_rn(make_float2(f32(sreg[16 * pg + x]), f32(sreg[16 * pg + x + 1])), b);
+              const float2 v = __fadd2_rn(make_float2(f32(sreg[16 * pg + x]), f32(sreg[16 * pg + x + 1])),
+                                          alibi_d2[x / 2]);
               sreg[16 * pg + x] = __float_as_uint(v.x);
               sreg[16 * pg + x + 1] = __float_as_uint(v.y);
             }
@@ -623,8 +632,21 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
           for (int x = 0; x < 128; ++x)
             if (x > lim_col) sreg[x] = 0xff800000u;           // -inf replaces the value (NaN-safe)
         }
+        if (KM == kKmAlibi) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) max_chunk(c);
+          for (int pg = 0; pg < kPagesPerTile; ++pg) {
+            float a0 = -INFINITY, a1 = -INFINITY;
+#pragma unroll
+            for (int x = 16 * pg; x < 16 * pg + 16; x += 4) {
+              a0 = fmaxf(fmaxf(a0, f32(sreg[x + 0])), f32(sreg[x + 1]));
+              a1 = fmaxf(fmaxf(a1, f32(sreg[x + 2])), f32(sreg[x + 3]));
+            }
+            mx0 = fmaxf(mx0, fmaxf(a0, a1) + abase[pg]);
+          }
+        } else {
+#pragma unroll
+          for (int c = 0; c < 4; ++c) max_chunk(c);
+        }
       }
       const float m_new = fmaxf(m_used, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
       if (j == 0) {
@@ -655,8 +677,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       for (int hf = 0; hf < 2; ++hf) {
 #pragma unroll
         for (int x = 32 * hf; x < 32 * hf + 32; x += 2) {
-          const float2 v0 = __fadd2_rn(make_float2(f32(sreg[2 * x]), f32(sreg[2 * x + 1])), negm);
-          const float2 v1 = __fadd2_rn(make_float2(f32(sreg[2 * x + 2]), f32(sreg[2 * x + 3])), negm);
+          const float2 nm = KM == kKmAlibi ? make_float2(abase[x >> 3] - m_used, abase[x >> 3] - m_used) : negm;
+          const float2 v0 = __fadd2_rn(make_float2(f32(sreg[2 * x]), f32(sreg[2 * x + 1])), nm);
+          const float2 v1 = __fadd2_rn(make_float2(f32(sreg[2 * x + 2]), f32(sreg[2 * x + 3])), nm);
           float2 p0, p1;
           if (LAZY_POLY_EVERY > 0 && (x / 2) % (LAZY_POLY_EVERY > 0 ? LAZY_POLY_EVERY : 1) == LAZY_POLY_EVERY - 1) {
             p0 = ex2_poly2(v0);
