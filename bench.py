@@ -364,6 +364,35 @@ def run_ablation(job, steps, warmup):
         torch.cuda.synchronize()
         res["alibi_shared_ms"] = float(np.mean([a.elapsed_time(b) for a, b in evs]))
         dv.close()
+    # f1 on the SHARED pool: every physical page stored rotated by its in-page offset only (page_stored_pos = 0 for
+    # all pages -- still reusable at any logical position); the kernels then owe one relative rotation per page
+    if True:
+        npg = int(dev.k_pool.shape[0])
+        allp = torch.arange(npg, dtype=torch.int32, device=d)
+        zeros = torch.zeros(npg, dtype=torch.int32, device=d)
+        k_loc = torch.empty_like(dev.k_pool)
+        B.lazy_materialize_pages(dev.handle, dev.k_pool, None, allp, zeros, True, k_loc, None, allp)
+        dv = DeviceBatch(batch, device=str(d), k_storage=B.LAZY_K_STORED_POS, page_stored_pos=zeros.cpu(),
+                         k_pool=k_loc, v_pool=dev.v_pool)
+
+        def attend_loc():
+            if st.kind == "decode":
+                B.lazy_attn_decode(dv.handle, rec["q"], dv.k_pool, dv.v_pool, rec["bt"], rec["pp"], rec["sl"], rec["out"])
+            else:
+                B.lazy_attn_prefill(dv.handle, rec["q"], dv.k_pool, dv.v_pool, rec["bt"], rec["pp"], rec["sl"],
+                                    rec["cu"], rec["max_q"], rec["out"])
+        for _ in range(warmup):
+            job.flush_l2(); attend_loc()
+        evs = []
+        for _ in range(steps):
+            job.flush_l2()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); attend_loc(); e1.record()
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+        res["page_local_shared_ms"] = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        dv.close()
+        del k_loc
     page_bytes = sh.num_kv_heads * P * sh.head_dim * 2
     res["rotation_overhead_pct"] = (res["unrotated_ms"] / res["absolute_ms"] - 1.0) * 100.0
     res["stored_pos_overhead_pct"] = (res["stored_pos_ms"] / res["absolute_ms"] - 1.0) * 100.0
