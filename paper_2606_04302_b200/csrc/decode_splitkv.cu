@@ -285,14 +285,18 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
 
     // Qhat = scale * R_angle q from one cos/sin row (a3/a4); `scale` is 1 when the K side carries the scale
     uint32_t qhat[2][C::NL];
+    float qf[2][C::NL][2];                          // q widened once per segment (it is re-rotated for every page)
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int w = 0; w < C::NL; ++w) { qf[h][w][0] = ptx::bf16_lo(qraw[h][w]); qf[h][w][1] = ptx::bf16_hi(qraw[h][w]); }
     auto rotate_q = [&](auto&& load_cs, float sgn, float scale) {
 #pragma unroll
       for (int w = 0; w < C::NL; ++w) {
         float4 c = load_cs(w);
         c.x *= scale; c.y *= scale;                 // (cos lo, cos hi, sin lo, sin hi) of the word's two pairs
         c.z *= sgn * scale; c.w *= sgn * scale;
-        float a_lo = ptx::bf16_lo(qraw[0][w]), a_hi = ptx::bf16_hi(qraw[0][w]);
-        float b_lo = ptx::bf16_lo(qraw[1][w]), b_hi = ptx::bf16_hi(qraw[1][w]);
+        const float a_lo = qf[0][w][0], a_hi = qf[0][w][1], b_lo = qf[1][w][0], b_hi = qf[1][w][1];
         qhat[0][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.z, a_hi * c.y - b_hi * c.w);
         qhat[1][w] = ptx::pack_bf16(a_lo * c.z + b_lo * c.x, a_hi * c.w + b_hi * c.y);
       }
