@@ -363,10 +363,13 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
 #pragma unroll
             for (int w = 0; w < C::NL; ++w) {
               const float4 c = ptx::lds128f(ctab_u32 + (rw * C::NL + w) * 512);
-              float a_lo = ptx::bf16_lo(kreg[0][rw][w]), a_hi = ptx::bf16_hi(kreg[0][rw][w]);
-              float b_lo = ptx::bf16_lo(kreg[1][rw][w]), b_hi = ptx::bf16_hi(kreg[1][rw][w]);
-              kreg[0][rw][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.z, a_hi * c.y - b_hi * c.w);
-              kreg[1][rw][w] = ptx::pack_bf16(a_lo * c.z + b_lo * c.x, a_hi * c.w + b_hi * c.y);
+              const float2 cc = make_float2(c.x, c.y), ss = make_float2(c.z, c.w);
+              const float2 x1 = make_float2(ptx::bf16_lo(kreg[0][rw][w]), ptx::bf16_hi(kreg[0][rw][w]));
+              const float2 x2 = make_float2(ptx::bf16_lo(kreg[1][rw][w]), ptx::bf16_hi(kreg[1][rw][w]));
+              const float2 y1 = __ffma2_rn(make_float2(-x2.x, -x2.y), ss, __fmul2_rn(x1, cc));
+              const float2 y2 = __ffma2_rn(x2, cc, __fmul2_rn(x1, ss));
+              kreg[0][rw][w] = ptx::pack_bf16(y1.x, y1.y);
+              kreg[1][rw][w] = ptx::pack_bf16(y2.x, y2.y);
             }
         }
         // ---- S = Khat Qhat^T : rows = tokens (g, g+8), cols = heads (2tq, 2tq+1)
