@@ -293,12 +293,15 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
     auto rotate_q = [&](auto&& load_cs, float sgn, float scale) {
 #pragma unroll
       for (int w = 0; w < C::NL; ++w) {
-        float4 c = load_cs(w);
-        c.x *= scale; c.y *= scale;                 // (cos lo, cos hi, sin lo, sin hi) of the word's two pairs
-        c.z *= sgn * scale; c.w *= sgn * scale;
-        const float a_lo = qf[0][w][0], a_hi = qf[0][w][1], b_lo = qf[1][w][0], b_hi = qf[1][w][1];
-        qhat[0][w] = ptx::pack_bf16(a_lo * c.x - b_lo * c.z, a_hi * c.y - b_hi * c.w);
-        qhat[1][w] = ptx::pack_bf16(a_lo * c.z + b_lo * c.x, a_hi * c.w + b_hi * c.y);
+        const float4 c = load_cs(w);                // (cos lo, cos hi, sin lo, sin hi) of the word's two pairs
+        const float2 cc = KM == LAZY_K_UNROTATED ? make_float2(c.x, c.y)      // the K side carries the scale
+                                                 : __fmul2_rn(make_float2(c.x, c.y), make_float2(scale, scale));
+        const float2 ss = __fmul2_rn(make_float2(c.z, c.w), make_float2(sgn * scale, sgn * scale));
+        const float2 x1 = make_float2(qf[0][w][0], qf[0][w][1]), x2 = make_float2(qf[1][w][0], qf[1][w][1]);
+        const float2 y1 = __ffma2_rn(make_float2(-x2.x, -x2.y), ss, __fmul2_rn(x1, cc));
+        const float2 y2 = __ffma2_rn(x2, cc, __fmul2_rn(x1, ss));
+        qhat[0][w] = ptx::pack_bf16(y1.x, y1.y);
+        qhat[1][w] = ptx::pack_bf16(y2.x, y2.y);
       }
     };
     float slope0 = 0.f, slope1 = 0.f;               // kKmAlibi: slopes (log2 units) of heads 2tq, 2tq+1
