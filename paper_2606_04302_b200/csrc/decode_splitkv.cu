@@ -30,8 +30,14 @@ namespace lazy {
 namespace {
 
 constexpr int kConsumerWarps = 8;
-constexpr int kDecodeThreads = (kConsumerWarps + 1) * 32;
+// 3 warpgroups: two of consumers, one holding the producer warp (+ 3 idle warps) so that setmaxnreg can move the
+// registers the producer does not need to the consumers (a 9-warp CTA is allocated registers as if it had 12 warps)
+constexpr int kDecodeThreads = 384;
+constexpr int kRegsConsumer = 224, kRegsProducer = 40;       // 2*128*224 + 128*40 = 62464 <= 65536
 constexpr int kMaxReqsSmem = 2048;
+#ifndef LAZY_CTAB_REGS
+#define LAZY_CTAB_REGS 1
+#endif
 
 template <int D, int HKV_CTA>
 struct DecodeCfg {
@@ -175,7 +181,9 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
     r0 = lo;
   }
 
-  if (warp == kConsumerWarps) {
+  if (warp >= kConsumerWarps) {
+    ptx::setmaxnreg_dec<kRegsProducer>();
+    if (warp > kConsumerWarps) return;              // idle warps of the producer's warpgroup
     // ================================= producer warp =====================================================
     const int pl = lane;                            // page lane within a stage (lanes < PPS are active)
     int r = r0, u = u_begin;
@@ -238,12 +246,23 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
   }
 
   // =================================== consumer warps ====================================================
+  ptx::setmaxnreg_inc<kRegsConsumer>();
   const int g = lane >> 2, tq = lane & 3;
   const int pl = warp / HKV_CTA;                    // page lane within a stage
   const int hl = warp % HKV_CTA;                    // kv head within the CTA's head group
   const int hk = hg * HKV_CTA + hl;
   const int group = sh.group;
   const uint32_t ctab_u32 = smem_base + C::OFF_CTAB + lane * 16;   // explicit ld.shared: generic LD costs a long scoreboard
+
+  // in-page rotation constants held in registers for the whole kernel (LAZY_CTAB_REGS token rows of the two a thread
+  // owns; the rest is re-read from shared memory for every page)
+  float4 ctab_r[LAZY_CTAB_REGS > 0 ? LAZY_CTAB_REGS : 1][C::NL];
+  if (KM == LAZY_K_UNROTATED) {
+#pragma unroll
+    for (int rw = 0; rw < LAZY_CTAB_REGS; ++rw)
+#pragma unroll
+      for (int w = 0; w < C::NL; ++w) ctab_r[rw][w] = ptx::lds128f(ctab_u32 + (rw * C::NL + w) * 512);
+  }
 
   int r = r0, u = u_begin, it = 0;
   while (u < u_end) {
@@ -365,7 +384,8 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
           for (int rw = 0; rw < 2; ++rw)
 #pragma unroll
             for (int w = 0; w < C::NL; ++w) {
-              const float4 c = ptx::lds128f(ctab_u32 + (rw * C::NL + w) * 512);
+              const float4 c = rw < LAZY_CTAB_REGS ? ctab_r[rw < LAZY_CTAB_REGS ? rw : 0][w]
+                                                   : ptx::lds128f(ctab_u32 + (rw * C::NL + w) * 512);
               const float2 cc = make_float2(c.x, c.y), ss = make_float2(c.z, c.w);
               const float2 x1 = make_float2(ptx::bf16_lo(kreg[0][rw][w]), ptx::bf16_hi(kreg[0][rw][w]));
               const float2 x2 = make_float2(ptx::bf16_lo(kreg[1][rw][w]), ptx::bf16_hi(kreg[1][rw][w]));
