@@ -19,26 +19,10 @@
 // TMEM (512 columns): S0 | S1 | O0 | O1, P_t aliases the first 64 columns of S_t.
 #include <climits>
 
-#include "lazy_internal.h"
-#include "ptx_util.cuh"
+#include "prefill_common.cuh"
 
 namespace lazy {
 namespace {
-
-constexpr int kPrefillThreads = 512;
-constexpr int kTileRows = 128;          // rows of a Q tile == keys of a KV tile
-constexpr int kHalfBytes = kTileRows * 128;   // one 64-column (128-byte) slab of a 128-row tile
-constexpr int kPagesPerTile = kTileRows / kPageSize;
-constexpr float kRescaleThreshold = 8.f;      // log2 units: O is rescaled only when the row max grew by > 2^8
-
-// Optional timeline probe (compile with -DLAZY_TRACE): one mid-grid CTA records clock64() at the hand-offs of 16
-// consecutive KV iterations into a device array read back by lazy_debug_trace().  Off in the product build.
-#ifdef LAZY_TRACE
-__device__ long long g_trace[16 * 16];
-#define LAZY_TR(slot) do { if (blockIdx.x == 300 && j >= 10 && j < 26) g_trace[(j - 10) * 16 + (slot)] = clock64(); } while (0)
-#else
-#define LAZY_TR(slot) do { } while (0)
-#endif
 
 template <int D>
 struct PrefillCfg {
@@ -52,15 +36,12 @@ struct PrefillCfg {
   static constexpr int OFF_V = 4 * TILE_BYTES;      // 2 stages
   static constexpr int OFF_CS = 6 * TILE_BYTES;     // 2 stages of 8 table rows (e^{i p0 theta_j} per page)
   static constexpr int OFF_BAR = OFF_CS + 2 * CS_STAGE_BYTES;
-  static constexpr int NUM_BARS = 24;
+  static constexpr int NUM_BARS = 26;
   static constexpr int OFF_TMEM = OFF_BAR + NUM_BARS * 8;
   static constexpr int OFF_SIGN = OFF_TMEM + 16;    // ring of 4 tiles x 8 pages: sign of the page's relative offset
                                                     // (LAZY_K_STORED_POS) or its logical start (ALiBi)
   static constexpr int SMEM_BYTES = OFF_SIGN + 4 * kPagesPerTile * 4 + 1024;   // + alignment slack
 };
-
-// register budgets per warpgroup (setmaxnreg; 2*128*184 + 128*104 + 128*40 = 65536)
-constexpr int kRegsSoftmax = 184, kRegsRotate = 104, kRegsMisc = 40;
 
 // barrier indices
 enum : int {
@@ -72,146 +53,13 @@ enum : int {
   B_VFULL = 10,   // +s   TMA -> MMA, fixer
   B_VEMPTY = 12,  // +s   MMA commit -> TMA
   B_VFIXED = 14,  //      fixer -> MMA (last tile only)
+  B_VLAST = 15,   //      TMA -> fixer: the last tile's V loads have been issued (one shot)
   B_SFULL = 16,   // +t   MMA commit -> softmax WG t
   B_PREADY = 18,  // +t   softmax WG t (4 warps) -> MMA
   B_OFULL = 20,   // +t   MMA commit -> softmax WG t (epilogue)
   B_PHALF = 22,   // +t   softmax WG t (4 warps) -> MMA: first half of P (keys 0..63) is in TMEM
+  B_PVH = 24,     // +t   MMA commit -> softmax WG t: PV over the first half of P has completed (slow path only)
 };
-
-struct PrefillArgs {
-  const int* block_table;
-  const int* page_pos;
-  const int* seq_lens;
-  const int* cu_q_lens;
-  __nv_bfloat16* out;
-  const float2* cs;
-  const int* stored_pos;   // LAZY_K_STORED_POS: [num_pages] position each physical page was stored at
-  const float* alibi;      // kKmAlibi: [Hq] slopes * log2(e)
-  const unsigned char* k_pool;   // raw pool pointers: only the L2 prefetch warp uses them (loads go through TMA)
-  const unsigned char* v_pool;
-  int num_reqs;
-  int q_interleaved;    // LAZY_ROPE_INTERLEAVED: q arrives with pairs (2j, 2j+1); de-interleaved while it is rotated
-  int mblocks;          // CTAs per (request, kv head)
-  int tokens_per_tile;  // 128 / group
-  Shape sh;
-};
-
-__device__ __forceinline__ void tma_load_4d(uint32_t dst, const void* tmap, uint32_t bar, int c0, int c1, int c2,
-                                            int c3) {
-  asm volatile(
-      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-      ::"r"(dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-      : "memory");
-}
-
-__device__ __forceinline__ float ex2(float x) {
-  float y;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-  return y;
-}
-__device__ __forceinline__ float f32(uint32_t x) { return __uint_as_float(x); }
-
-// 2^x for a PAIR of elements on the FMA pipe instead of the MUFU (ex2.approx runs at 16/clk/SM and is as loaded as
-// the tensor pipe in this kernel): Cody-Waite split x = floor(x) + f with a round-down magic-number
-// add, degree-3 polynomial for 2^f on [0,1) (max relative error 8.8e-5, far inside P's bf16 rounding 2^-9), exponent
-// inserted with one integer shift-add.  x is clamped to >= -126 (covers -inf of masked columns: result 2^-126 ~ 0).
-// Softmax ping-pong (FA3-style named-barrier hand-off between the two softmax warpgroups): 0 = free running,
-// 1 = the whole softmax of a tile is exclusive, 2 = only the exponential phase is exclusive.
-#ifndef LAZY_PINGPONG
-#define LAZY_PINGPONG 2
-#endif
-// L2 prefetch distance in KV tiles (warp 15; 0 = off: measured 2-4 % slower at 1-3 tiles)
-#ifndef LAZY_L2_AHEAD
-#define LAZY_L2_AHEAD 0
-#endif
-#ifndef LAZY_POLY_EVERY
-#define LAZY_POLY_EVERY 0   // every LAZY_POLY_EVERY-th group of 4 columns takes this path (0 = never: measured slower)
-#endif
-__device__ __forceinline__ float2 ex2_poly2(float2 v) {
-  v.x = fmaxf(v.x, -126.f);
-  v.y = fmaxf(v.y, -126.f);
-  unsigned long long vv, rr;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(vv) : "f"(v.x), "f"(v.y));
-  asm("add.rm.ftz.f32x2 %0, %1, %2;" : "=l"(rr) : "l"(vv), "l"(0x4b4000004b400000ull));   // + 1.5 * 2^23, round down
-  float2 xr;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(xr.x), "=f"(xr.y) : "l"(rr));
-  const float2 fl = __fadd2_rn(xr, make_float2(-12582912.f, -12582912.f));               // floor(x)
-  const float2 f = __ffma2_rn(fl, make_float2(-1.f, -1.f), v);                           // x - floor(x) in [0, 1)
-  float2 p = __ffma2_rn(make_float2(0.077119089663028717f, 0.077119089663028717f), f,
-                        make_float2(0.227564394474029541f, 0.227564394474029541f));
-  p = __ffma2_rn(p, f, make_float2(0.695146143436431885f, 0.695146143436431885f));
-  p = __ffma2_rn(p, f, make_float2(1.f, 1.f));
-  return make_float2(__int_as_float(__float_as_int(p.x) + (__float_as_int(xr.x) << 23)),
-                     __int_as_float(__float_as_int(p.y) + (__float_as_int(xr.y) << 23)));
-}
-
-// Index (in 16-byte units) inside a table row of the chunk holding (cos j, cos j+1, sin j, sin j+1), j = 8c + 2x
-// (row layout: cs_cos_index in ptx_util.cuh).
-template <int D>
-__device__ __forceinline__ int cs_f4_index(int c, int x) {
-  constexpr int JT = D / 8;
-  const int j0 = 8 * c;
-  return ((j0 % JT) / 2 + x) * 4 + j0 / JT;
-}
-// (cos, sin) of the 8 rotation pairs j = 8c .. 8c+7 from one table row in global memory / in shared memory.
-template <int D>
-__device__ __forceinline__ void load_cs8(const float2* __restrict__ cs_row, int c, float (&co)[8], float (&si)[8]) {
-  const float4* p = reinterpret_cast<const float4*>(cs_row);
-#pragma unroll
-  for (int x = 0; x < 4; ++x) {
-    float4 v = __ldg(p + cs_f4_index<D>(c, x));
-    co[2 * x] = v.x; co[2 * x + 1] = v.y; si[2 * x] = v.z; si[2 * x + 1] = v.w;
-  }
-}
-template <int D>
-__device__ __forceinline__ void load_cs8_smem(uint32_t row_addr, int c, float (&co)[8], float (&si)[8]) {
-#pragma unroll
-  for (int x = 0; x < 4; ++x) {
-    uint4 v = ptx::lds128(row_addr + 16 * cs_f4_index<D>(c, x));
-    co[2 * x] = f32(v.x); co[2 * x + 1] = f32(v.y); si[2 * x] = f32(v.z); si[2 * x + 1] = f32(v.w);
-  }
-}
-
-// byte offset of 16-byte chunk `ci` (8 dims: 8ci .. 8ci+7) of row `row` inside a 128-row, 128B-swizzled tile
-__device__ __forceinline__ uint32_t chunk_off(int row, int ci) {
-  return (ci >> 3) * kHalfBytes + row * 128 + (((ci & 7) ^ (row & 7)) << 4);
-}
-
-// rotate 8 pairs held as two 16-byte chunks (x1 = dims j, x2 = dims j + D/2) by (co, si), round to bf16
-__device__ __forceinline__ void rotate8(uint4& a, uint4& b, const float (&co)[8], const float (&si)[8]) {
-  uint32_t* aw = reinterpret_cast<uint32_t*>(&a);
-  uint32_t* bw = reinterpret_cast<uint32_t*>(&b);
-#pragma unroll
-  for (int w = 0; w < 4; ++w) {
-    float a0 = ptx::bf16_lo(aw[w]), a1 = ptx::bf16_hi(aw[w]);
-    float b0 = ptx::bf16_lo(bw[w]), b1 = ptx::bf16_hi(bw[w]);
-    aw[w] = ptx::pack_bf16(a0 * co[2 * w] - b0 * si[2 * w], a1 * co[2 * w + 1] - b1 * si[2 * w + 1]);
-    bw[w] = ptx::pack_bf16(a0 * si[2 * w] + b0 * co[2 * w], a1 * si[2 * w + 1] + b1 * co[2 * w + 1]);
-  }
-}
-
-// KM = lazy_config.k_storage.  LAZY_K_UNROTATED: K tile rotated by the absolute angle of its tokens.
-// LAZY_K_STORED_POS (Eq. 5): K tile rotated once by the page's relative offset
-// D = p0 - stored[page] (one table row per page, no in-page composition).  LAZY_K_ABSOLUTE: the K tile goes to
-// the MMA as it landed (the "rotation compiled out" arm of the overhead ablation, Fig. 5).  kKmAlibi
-// (PAPER.md L221): nothing is rotated; the softmax warpgroups add slope[head] * (n - m) to S, with the key position
-// n = page start + t taken from a small per-tile ring the producer fills.
-// Same rotation on packed f32x2 lanes (FMUL2 / FFMA2: half the FMA-pipe issue slots).  zc[w], zs[w] hold the
-// (cos, sin) of the two pairs whose x1 / x2 elements are the bf16 halves of word w of a / b.
-__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
-__device__ __forceinline__ void rotate8_packed(uint4& a, uint4& b, const float2 (&zc)[4], const float2 (&zs)[4]) {
-  uint32_t* aw = reinterpret_cast<uint32_t*>(&a);
-  uint32_t* bw = reinterpret_cast<uint32_t*>(&b);
-#pragma unroll
-  for (int w = 0; w < 4; ++w) {
-    const float2 x1 = make_float2(ptx::bf16_lo(aw[w]), ptx::bf16_hi(aw[w]));
-    const float2 x2 = make_float2(ptx::bf16_lo(bw[w]), ptx::bf16_hi(bw[w]));
-    const float2 y1 = __ffma2_rn(neg2(x2), zs[w], __fmul2_rn(x1, zc[w]));
-    const float2 y2 = __ffma2_rn(x2, zc[w], __fmul2_rn(x1, zs[w]));
-    aw[w] = ptx::pack_bf16(y1.x, y1.y);
-    bw[w] = ptx::pack_bf16(y2.x, y2.y);
-  }
-}
 
 template <int D, int KM>
 __global__ void __launch_bounds__(kPrefillThreads, 1)
@@ -233,7 +81,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
   const int group = sh.group, TPT = a.tokens_per_tile, TPC = 2 * TPT;
 
   // ---- work item: (request, kv head, block of 2*TPT query tokens) -------------------------------------------
-  const int mblk = blockIdx.x % a.mblocks;
+  // the m-blocks of one (request, kv head) stay adjacent (they share K/V through the L2); the last one, which sees
+  // the most keys under the causal mask, goes first
+  const int mblk = a.mblocks - 1 - blockIdx.x % a.mblocks;
   const int hk = (blockIdx.x / a.mblocks) % sh.Hkv;
   const int r = blockIdx.x / (a.mblocks * sh.Hkv);
   const int q_begin = a.cu_q_lens[r];
@@ -263,9 +113,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       ptx::mbar_init(bar(B_KEMPTY + x), 1); ptx::mbar_init(bar(B_VFULL + x), 1);
       ptx::mbar_init(bar(B_VEMPTY + x), 1); ptx::mbar_init(bar(B_SFULL + x), 1);
       ptx::mbar_init(bar(B_PREADY + x), 4); ptx::mbar_init(bar(B_OFULL + x), 1);
-      ptx::mbar_init(bar(B_PHALF + x), 4);
+      ptx::mbar_init(bar(B_PHALF + x), 4);  ptx::mbar_init(bar(B_PVH + x), 1);
     }
     ptx::mbar_init(bar(B_VFIXED), 1);
+    ptx::mbar_init(bar(B_VLAST), 1);
     ptx::fence_mbar_init();
   }
   if (warp == 13) {
@@ -337,6 +188,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         if (lane == 0) ptx::mbar_arrive_expect_tx(bar(B_VFULL + s), npv * C::NH * kPageSize * 128);
         __syncwarp();
         if (kvsel == 1 && lane_on && pg < npv) ptx::tma_load_2d(sV + dst, &tmap_v, bar(B_VFULL + s), half * 64, row0);
+        if (j == n_kv - 1) {
+          __syncwarp();
+          if (lane == 0) ptx::mbar_arrive(bar(B_VLAST));
+        }
       }
     } else if (warp == 13) {
       // ================================ MMA issuer ==========================================================
@@ -388,20 +243,18 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
           ptx::mbar_wait(bar(B_PHALF + t), j & 1);
           ptx::tc_fence_after();
           pv(t, s, j > 0, 0, kTileRows / 32);
+          commit(B_PVH + t);
           ptx::mbar_wait(bar(B_PREADY + t), j & 1);
           ptx::tc_fence_after();
-          if (leader) LAZY_TR(8 + 3 * t);
           pv(t, s, 1u, kTileRows / 32, kTileRows / 16);
           if (t == 1) commit(B_VEMPTY + s);
           if (j + 1 < nkv) {
             if (t == 0) {
               ptx::mbar_wait(bar(B_KREADY + (s ^ 1)), ((j + 1) >> 1) & 1);
               ptx::tc_fence_after();
-              if (leader) LAZY_TR(9);
             }
             qk(t, s ^ 1);
             commit(B_SFULL + t);
-            if (leader) LAZY_TR(10 + 3 * t);
             if (t == 1) commit(B_KEMPTY + (s ^ 1));
           } else {
             commit(B_OFULL + t);
@@ -411,8 +264,12 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       __syncwarp();
     } else if (warp == 14) {
       // ================================ V tail fixer ========================================================
-      for (int j = 0; j < n_kv; ++j) ptx::mbar_wait_sleep(bar(B_VFULL + (j & 1)), (j >> 1) & 1);
+      // The fixer is not part of the V ring's full/empty hand-shake, so it must not walk the ring's phases (a lagging
+      // observer would alias parities).  It sleeps on a one-shot barrier until the producer has ISSUED the last tile's
+      // V loads: from then on VFULL[s] is in that tile's phase and cannot advance (the MMA warp waits for VFIXED).
       const int jl = n_kv - 1;
+      ptx::mbar_wait_sleep(bar(B_VLAST), 0);
+      ptx::mbar_wait_sleep(bar(B_VFULL + (jl & 1)), (jl >> 1) & 1);
       const int rows_valid = min(kTileRows, L - jl * kTileRows);
       if (rows_valid < kTileRows) {
         const int per_half = (kTileRows - rows_valid) * 8;          // 16-byte chunks to clear per column slab
@@ -423,40 +280,29 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       ptx::fence_proxy_async();
       __syncwarp();
       if (lane == 0) ptx::mbar_arrive(bar(B_VFIXED));
-    } else if (LAZY_L2_AHEAD > 0) {
-      // ================================ L2 prefetcher (warp 15) =============================================
-      // touches the K and V pages of tile j + LAZY_L2_AHEAD with plain prefetch instructions (LSU path, not the
-      // TMA unit), throttled by the arrival of tile j, so that the TMA gather of a freed stage hits the L2
-      const int pgi = lane & 7, part = lane >> 3;   // lane -> (page of the tile, K lo / K hi / V lo / V hi half)
-      constexpr int kHalfPage = kPageSize * D;      // bytes of half a (page, head) tile
-      for (int j = 0; j < n_kv; ++j) {
-        const int idx = (j + LAZY_L2_AHEAD) * kPagesPerTile + pgi;
-        if (j + LAZY_L2_AHEAD < n_kv && idx < num_pages) {
-          const unsigned char* p = (part < 2 ? a.k_pool : a.v_pool) +
-                                   ((size_t)bt[idx] * sh.Hkv + hk) * (2 * kHalfPage) + (part & 1) * kHalfPage;
-#pragma unroll
-          for (int l = 0; l < kHalfPage / 128; ++l)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(p + 128 * l));
-        }
-        ptx::mbar_wait_sleep(bar(B_KFULL + (j & 1)), (j >> 1) & 1);
-      }
     }
   } else if (warp >= 8) {
     // ================================ K-rotate warpgroup ======================================================
+    // thread = (page of the tile, group of CPR consecutive tokens, chunk pair c = 8 rotation pairs): it reads the
+    // page's table row w = e^{i p0 theta_j} ONCE, composes it with the group's first in-page offset and then walks
+    // its tokens with the one-step recurrence z <- z * e^{i theta_j} (at most 7 fp32 complex products away from a
+    // table value built in fp64: ~4e-7 relative, PAPER.md L455's drift concern does not arise).  This takes the
+    // per-token table reads (64 KB of LDS per tile, 2-way bank-conflicted) out of the shared-memory pipe, which the
+    // tensor cores' operand fetches already load to ~40 % (profiles/r2_prefill_smem_attribution.md).
     ptx::setmaxnreg_dec<kRegsRotate>();
-    constexpr int TPP = 16 * C::CPR;                // threads per page
-    constexpr int PPP = 128 / TPP;                  // pages per pass
-    constexpr int PASSES = kPagesPerTile / PPP;
+    constexpr int TOK = C::CPR;                     // tokens per thread (16 threads serve a page)
     const int wtid = tid - 256;
-    const int pp_ = wtid / TPP, t = (wtid % TPP) / C::CPR, c = wtid % C::CPR;
-    float2 uc[4], us[4];                            // e^{i t theta_j}: in-page offset, fixed per thread
+    const int i = wtid >> 4;                        // page of the tile
+    const int t0 = ((wtid & 15) / C::CPR) * TOK, c = wtid % C::CPR;
+    float2 u0c[4], u0s[4], u1c[4], u1s[4];          // e^{i t0 theta_j}, e^{i theta_j} for this thread's 8 pairs
     if (KM == LAZY_K_UNROTATED) {
-      const float4* urow = reinterpret_cast<const float4*>(a.cs + (size_t)t * (D / 2));
+      const float4* r0 = reinterpret_cast<const float4*>(a.cs + (size_t)t0 * (D / 2));
+      const float4* r1 = reinterpret_cast<const float4*>(a.cs + (size_t)1 * (D / 2));
 #pragma unroll
       for (int x = 0; x < 4; ++x) {
-        const float4 v = __ldg(urow + cs_f4_index<D>(c, x));
-        uc[x] = make_float2(v.x, v.y);
-        us[x] = make_float2(v.z, v.w);
+        const float4 v0 = __ldg(r0 + cs_f4_index<D>(c, x)), v1 = __ldg(r1 + cs_f4_index<D>(c, x));
+        u0c[x] = make_float2(v0.x, v0.y); u0s[x] = make_float2(v0.z, v0.w);
+        u1c[x] = make_float2(v1.x, v1.y); u1s[x] = make_float2(v1.z, v1.w);
       }
     }
     const int* s_sign = reinterpret_cast<const int*>(smem + C::OFF_SIGN);
@@ -466,41 +312,53 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       const uint32_t kb = sK + s * C::TILE_BYTES;
       const uint32_t cb = sCS + s * C::CS_STAGE_BYTES;
       ptx::mbar_wait(bar(B_KFULL + s), (j >> 1) & 1);
-      if (wtid == 0) LAZY_TR(6);
+      if (!kNoRotate && i < npv) {
+        float2 zc[4], zs[4];                        // e^{i (p0+t) theta_j}, or e^{i Delta theta_j} of the page
 #pragma unroll
-      for (int ps = 0; ps < PASSES; ++ps) {
-        const int i = ps * PPP + pp_;
-        if (!kNoRotate && i < npv) {
-          float2 zc[4], zs[4];                      // e^{i (p0+t) theta_j}, or e^{i Delta theta_j} of the page
-          const int row = i * kPageSize + t;
-          const uint32_t pa = kb + chunk_off(row, c), pb = kb + chunk_off(row, c + C::CPR);
+        for (int x = 0; x < 4; ++x) {
+          const uint4 v = ptx::lds128(cb + i * C::CS_ROW_BYTES + 16 * cs_f4_index<D>(c, x));
+          zc[x] = make_float2(f32(v.x), f32(v.y));
+          zs[x] = make_float2(f32(v.z), f32(v.w));
+        }
+        if (KM == LAZY_K_UNROTATED) {               // first token of the group: z = w * u0
 #pragma unroll
           for (int x = 0; x < 4; ++x) {
-            const uint4 v = ptx::lds128(cb + i * C::CS_ROW_BYTES + 16 * cs_f4_index<D>(c, x));
-            zc[x] = make_float2(f32(v.x), f32(v.y));
-            zs[x] = make_float2(f32(v.z), f32(v.w));
+            const float2 wc = zc[x], ws = zs[x];
+            zc[x] = __ffma2_rn(neg2(ws), u0s[x], __fmul2_rn(wc, u0c[x]));
+            zs[x] = __ffma2_rn(wc, u0s[x], __fmul2_rn(ws, u0c[x]));
           }
-          uint4 va = ptx::lds128(pa), vb = ptx::lds128(pb);
-          if (KM == LAZY_K_UNROTATED) {             // compose with the in-page offset: z = w * u
+        } else {                                    // one relative rotation for the whole page (may be negative)
+          const float sgn = (float)s_sign[(j & 3) * kPagesPerTile + i];
 #pragma unroll
-            for (int x = 0; x < 4; ++x) {
-              const float2 wc = zc[x], ws = zs[x];
-              zc[x] = __ffma2_rn(neg2(ws), us[x], __fmul2_rn(wc, uc[x]));
-              zs[x] = __ffma2_rn(wc, us[x], __fmul2_rn(ws, uc[x]));
+          for (int x = 0; x < 4; ++x) zs[x] = __fmul2_rn(zs[x], make_float2(sgn, sgn));
+        }
+        const int row0 = i * kPageSize + t0;
+#pragma unroll
+        for (int tb = 0; tb < TOK; tb += 4) {
+          uint4 va[4], vb[4];
+#pragma unroll
+          for (int tt = 0; tt < 4; ++tt) {
+            va[tt] = ptx::lds128(kb + chunk_off(row0 + tb + tt, c));
+            vb[tt] = ptx::lds128(kb + chunk_off(row0 + tb + tt, c + C::CPR));
+          }
+#pragma unroll
+          for (int tt = 0; tt < 4; ++tt) {
+            rotate8_packed(va[tt], vb[tt], zc, zs);
+            ptx::sts128(kb + chunk_off(row0 + tb + tt, c), va[tt]);
+            ptx::sts128(kb + chunk_off(row0 + tb + tt, c + C::CPR), vb[tt]);
+            if (KM == LAZY_K_UNROTATED && tb + tt + 1 < TOK) {      // next token: z <- z * e^{i theta_j}
+#pragma unroll
+              for (int x = 0; x < 4; ++x) {
+                const float2 wc = zc[x], ws = zs[x];
+                zc[x] = __ffma2_rn(neg2(ws), u1s[x], __fmul2_rn(wc, u1c[x]));
+                zs[x] = __ffma2_rn(wc, u1s[x], __fmul2_rn(ws, u1c[x]));
+              }
             }
-          } else {                                  // one relative rotation for the whole page (may be negative)
-            const float sgn = (float)s_sign[(j & 3) * kPagesPerTile + i];
-#pragma unroll
-            for (int x = 0; x < 4; ++x) zs[x] = __fmul2_rn(zs[x], make_float2(sgn, sgn));
           }
-          rotate8_packed(va, vb, zc, zs);
-          ptx::sts128(pa, va);
-          ptx::sts128(pb, vb);
         }
       }
       ptx::fence_proxy_async();
       __syncwarp();
-      if (wtid == 0) LAZY_TR(7);
       if (lane == 0) ptx::mbar_arrive(bar(B_KREADY + s));
     }
   } else {
@@ -576,86 +434,108 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       for (int x = 0; x < kPageSize / 2; ++x)
         alibi_d2[x] = make_float2(alibi_slope * (float)(2 * x), alibi_slope * (float)(2 * x + 1));
     }
+    // Online softmax with OPTIMISTIC exponentials.  The output is O / l whatever reference value m the exponentials
+    // use (floating point keeps relative precision at any scale), so after the first tile -- whose exact row max
+    // becomes m_used -- a tile's P = 2^(S - m_used) is computed straight away with the m_used already at hand, and
+    // the tile's own maximum is taken alongside (it has no consumer on the critical path).  Only if a score
+    // exceeds m_used by more than kDanger (P > 2^20: never with sane inputs after the first 128 keys) the warp takes
+    // the slow path: it brings O and l to the new maximum and recomputes that half of P.  This takes the
+    // load-then-max phase (~600 cycles per tile) out of the softmax -> PV -> QK -> softmax chain that sets the
+    // kernel's pace.
+    constexpr float kDanger = 20.f;
     float m_used = -INFINITY, l_run = 0.f;
-    if (LAZY_PINGPONG && t == 1) ptx::named_bar_arrive(2, 256);          // tile 0 goes first
+    if (t == 1) ptx::named_bar_arrive(2, 256);                            // tile 0 goes first
     for (int j = 0; j < n_kv; ++j) {
-      uint32_t sreg[128];                                     // this row of S (fp32 bits), later packed P
+      uint32_t sreg[128];                                     // this row of S (fp32 bits); P is packed over it in place
       ptx::mbar_wait(bar(B_SFULL + t), j & 1);
-      if (LAZY_PINGPONG == 1) ptx::named_bar_sync(2 + t, 256);             // my turn
       ptx::tc_fence_after();
-      if (row == 0) LAZY_TR(3 * t);
       float abase[kPagesPerTile];                             // kKmAlibi: slope * (page start - m) of the tile's pages
-      float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
-      auto max_chunk = [&](int c) {                           // running row max over columns 32c .. 32c+31
 #pragma unroll
-        for (int x = 32 * c; x < 32 * c + 32; x += 8) {
-          mx0 = fmaxf(fmaxf(mx0, f32(sreg[x + 0])), f32(sreg[x + 1]));
-          mx1 = fmaxf(fmaxf(mx1, f32(sreg[x + 2])), f32(sreg[x + 3]));
-          mx2 = fmaxf(fmaxf(mx2, f32(sreg[x + 4])), f32(sreg[x + 5]));
-          mx3 = fmaxf(fmaxf(mx3, f32(sreg[x + 6])), f32(sreg[x + 7]));
-        }
-      };
+      for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
+      if (KM == kKmAlibi) {
+        const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 3) * kPagesPerTile;
+#pragma unroll
+        for (int pg = 0; pg < kPagesPerTile; ++pg) abase[pg] = alibi_slope * (float)(pstart[pg] - alibi_pos_q);
+      }
       const bool edge = j * kTileRows + kTileRows - 1 > lim_min;   // tile touches the causal edge / the tail: rare
-      if (KM != kKmAlibi && !edge) {
-        // interior tile: the TMEM load of chunk c+1 is in flight while the max of chunk c is taken
-        ptx::tmem_ld32(tS, sreg);
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          ptx::tmem_wait_ld();
-          if (c + 1 < 4) ptx::tmem_ld32(tS + (c + 1) * 32, sreg + (c + 1) * 32);
-          max_chunk(c);
-        }
-      } else {
-#pragma unroll
-        for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
-        ptx::tmem_wait_ld();
+      const int lim_col = lim_row - j * kTileRows;            // column visible iff col <= lim_col
+      // columns 64hf .. 64hf+63 as they enter the softmax: ALiBi's in-page part slope * t added (S += slope * (n - m),
+      // n = page start + t; the per-page part abase[] is folded into the maxima and into the exponential's constant),
+      // masked columns replaced by -inf (never multiplied: poisoned bytes past the tail may be NaN)
+      auto prep_half = [&](int hf) {
         if (KM == kKmAlibi) {
-          // S += slope * (n - m), n = page start + t: only the in-page part slope * t is added to the elements
-          // (one packed add per pair); the per-page part abase[page] = slope * (page start - m) is folded into the
-          // page maxima below and into the constant of the exponential
-          const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 3) * kPagesPerTile;
 #pragma unroll
-          for (int pg = 0; pg < kPagesPerTile; ++pg) {
-            abase[pg] = alibi_slope * (float)(pstart[pg] - alibi_pos_q);
-#pragma unroll
-            for (int x = 0; x < kPageSize; x += 2) {
-              const float2 v = __fadd2_rn(make_float2(f32(sreg[16 * pg + x]), f32(sreg[16 * pg + x + 1])),
-                                          alibi_d2[x / 2]);
-              sreg[16 * pg + x] = __float_as_uint(v.x);
-              sreg[16 * pg + x + 1] = __float_as_uint(v.y);
-            }
+          for (int x = 64 * hf; x < 64 * hf + 64; x += 2) {
+            const float2 v = __fadd2_rn(make_float2(f32(sreg[x]), f32(sreg[x + 1])), alibi_d2[(x & 15) >> 1]);
+            sreg[x] = __float_as_uint(v.x);
+            sreg[x + 1] = __float_as_uint(v.y);
           }
         }
         if (edge) {
-          const int lim_col = lim_row - j * kTileRows;        // column visible iff col <= lim_col
 #pragma unroll
-          for (int x = 0; x < 128; ++x)
-            if (x > lim_col) sreg[x] = 0xff800000u;           // -inf replaces the value (NaN-safe)
+          for (int x = 64 * hf; x < 64 * hf + 64; ++x)
+            if (x > lim_col) sreg[x] = 0xff800000u;
         }
-        if (KM == kKmAlibi) {
+      };
+      ptx::tmem_wait_ld();
+      prep_half(0);
+      prep_half(1);
+      if (j == 0) {                                           // first tile: the exact row max (column 0 is always visible)
+        float r0 = -INFINITY, r1 = -INFINITY;
 #pragma unroll
-          for (int pg = 0; pg < kPagesPerTile; ++pg) {
-            float a0 = -INFINITY, a1 = -INFINITY;
+        for (int pg = 0; pg < kPagesPerTile; ++pg) {
+          float a0 = -INFINITY, a1 = -INFINITY;
 #pragma unroll
-            for (int x = 16 * pg; x < 16 * pg + 16; x += 4) {
-              a0 = fmaxf(fmaxf(a0, f32(sreg[x + 0])), f32(sreg[x + 1]));
-              a1 = fmaxf(fmaxf(a1, f32(sreg[x + 2])), f32(sreg[x + 3]));
-            }
-            mx0 = fmaxf(mx0, fmaxf(a0, a1) + abase[pg]);
+          for (int x = 16 * pg; x < 16 * pg + 16; x += 4) {
+            a0 = fmaxf(fmaxf(a0, f32(sreg[x + 0])), f32(sreg[x + 1]));
+            a1 = fmaxf(fmaxf(a1, f32(sreg[x + 2])), f32(sreg[x + 3]));
           }
-        } else {
-#pragma unroll
-          for (int c = 0; c < 4; ++c) max_chunk(c);
+          if (KM == kKmAlibi) r0 = fmaxf(r0, fmaxf(a0, a1) + abase[pg]);
+          else { r0 = fmaxf(r0, a0); r1 = fmaxf(r1, a1); }
         }
+        m_used = fmaxf(r0, r1);
       }
-      const float m_new = fmaxf(m_used, fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)));
-      if (j == 0) {
-        m_used = m_new;
-      } else {
-        const bool grow = m_new > m_used + kRescaleThreshold;
-        if (__any_sync(0xffffffffu, grow)) {                  // PV(j-1) has completed: S(j) was committed after it
-          const float f = grow ? ex2(m_used - m_new) : 1.f;
-          if (grow) m_used = m_new;
+      ptx::named_bar_sync(2 + t, 256);                                   // my turn on the MUFU
+#pragma unroll
+      for (int hf = 0; hf < 2; ++hf) {
+        // P = 2^(S - m_used) for this half, packed in place; the half's own maximum is taken alongside
+        const float2 negm = make_float2(-m_used, -m_used);
+        float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
+        float mx0 = -INFINITY, mx1 = -INFINITY, mxa = -INFINITY;
+#pragma unroll
+        for (int x = 32 * hf; x < 32 * hf + 32; x += 2) {
+          const float s0 = f32(sreg[2 * x]), s1 = f32(sreg[2 * x + 1]), s2 = f32(sreg[2 * x + 2]), s3 = f32(sreg[2 * x + 3]);
+          const float2 nm = KM == kKmAlibi ? make_float2(abase[x >> 3] - m_used, abase[x >> 3] - m_used) : negm;
+          const float2 v0 = __fadd2_rn(make_float2(s0, s1), nm);
+          const float2 v1 = __fadd2_rn(make_float2(s2, s3), nm);
+          mx0 = fmaxf(fmaxf(mx0, s0), s1);
+          mx1 = fmaxf(fmaxf(mx1, s2), s3);
+          const float2 p0 = make_float2(ex2(v0.x), ex2(v0.y));
+          const float2 p1 = make_float2(ex2(v1.x), ex2(v1.y));
+          sum0 = __fadd2_rn(sum0, p0);
+          sum1 = __fadd2_rn(sum1, p1);
+          sreg[x] = ptx::pack_bf16(p0.x, p0.y);
+          sreg[x + 1] = ptx::pack_bf16(p1.x, p1.y);
+          if (KM == kKmAlibi && (x & 7) == 6) {               // end of a page: fold its per-page bias into the maximum
+            mxa = fmaxf(mxa, fmaxf(mx0, mx1) + abase[x >> 3]);
+            mx0 = -INFINITY; mx1 = -INFINITY;
+          }
+        }
+        const float mxh = KM == kKmAlibi ? mxa : fmaxf(mx0, mx1);
+        float hsum = (sum0.x + sum0.y) + (sum1.x + sum1.y);
+        const bool slow = j > 0 && __any_sync(0xffffffffu, mxh > m_used + kDanger);
+        if (slow) {
+          // Slow path (a score beyond 2^kDanger of m_used).  O and l -- which hold the tiles < j, and keys 0..63 of
+          // this tile once the first half of PV has completed -- move to the new maximum; then this half of P is
+          // rebuilt 16 columns at a time straight from S in TMEM (P half 0 sits in columns 0..31, so the S columns
+          // still to be read are intact) and written back to TMEM from here.
+          if (hf == 1) {
+            ptx::mbar_wait(bar(B_PVH + t), j & 1);
+            ptx::tc_fence_after();
+          }
+          const float m_new = fmaxf(m_used, mxh);
+          const float f = ex2(m_used - m_new);
+          m_used = m_new;
           l_run *= f;
 #pragma unroll 1
           for (int c = 0; c < D / 16; ++c) {
@@ -667,45 +547,40 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
             ptx::tmem_st16(tO + c * 16, rr);
           }
           ptx::tmem_wait_st();
-        }
-      }
-      if (row == 0) LAZY_TR(3 * t + 1);
-      if (LAZY_PINGPONG == 2) ptx::named_bar_sync(2 + t, 256);             // my turn on the MUFU
-      const float2 negm = make_float2(-m_used, -m_used);
-      float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
+          hsum = 0.f;
+          const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 3) * kPagesPerTile;
+#pragma unroll 1
+          for (int c = 0; c < 4; ++c) {
+            const int col0 = 64 * hf + 16 * c;                // one page of the tile
+            uint32_t rr[16], pk[8];
+            ptx::tmem_ld16(tS + col0, rr);
+            ptx::tmem_wait_ld();
+            float off = -m_used;
+            if (KM == kKmAlibi) off += alibi_slope * (float)(pstart[col0 >> 4] - alibi_pos_q);
 #pragma unroll
-      for (int hf = 0; hf < 2; ++hf) {
-#pragma unroll
-        for (int x = 32 * hf; x < 32 * hf + 32; x += 2) {
-          const float2 nm = KM == kKmAlibi ? make_float2(abase[x >> 3] - m_used, abase[x >> 3] - m_used) : negm;
-          const float2 v0 = __fadd2_rn(make_float2(f32(sreg[2 * x]), f32(sreg[2 * x + 1])), nm);
-          const float2 v1 = __fadd2_rn(make_float2(f32(sreg[2 * x + 2]), f32(sreg[2 * x + 3])), nm);
-          float2 p0, p1;
-          if (LAZY_POLY_EVERY > 0 && (x / 2) % (LAZY_POLY_EVERY > 0 ? LAZY_POLY_EVERY : 1) == LAZY_POLY_EVERY - 1) {
-            p0 = ex2_poly2(v0);
-            p1 = ex2_poly2(v1);
-          } else {
-            p0 = make_float2(ex2(v0.x), ex2(v0.y));
-            p1 = make_float2(ex2(v1.x), ex2(v1.y));
+            for (int x = 0; x < 16; x += 2) {
+              float v0 = f32(rr[x]) + off, v1 = f32(rr[x + 1]) + off;
+              if (KM == kKmAlibi) { v0 += alibi_slope * (float)x; v1 += alibi_slope * (float)(x + 1); }
+              if (col0 + x > lim_col) v0 = -INFINITY;         // lim_col >= 127 on interior tiles
+              if (col0 + x + 1 > lim_col) v1 = -INFINITY;
+              const float q0 = ex2(v0), q1 = ex2(v1);
+              hsum += q0 + q1;
+              pk[x >> 1] = ptx::pack_bf16(q0, q1);
+            }
+            ptx::tmem_st8(tS + (col0 >> 1), pk);
           }
-          sum0 = __fadd2_rn(sum0, p0);
-          sum1 = __fadd2_rn(sum1, p1);
-          sreg[x] = ptx::pack_bf16(p0.x, p0.y);
-          sreg[x + 1] = ptx::pack_bf16(p1.x, p1.y);
         }
-        if (hf == 1 && LAZY_PINGPONG) ptx::named_bar_arrive(2 + (t ^ 1), 256);   // the other tile's turn
-        ptx::tmem_st32(tS + 32 * hf, sreg + 32 * hf);         // P (bf16 pairs) over the first 64 columns of S
+        l_run += hsum;
+        if (hf == 1) ptx::named_bar_arrive(2 + (t ^ 1), 256);                 // the other tile's turn
+        if (!slow) ptx::tmem_st32(tS + 32 * hf, sreg + 32 * hf);   // P (bf16 pairs) over the first 64 columns of S
         ptx::tmem_wait_st();
         ptx::tc_fence_before();
         __syncwarp();
-        if (hf == 0 && lane == 0) ptx::mbar_arrive(bar(B_PHALF + t));
+        if (lane == 0) ptx::mbar_arrive(bar((hf == 0 ? B_PHALF : B_PREADY) + t));
       }
-      l_run += (sum0.x + sum0.y) + (sum1.x + sum1.y);
-      if (row == 0) LAZY_TR(3 * t + 2);
-      if (lane == 0) ptx::mbar_arrive(bar(B_PREADY + t));
     }
 
-    if (LAZY_PINGPONG && t == 0) ptx::named_bar_sync(2, 256);            // consume tile 1's last hand-off
+    if (t == 0) ptx::named_bar_sync(2, 256);                              // consume tile 1's last hand-off
     // ---- epilogue (a9): normalise, round to bf16, store the row -------------------------------------------
     ptx::mbar_wait(bar(B_OFULL + t), 0);
     ptx::tc_fence_after();
@@ -754,12 +629,6 @@ static int launch_prefill_t(const lazy_handle* h, const PrefillArgs& args, int g
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
 
-#ifdef LAZY_TRACE
-extern "C" int lazy_debug_trace(long long* host_out) {
-  return cudaMemcpyFromSymbol(host_out, g_trace, sizeof(long long) * 256) == cudaSuccess ? 0 : -1;
-}
-#endif
-
 int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                    const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                    const int32_t* cu_q_lens, int num_reqs, int total_q, int max_q_len, void* out,
@@ -790,8 +659,6 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   a.cs = h->ws.cs;
   a.stored_pos = h->page_stored_pos;
   a.alibi = h->ws.alibi;
-  a.k_pool = static_cast<const unsigned char*>(k_cache);
-  a.v_pool = static_cast<const unsigned char*>(v_cache);
   a.num_reqs = num_reqs;
   a.q_interleaved = c.rope_style == LAZY_ROPE_INTERLEAVED;
   a.mblocks = (max_q_len + 2 * tpt - 1) / (2 * tpt);
