@@ -99,6 +99,8 @@ typedef struct lazy_config {
 
 /* flags: debugging aids, never set by bench.py */
 #define LAZY_FLAG_ROWWISE_KERNELS 1  /* run the simple one-row-per-CTA CUDA kernels for prefill and decode */
+#define LAZY_FLAG_PREFILL_ONE_CTA 2  /* head_dim 128: run prefill on single CTAs (prefill_umma.cu) instead of CTA
+                                      pairs (prefill_umma2.cu); the A/B arm of DESIGN.md 6.2 */
 
 #define LAZY_OK               0
 #define LAZY_ERR_INVALID     -1  /* null / misaligned pointer, negative count, num_reqs > max_reqs ...     */

@@ -610,13 +610,10 @@ bool encode_q_tmap(void* out_map, const void* q, int total_q, int Hq, int Hkv, i
 template <int D, int HKV_CTA, int KM>
 static int launch_decode_km(lazy_handle* h, const DecodeArgs& args, int grid_x, int grid_y, cudaStream_t stream) {
   using C = DecodeCfg<D, HKV_CTA>;
-  static bool attr_set = false;
   auto kern = decode_splitkv_kernel<D, HKV_CTA, KM>;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
-      return LAZY_ERR_CUDA;
-    attr_set = true;
-  }
+  // per launch: the attribute is per device, and a process may hold handles on several devices
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
+    return LAZY_ERR_CUDA;
   const CUtensorMap* mk = reinterpret_cast<const CUtensorMap*>(h->tmap_k);
   const CUtensorMap* mv = reinterpret_cast<const CUtensorMap*>(h->tmap_v);
   kern<<<dim3(grid_x, grid_y), kDecodeThreads, C::SMEM_BYTES, stream>>>(*mk, *mv, args);

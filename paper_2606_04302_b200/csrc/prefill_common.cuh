@@ -6,15 +6,6 @@
 #include "ptx_util.cuh"
 
 namespace lazy {
-namespace {
-
-constexpr int kPrefillThreads = 512;
-constexpr int kTileRows = 128;          // rows of a Q tile == keys of a KV tile
-constexpr int kHalfBytes = kTileRows * 128;   // one 64-column (128-byte) slab of a 128-row tile
-constexpr int kPagesPerTile = kTileRows / kPageSize;
-
-// register budgets per warpgroup (setmaxnreg; 2*128*184 + 128*104 + 128*40 = 65536)
-constexpr int kRegsSoftmax = 184, kRegsRotate = 104, kRegsMisc = 40;
 
 struct PrefillArgs {
   const int* block_table;
@@ -31,6 +22,20 @@ struct PrefillArgs {
   int tokens_per_tile;  // 128 / group
   Shape sh;
 };
+
+// prefill_umma2.cu: head_dim 128 on CTA pairs; `a.mblocks` counts pairs per (request, kv head), `grid` = 2 CTAs per pair
+int launch_prefill_pair(const lazy_handle* h, const PrefillArgs& a, int km, int grid, cudaStream_t stream);
+
+namespace {
+
+constexpr int kPrefillThreads = 512;
+constexpr int kTileRows = 128;          // rows of a Q tile == keys of a KV tile
+constexpr int kHalfBytes = kTileRows * 128;   // one 64-column (128-byte) slab of a 128-row tile
+constexpr int kPagesPerTile = kTileRows / kPageSize;
+
+// register budgets per warpgroup (setmaxnreg; 2*128*184 + 128*104 + 128*40 = 65536)
+constexpr int kRegsSoftmax = 184, kRegsRotate = 104, kRegsMisc = 40;
+
 
 __device__ __forceinline__ void tma_load_4d(uint32_t dst, const void* tmap, uint32_t bar, int c0, int c1, int c2,
                                             int c3) {

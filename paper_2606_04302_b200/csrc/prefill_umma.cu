@@ -615,13 +615,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 template <int D, int KM>
 static int launch_prefill_t(const lazy_handle* h, const PrefillArgs& args, int grid, cudaStream_t stream) {
   using C = PrefillCfg<D>;
-  static bool attr_set = false;
   auto kern = prefill_umma_kernel<D, KM>;
-  if (!attr_set) {
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
-      return LAZY_ERR_CUDA;
-    attr_set = true;
-  }
+  // per launch: the attribute is per device, and a process may hold handles on several devices
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
+    return LAZY_ERR_CUDA;
   const CUtensorMap* mq = reinterpret_cast<const CUtensorMap*>(h->tmap_pq);
   const CUtensorMap* mk = reinterpret_cast<const CUtensorMap*>(h->tmap_pk);
   const CUtensorMap* mv = reinterpret_cast<const CUtensorMap*>(h->tmap_pv);
@@ -664,6 +661,14 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   a.mblocks = (max_q_len + 2 * tpt - 1) / (2 * tpt);
   a.tokens_per_tile = tpt;
   a.sh = h->shape;
+  if (c.head_dim == 128 && !(c.flags & LAZY_FLAG_PREFILL_ONE_CTA)) {
+    // CTA pairs (prefill_umma2.cu): a pair covers 4 * tpt query tokens
+    a.mblocks = (max_q_len + 4 * tpt - 1) / (4 * tpt);
+    const long long pgrid = 2LL * a.mblocks * c.num_kv_heads * num_reqs;
+    if (pgrid <= 0 || pgrid > INT_MAX) return LAZY_ERR_INVALID;
+    const int km = c.rope_style == LAZY_POS_ALIBI ? kKmAlibi : c.k_storage;
+    return launch_prefill_pair(h, a, km, (int)pgrid, stream);
+  }
   const long long grid = (long long)a.mblocks * c.num_kv_heads * num_reqs;
   if (grid <= 0 || grid > INT_MAX) return LAZY_ERR_INVALID;
   const int g = (int)grid;
