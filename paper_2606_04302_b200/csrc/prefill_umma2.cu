@@ -16,7 +16,7 @@
 //     copies of both CTAs.  V boxes of both CTAs count their bytes on the leader's barrier (TMA .cta_group::2).
 //
 // CTA = 2 Q tiles of 128 rows (GQA group packed into M); pair = 4 Q tiles.  16 warps per CTA as in prefill_umma.cu.
-// TMEM per CTA (512 columns): S0 | S1 | O0 | O1, P_t aliases the first 64 columns of S_t.
+// TMEM per CTA (512 columns): S0 | S1 | O0 | O1; S_t is two key halves of 64 columns, P_h aliases the first 32 of S_h.
 #include <climits>
 
 #include "prefill_common.cuh"
@@ -40,28 +40,28 @@ struct PairCfg {                        // head_dim 128
   static constexpr int OFF_V = OFF_K + kStages * K_STAGE;
   static constexpr int OFF_CS = OFF_V + kStages * V_STAGE;
   static constexpr int OFF_BAR = OFF_CS + kStages * CS_STAGE;
-  static constexpr int NUM_BARS = 36;
+  static constexpr int NUM_BARS = 40;
   static constexpr int OFF_TMEM = OFF_BAR + NUM_BARS * 8;
   static constexpr int OFF_SIGN = OFF_TMEM + 16;                // ring of 8 tiles x 8 pages (sign / page start)
   static constexpr int SMEM_BYTES = OFF_SIGN + 8 * kPagesPerTile * 4 + 1024;   // + alignment slack
 };
 
 // barrier indices.  (L): only the leader CTA's copy is used, threads of both CTAs arrive on it.
+// t = Q tile of the CTA (0, 1); h = half of a KV tile's keys (see "key halves" in the kernel).
 enum : int {
-  P_QFULL = 0,      // +t   TMA -> softmax WG t                                   (local)
-  P_QREADY = 2,     // +t   softmax WG t of both CTAs (8 warps) -> MMA            (L)
-  P_KFULL = 4,      // +s   TMA (K boxes + table rows) -> rotate WG               (local)
-  P_KREADY = 8,     // +s   rotate WGs of both CTAs (8 warps) -> MMA              (L)
-  P_KEMPTY = 12,    // +s   MMA commit (multicast) -> TMA of both CTAs
-  P_VFULL = 16,     // +s   V boxes of both CTAs -> MMA                           (L)
-  P_VEMPTY = 20,    // +s   MMA commit (multicast) -> TMA of both CTAs
-  P_VLASTFULL = 24, //      last tile's V boxes -> this CTA's fixer               (local, one shot)
-  P_VFIXED = 25,    //      fixers of both CTAs -> MMA                            (L, last tile only)
-  P_SFULL = 26,     // +t   MMA commit (multicast) -> softmax WG t
-  P_PREADY = 28,    // +t   softmax WG t of both CTAs -> MMA                      (L)
-  P_OFULL = 30,     // +t   MMA commit (multicast) -> softmax WG t (epilogue)
-  P_PHALF = 32,     // +t   softmax WG t of both CTAs -> MMA: keys 0..63 of P are in TMEM   (L)
-  P_PVH = 34,       // +t   MMA commit (multicast) -> softmax WG t: first half of PV done (slow path only)
+  P_QFULL = 0,      // +t     TMA -> softmax WG t                                   (local)
+  P_QREADY = 2,     // +t     softmax WG t of both CTAs (8 warps) -> MMA            (L)
+  P_KFULL = 4,      // +s     TMA (K boxes + table rows) -> rotate WG               (local)
+  P_KREADY = 8,     // +s     rotate WGs of both CTAs (8 warps) -> MMA              (L)
+  P_KEMPTY = 12,    // +s     MMA commit (multicast) -> TMA of both CTAs
+  P_VFULL = 16,     // +s     V boxes of both CTAs -> MMA                           (L)
+  P_VEMPTY = 20,    // +s     MMA commit (multicast) -> TMA of both CTAs
+  P_VLASTFULL = 24, //        last tile's V boxes -> this CTA's fixer               (local, one shot)
+  P_VFIXED = 25,    //        fixers of both CTAs -> MMA                            (L, last tile only)
+  P_SFULL = 26,     // +2t+h  MMA commit (multicast) -> softmax WG t: S half h is in TMEM
+  P_PREADY = 30,    // +2t+h  softmax WG t of both CTAs -> MMA: P half h is in TMEM (L)
+  P_PVDONE = 34,    // +2t+h  MMA commit (multicast) -> softmax WG t: O_t += P_h V has completed (slow path only)
+  P_OFULL = 38,     // +t     MMA commit (multicast) -> softmax WG t (epilogue)
 };
 
 // byte offset of 16-byte chunk `ci` of row `row` (0..63) inside a K half-stage (two 64-row slabs, 128B swizzle)
@@ -122,9 +122,11 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
   if (tid == 0) {
     for (int x = 0; x < 2; ++x) {
       ptx::mbar_init(bar(P_QFULL + x), 1);  ptx::mbar_init(bar(P_QREADY + x), 8);
+      ptx::mbar_init(bar(P_OFULL + x), 1);
+    }
+    for (int x = 0; x < 4; ++x) {
       ptx::mbar_init(bar(P_SFULL + x), 1);  ptx::mbar_init(bar(P_PREADY + x), 8);
-      ptx::mbar_init(bar(P_OFULL + x), 1);  ptx::mbar_init(bar(P_PHALF + x), 8);
-      ptx::mbar_init(bar(P_PVH + x), 1);
+      ptx::mbar_init(bar(P_PVDONE + x), 1);
     }
     for (int x = 0; x < kStages; ++x) {
       ptx::mbar_init(bar(P_KFULL + x), 1);  ptx::mbar_init(bar(P_KREADY + x), 8);
@@ -218,28 +220,39 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       // ================================ MMA issuer (leader CTA only) ========================================
       // The whole warp walks the loop convergently and ONE elected lane issues, so that every operand of
       // tcgen05.mma / tcgen05.commit is warp-uniform and lives in uniform registers.
+      //
+      // Key halves.  S_t = Q_t Khat^T of a 128-key tile is issued as TWO MMAs of N = 64: half h takes rows 32h..32h+31
+      // of each CTA's 64-key K stage, i.e. keys {32h..32h+31} u {64+32h..64+32h+31} of the tile, into columns
+      // 64h..64h+63 of S_t (P_h is packed over the first 32 of them).  O_t += P_h V follows with the matching V rows.
+      // What this buys: the columns of half h are free again as soon as PV_h has run, so QK_h of the NEXT tile is
+      // issued right behind it, while the softmax warpgroup is still busy with the other half.  S is therefore
+      // (nearly) always waiting when a warpgroup comes back for it, and the softmax -> PV -> QK -> softmax chain that
+      // paced the kernel (with S_t of N = 128 aliased by P_t it could not be cut) is gone.  The price is the Q operand
+      // read twice per tile (N = 64 MMAs are shared-memory-bound: ~40 instead of 32 cycles per k-step).
       if (rank == 0) {
-        constexpr uint32_t IDESC_QK = ptx::umma_idesc_bf16(256, 128, 0, 0);
+        constexpr uint32_t IDESC_QK = ptx::umma_idesc_bf16(256, 64, 0, 0);
         constexpr uint32_t IDESC_PV = ptx::umma_idesc_bf16(256, D, 0, 1);       // B = V is MN-major
         const uint32_t tb = __shfl_sync(0xffffffffu, tbase, 0);
         const int nkv = __shfl_sync(0xffffffffu, n_kv, 0);
         const bool leader = ptx::elect_one();
-        auto qk = [&](int t, int s) {
+        auto qk = [&](int t, int s, int h) {
           if (leader) {
-            const uint32_t qa = sQ + t * C::Q_TILE, ka = sK + s * C::K_STAGE;
+            const uint32_t qa = sQ + t * C::Q_TILE, ka = sK + s * C::K_STAGE + h * (32 * 128);
 #pragma unroll
             for (int k = 0; k < D / 16; ++k)
-              ptx::umma_ss_pair(tb + t * 128, ptx::umma_desc_sw128(qa + (k >> 2) * kHalfBytes + (k & 3) * 32, 0, 1024),
+              ptx::umma_ss_pair(tb + t * 128 + h * 64,
+                                ptx::umma_desc_sw128(qa + (k >> 2) * kHalfBytes + (k & 3) * 32, 0, 1024),
                                 ptx::umma_desc_sw128(ka + (k >> 2) * C::K_SLAB + (k & 3) * 32, 0, 1024), IDESC_QK, k > 0);
           }
         };
-        auto pv = [&](int t, int s, uint32_t acc, int k0, int k1) {
+        auto pv = [&](int t, int s, int h, uint32_t acc) {
           if (leader) {
-            const uint32_t va = sV + s * C::V_STAGE;
+            const uint32_t va = sV + s * C::V_STAGE + h * (32 * 128);
 #pragma unroll
-            for (int k = k0; k < k1; ++k)
-              ptx::umma_ts_pair(tb + 256 + t * 128, tb + t * 128 + k * 8,
-                                ptx::umma_desc_sw128(va + k * 2048, kHalfBytes, 1024), IDESC_PV, acc | (uint32_t)(k > 0));
+            for (int k = 0; k < 4; ++k)                       // keys 32h + 16k (k < 2), 64 + 32h + 16(k-2) (k >= 2)
+              ptx::umma_ts_pair(tb + 256 + t * 128, tb + t * 128 + h * 64 + k * 8,
+                                ptx::umma_desc_sw128(va + ((k & 1) * 16 + (k >> 1) * 64) * 128, kHalfBytes, 1024), IDESC_PV,
+                                acc | (uint32_t)(k > 0));
           }
         };
         auto commit = [&](int idx) { if (leader) ptx::umma_commit_pair(bar(idx)); };
@@ -247,35 +260,37 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         for (int t = 0; t < 2; ++t) {
           ptx::mbar_wait(bar(P_QREADY + t), 0);
           ptx::tc_fence_after();
-          qk(t, 0);
-          commit(P_SFULL + t);
+          for (int h = 0; h < 2; ++h) { qk(t, 0, h); commit(P_SFULL + 2 * t + h); }
         }
         commit(P_KEMPTY + 0);
+        // Hand-offs are taken in the fixed order (tile 0, half 0), (tile 1, half 0), (tile 0, half 1), (tile 1, half 1):
+        // the two Q tiles stay in lockstep, so the K / V rings -- which only turn when BOTH tiles have consumed a
+        // stage -- keep flowing.  (Serving whichever tile was ready first let one softmax warpgroup run a full ring
+        // ahead of the other; the kernel then alternated between bursts of one tile and refill latencies: 668 TFLOP/s.)
         for (int j = 0; j < nkv; ++j) {
           const int s = j & (kStages - 1), sn = (j + 1) & (kStages - 1);
           if (j == nkv - 1) ptx::mbar_wait(bar(P_VFIXED), 0);
           else ptx::mbar_wait(bar(P_VFULL + s), (j / kStages) & 1);
 #pragma unroll
-          for (int t = 0; t < 2; ++t) {
-            // PV starts on the first 64 keys while the softmax warpgroups are still exponentiating the other 64
-            ptx::mbar_wait(bar(P_PHALF + t), j & 1);
-            ptx::tc_fence_after();
-            pv(t, s, j > 0, 0, kTileRows / 32);
-            commit(P_PVH + t);
-            ptx::mbar_wait(bar(P_PREADY + t), j & 1);
-            ptx::tc_fence_after();
-            pv(t, s, 1u, kTileRows / 32, kTileRows / 16);
-            if (t == 1) commit(P_VEMPTY + s);
-            if (j + 1 < nkv) {
-              if (t == 0) {
-                ptx::mbar_wait(bar(P_KREADY + sn), ((j + 1) / kStages) & 1);
-                ptx::tc_fence_after();
+          for (int h = 0; h < 2; ++h) {
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+              ptx::mbar_wait(bar(P_PREADY + 2 * t + h), j & 1);
+              ptx::tc_fence_after();
+              pv(t, s, h, (uint32_t)(j > 0 || h > 0));
+              commit(P_PVDONE + 2 * t + h);
+              if (h == 1 && t == 1) commit(P_VEMPTY + s);
+              if (j + 1 < nkv) {
+                if (h == 0 && t == 0) {
+                  ptx::mbar_wait(bar(P_KREADY + sn), ((j + 1) / kStages) & 1);
+                  ptx::tc_fence_after();
+                }
+                qk(t, sn, h);
+                commit(P_SFULL + 2 * t + h);
+                if (h == 1 && t == 1) commit(P_KEMPTY + sn);
+              } else if (h == 1) {
+                commit(P_OFULL + t);
               }
-              qk(t, sn);
-              commit(P_SFULL + t);
-              if (t == 1) commit(P_KEMPTY + sn);
-            } else {
-              commit(P_OFULL + t);
             }
           }
         }
@@ -443,28 +458,34 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       for (int x = 0; x < kPageSize / 2; ++x)
         alibi_d2[x] = make_float2(alibi_slope * (float)(2 * x), alibi_slope * (float)(2 * x + 1));
     }
-    // Online softmax with optimistic exponentials: see prefill_umma.cu (same code, barriers of the pair).
+    // Online softmax with optimistic exponentials (see prefill_umma.cu), one key half at a time: columns c of half h
+    // are the keys key(c) = 32h + c (c < 32), 64 + 32h + (c - 32) (c >= 32) of the tile.  The two warpgroups run free.
     constexpr float kDanger = 20.f;
     float m_used = -INFINITY, l_run = 0.f;
-    if (t == 1) ptx::named_bar_arrive(2, 256);                            // tile 0 goes first
     for (int j = 0; j < n_kv; ++j) {
-      uint32_t sreg[128];                                     // this row of S (fp32 bits); P is packed over it in place
-      ptx::mbar_wait(bar(P_SFULL + t), j & 1);
-      ptx::tc_fence_after();
-      float abase[kPagesPerTile];                             // kKmAlibi: slope * (page start - m) of the tile's pages
-#pragma unroll
-      for (int c = 0; c < 4; ++c) ptx::tmem_ld32(tS + c * 32, sreg + c * 32);
-      if (KM == kKmAlibi) {
-        const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 7) * kPagesPerTile;
-#pragma unroll
-        for (int pg = 0; pg < kPagesPerTile; ++pg) abase[pg] = alibi_slope * (float)(pstart[pg] - alibi_pos_q);
-      }
       const bool edge = j * kTileRows + kTileRows - 1 > lim_min;   // tile touches the causal edge / the tail
-      const int lim_col = lim_row - j * kTileRows;            // column visible iff col <= lim_col
-      auto prep_half = [&](int hf) {
+      const int lim_col = lim_row - j * kTileRows;            // key of the tile visible iff key <= lim_col
+      const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 7) * kPagesPerTile;
+#pragma unroll
+      for (int hf = 0; hf < 2; ++hf) {
+        uint32_t sreg[64];                                    // this row of S half (fp32 bits); P is packed over it
+        const uint32_t tSh = tS + 64 * hf;
+        ptx::mbar_wait(bar(P_SFULL + 2 * t + hf), j & 1);
+        ptx::tc_fence_after();
+        ptx::tmem_ld32(tSh, sreg);
+        ptx::tmem_ld32(tSh + 32, sreg + 32);
+        float abase[4];                                       // kKmAlibi: slope * (page start - m) of the half's 4 pages
         if (KM == kKmAlibi) {
 #pragma unroll
-          for (int x = 64 * hf; x < 64 * hf + 64; x += 2) {
+          for (int pg = 0; pg < 4; ++pg)
+            abase[pg] = alibi_slope * (float)(pstart[2 * hf + (pg & 1) + 4 * (pg >> 1)] - alibi_pos_q);
+        }
+        ptx::tmem_wait_ld();
+        if (KM == kKmAlibi) {
+          // S += slope * (n - m), n = page start + t: the in-page part slope * t goes to the elements here, the
+          // per-page part abase[] into the maxima and into the constant of the exponential
+#pragma unroll
+          for (int x = 0; x < 64; x += 2) {
             const float2 v = __fadd2_rn(make_float2(f32(sreg[x]), f32(sreg[x + 1])), alibi_d2[(x & 15) >> 1]);
             sreg[x] = __float_as_uint(v.x);
             sreg[x + 1] = __float_as_uint(v.y);
@@ -472,36 +493,31 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         }
         if (edge) {
 #pragma unroll
-          for (int x = 64 * hf; x < 64 * hf + 64; ++x)
-            if (x > lim_col) sreg[x] = 0xff800000u;           // -inf replaces the value (NaN-safe)
+          for (int x = 0; x < 64; ++x)
+            if (32 * hf + x + (x >= 32 ? 32 : 0) > lim_col) sreg[x] = 0xff800000u;   // -inf replaces the value (NaN-safe)
         }
-      };
-      ptx::tmem_wait_ld();
-      prep_half(0);
-      prep_half(1);
-      if (j == 0) {                                           // first tile: the exact row max (column 0 is always visible)
-        float r0 = -INFINITY, r1 = -INFINITY;
+        const bool first = j == 0 && hf == 0;
+        if (first) {                                          // the exact max of the first half (key 0 is always visible)
+          float r0 = -INFINITY, r1 = -INFINITY;
 #pragma unroll
-        for (int pg = 0; pg < kPagesPerTile; ++pg) {
-          float a0 = -INFINITY, a1 = -INFINITY;
+          for (int pg = 0; pg < 4; ++pg) {
+            float a0 = -INFINITY, a1 = -INFINITY;
 #pragma unroll
-          for (int x = 16 * pg; x < 16 * pg + 16; x += 4) {
-            a0 = fmaxf(fmaxf(a0, f32(sreg[x + 0])), f32(sreg[x + 1]));
-            a1 = fmaxf(fmaxf(a1, f32(sreg[x + 2])), f32(sreg[x + 3]));
+            for (int x = 16 * pg; x < 16 * pg + 16; x += 4) {
+              a0 = fmaxf(fmaxf(a0, f32(sreg[x + 0])), f32(sreg[x + 1]));
+              a1 = fmaxf(fmaxf(a1, f32(sreg[x + 2])), f32(sreg[x + 3]));
+            }
+            if (KM == kKmAlibi) r0 = fmaxf(r0, fmaxf(a0, a1) + abase[pg]);
+            else { r0 = fmaxf(r0, a0); r1 = fmaxf(r1, a1); }
           }
-          if (KM == kKmAlibi) r0 = fmaxf(r0, fmaxf(a0, a1) + abase[pg]);
-          else { r0 = fmaxf(r0, a0); r1 = fmaxf(r1, a1); }
+          m_used = fmaxf(r0, r1);
         }
-        m_used = fmaxf(r0, r1);
-      }
-      ptx::named_bar_sync(2 + t, 256);                                   // my turn on the MUFU
-#pragma unroll
-      for (int hf = 0; hf < 2; ++hf) {
+        // P = 2^(S - m_used), packed in place; the half's own maximum is taken alongside
         const float2 negm = make_float2(-m_used, -m_used);
         float2 sum0 = make_float2(0.f, 0.f), sum1 = make_float2(0.f, 0.f);
         float mx0 = -INFINITY, mx1 = -INFINITY, mxa = -INFINITY;
 #pragma unroll
-        for (int x = 32 * hf; x < 32 * hf + 32; x += 2) {
+        for (int x = 0; x < 32; x += 2) {
           const float s0 = f32(sreg[2 * x]), s1 = f32(sreg[2 * x + 1]), s2 = f32(sreg[2 * x + 2]), s3 = f32(sreg[2 * x + 3]);
           const float2 nm = KM == kKmAlibi ? make_float2(abase[x >> 3] - m_used, abase[x >> 3] - m_used) : negm;
           const float2 v0 = __fadd2_rn(make_float2(s0, s1), nm);
@@ -521,12 +537,13 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         }
         const float mxh = KM == kKmAlibi ? mxa : fmaxf(mx0, mx1);
         float hsum = (sum0.x + sum0.y) + (sum1.x + sum1.y);
-        const bool slow = j > 0 && __any_sync(0xffffffffu, mxh > m_used + kDanger);
-        if (slow) {                                            // see prefill_umma.cu
-          if (hf == 1) {
-            ptx::mbar_wait(bar(P_PVH + t), j & 1);
-            ptx::tc_fence_after();
-          }
+        const bool slow = !first && __any_sync(0xffffffffu, mxh > m_used + kDanger);
+        if (slow) {
+          // Slow path (a score beyond 2^kDanger of m_used).  O and l move to the new maximum -- once the last PV
+          // issued for this Q tile (the other half: of this tile for h = 1, of the previous tile for h = 0) has
+          // completed -- and this half of P is rebuilt 16 columns (one page) at a time straight from S in TMEM.
+          ptx::mbar_wait(bar(P_PVDONE + 2 * t + (hf ^ 1)), (hf == 1 ? j : j - 1) & 1);
+          ptx::tc_fence_after();
           const float m_new = fmaxf(m_used, mxh);
           const float f = ex2(m_used - m_new);
           m_used = m_new;
@@ -542,39 +559,36 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
           }
           ptx::tmem_wait_st();
           hsum = 0.f;
-          const int* pstart = reinterpret_cast<const int*>(smem + C::OFF_SIGN) + (j & 7) * kPagesPerTile;
 #pragma unroll 1
           for (int c = 0; c < 4; ++c) {
-            const int col0 = 64 * hf + 16 * c;                // one page of the tile
+            const int key0 = 32 * hf + 16 * (c & 1) + 64 * (c >> 1);     // first key of this page of the half
             uint32_t rr[16], pk[8];
-            ptx::tmem_ld16(tS + col0, rr);
+            ptx::tmem_ld16(tSh + 16 * c, rr);
             ptx::tmem_wait_ld();
             float off = -m_used;
-            if (KM == kKmAlibi) off += alibi_slope * (float)(pstart[col0 >> 4] - alibi_pos_q);
+            if (KM == kKmAlibi) off += alibi_slope * (float)(pstart[key0 >> 4] - alibi_pos_q);
 #pragma unroll
             for (int x = 0; x < 16; x += 2) {
               float v0 = f32(rr[x]) + off, v1 = f32(rr[x + 1]) + off;
               if (KM == kKmAlibi) { v0 += alibi_slope * (float)x; v1 += alibi_slope * (float)(x + 1); }
-              if (col0 + x > lim_col) v0 = -INFINITY;         // lim_col >= 127 on interior tiles
-              if (col0 + x + 1 > lim_col) v1 = -INFINITY;
+              if (key0 + x > lim_col) v0 = -INFINITY;         // lim_col >= 127 on interior tiles
+              if (key0 + x + 1 > lim_col) v1 = -INFINITY;
               const float q0 = ex2(v0), q1 = ex2(v1);
               hsum += q0 + q1;
               pk[x >> 1] = ptx::pack_bf16(q0, q1);
             }
-            ptx::tmem_st8(tS + (col0 >> 1), pk);
+            ptx::tmem_st8(tSh + 8 * c, pk);
           }
         }
         l_run += hsum;
-        if (hf == 1) ptx::named_bar_arrive(2 + (t ^ 1), 256);                 // the other tile's turn
-        if (!slow) ptx::tmem_st32(tS + 32 * hf, sreg + 32 * hf);   // P (bf16 pairs) over the first 64 columns of S
+        if (!slow) ptx::tmem_st32(tSh, sreg);                 // P_h (bf16 pairs) over the first 32 columns of S_h
         ptx::tmem_wait_st();
         ptx::tc_fence_before();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive_cluster(lbar((hf == 0 ? P_PHALF : P_PREADY) + t));
+        if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_PREADY + 2 * t + hf));
       }
     }
 
-    if (t == 0) ptx::named_bar_sync(2, 256);                              // consume tile 1's last hand-off
     // ---- epilogue (a9): normalise, round to bf16, store the row -------------------------------------------
     ptx::mbar_wait(bar(P_OFULL + t), 0);
     ptx::tc_fence_after();
