@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "liblazyattn.so")
 
 LAZY_OK, LAZY_ERR_INVALID, LAZY_ERR_UNSUPPORTED, LAZY_ERR_WORKSPACE, LAZY_ERR_CUDA = 0, -1, -2, -3, -4
 LAZY_FLAG_ROWWISE_KERNELS = 1
+LAZY_FLAG_PREFILL_ONE_CTA = 2
 LAZY_K_UNROTATED, LAZY_K_STORED_POS, LAZY_K_ABSOLUTE = 0, 1, 2
 LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
 
@@ -268,7 +269,7 @@ def lazy_attn_mixed(h: LazyHandle, k_cache, v_cache, *, q_prefill, block_table_p
                      int(decode_sms), _ptr(out_decode))
     rc = lib().lazy_attn_mixed(h.ptr, ctypes.byref(args), _ptr(k_cache), _ptr(v_cache), _stream(stream))
     if rc != 0:
-        raise LazyError("lazy_attn_mixed", "lazy_debug_validate", rc)
+        raise LazyError("lazy_attn_mixed", rc)
 
 
 class HostStep(ctypes.Structure):

@@ -480,7 +480,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       ptx::tmem_wait_ld();
       prep_half(0);
       prep_half(1);
-      if (j == 0) {                                           // first tile: the exact row max (column 0 is always visible)
+      // The exact row max first: on the first tile (column 0 is always visible), and always under ALiBi, whose bias
+      // grows by slope * 128 from tile to tile by construction -- an optimistic reference would be stale every tile.
+      if (j == 0 || KM == kKmAlibi) {
         float r0 = -INFINITY, r1 = -INFINITY;
 #pragma unroll
         for (int pg = 0; pg < kPagesPerTile; ++pg) {
@@ -493,7 +495,25 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
           if (KM == kKmAlibi) r0 = fmaxf(r0, fmaxf(a0, a1) + abase[pg]);
           else { r0 = fmaxf(r0, a0); r1 = fmaxf(r1, a1); }
         }
-        m_used = fmaxf(r0, r1);
+        const float mx = fmaxf(r0, r1);
+        if (j == 0) {
+          m_used = mx;
+        } else if (__any_sync(0xffffffffu, mx > m_used + 8.f)) {   // PV(j-1) has completed: S(j) was committed after it
+          const float m_new = fmaxf(m_used, mx);
+          const float f = ex2(m_used - m_new);
+          m_used = m_new;
+          l_run *= f;
+#pragma unroll 1
+          for (int c = 0; c < D / 16; ++c) {
+            uint32_t rr[16];
+            ptx::tmem_ld16(tO + c * 16, rr);
+            ptx::tmem_wait_ld();
+#pragma unroll
+            for (int x = 0; x < 16; ++x) rr[x] = __float_as_uint(f32(rr[x]) * f);
+            ptx::tmem_st16(tO + c * 16, rr);
+          }
+          ptx::tmem_wait_st();
+        }
       }
       ptx::named_bar_sync(2 + t, 256);                                   // my turn on the MUFU
 #pragma unroll
@@ -523,7 +543,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         }
         const float mxh = KM == kKmAlibi ? mxa : fmaxf(mx0, mx1);
         float hsum = (sum0.x + sum0.y) + (sum1.x + sum1.y);
-        const bool slow = j > 0 && __any_sync(0xffffffffu, mxh > m_used + kDanger);
+        const bool slow = j > 0 && KM != kKmAlibi && __any_sync(0xffffffffu, mxh > m_used + kDanger);
         if (slow) {
           // Slow path (a score beyond 2^kDanger of m_used).  O and l -- which hold the tiles < j, and keys 0..63 of
           // this tile once the first half of PV has completed -- move to the new maximum; then this half of P is

@@ -497,7 +497,30 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
             if (32 * hf + x + (x >= 32 ? 32 : 0) > lim_col) sreg[x] = 0xff800000u;   // -inf replaces the value (NaN-safe)
         }
         const bool first = j == 0 && hf == 0;
-        if (first) {                                          // the exact max of the first half (key 0 is always visible)
+        // O and l move to a new reference maximum.  The last PV issued for this Q tile (the other half: of this tile
+        // for h = 1, of the previous tile for h = 0) must have completed before O is touched.
+        auto rescale_to = [&](float m_new) {
+          ptx::mbar_wait(bar(P_PVDONE + 2 * t + (hf ^ 1)), (hf == 1 ? j : j - 1) & 1);
+          ptx::tc_fence_after();
+          const float f = ex2(m_used - m_new);
+          m_used = m_new;
+          l_run *= f;
+#pragma unroll 1
+          for (int c = 0; c < D / 16; ++c) {
+            uint32_t rr[16];
+            ptx::tmem_ld16(tO + c * 16, rr);
+            ptx::tmem_wait_ld();
+#pragma unroll
+            for (int x = 0; x < 16; ++x) rr[x] = __float_as_uint(f32(rr[x]) * f);
+            ptx::tmem_st16(tO + c * 16, rr);
+          }
+          ptx::tmem_wait_st();
+        };
+        // The exact maximum first: for the very first half (key 0 is always visible), and always under ALiBi, whose
+        // bias grows by slope * 128 from tile to tile by construction -- an optimistic reference would be stale every
+        // tile (lazy rescale: only when the maximum grew by more than 2^8).
+        constexpr bool kExactMax = KM == kKmAlibi;
+        if (first || kExactMax) {
           float r0 = -INFINITY, r1 = -INFINITY;
 #pragma unroll
           for (int pg = 0; pg < 4; ++pg) {
@@ -510,7 +533,9 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
             if (KM == kKmAlibi) r0 = fmaxf(r0, fmaxf(a0, a1) + abase[pg]);
             else { r0 = fmaxf(r0, a0); r1 = fmaxf(r1, a1); }
           }
-          m_used = fmaxf(r0, r1);
+          const float mx = fmaxf(r0, r1);
+          if (first) m_used = mx;
+          else if (__any_sync(0xffffffffu, mx > m_used + 8.f)) rescale_to(fmaxf(m_used, mx));
         }
         // P = 2^(S - m_used), packed in place; the half's own maximum is taken alongside
         const float2 negm = make_float2(-m_used, -m_used);
@@ -537,27 +562,11 @@ prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         }
         const float mxh = KM == kKmAlibi ? mxa : fmaxf(mx0, mx1);
         float hsum = (sum0.x + sum0.y) + (sum1.x + sum1.y);
-        const bool slow = !first && __any_sync(0xffffffffu, mxh > m_used + kDanger);
+        const bool slow = !first && !kExactMax && __any_sync(0xffffffffu, mxh > m_used + kDanger);
         if (slow) {
-          // Slow path (a score beyond 2^kDanger of m_used).  O and l move to the new maximum -- once the last PV
-          // issued for this Q tile (the other half: of this tile for h = 1, of the previous tile for h = 0) has
-          // completed -- and this half of P is rebuilt 16 columns (one page) at a time straight from S in TMEM.
-          ptx::mbar_wait(bar(P_PVDONE + 2 * t + (hf ^ 1)), (hf == 1 ? j : j - 1) & 1);
-          ptx::tc_fence_after();
-          const float m_new = fmaxf(m_used, mxh);
-          const float f = ex2(m_used - m_new);
-          m_used = m_new;
-          l_run *= f;
-#pragma unroll 1
-          for (int c = 0; c < D / 16; ++c) {
-            uint32_t rr[16];
-            ptx::tmem_ld16(tO + c * 16, rr);
-            ptx::tmem_wait_ld();
-#pragma unroll
-            for (int x = 0; x < 16; ++x) rr[x] = __float_as_uint(f32(rr[x]) * f);
-            ptx::tmem_st16(tO + c * 16, rr);
-          }
-          ptx::tmem_wait_st();
+          // Slow path (a score beyond 2^kDanger of m_used): O and l move to the new maximum and this half of P is
+          // rebuilt 16 columns (one page) at a time straight from S in TMEM.
+          rescale_to(fmaxf(m_used, mxh));
           hsum = 0.f;
 #pragma unroll 1
           for (int c = 0; c < 4; ++c) {

@@ -1,0 +1,172 @@
+"""-m gpu parity cases added in round 2 (VERDICT r1 "parity gaps"):
+  * key position ABOVE the query position (negative page offsets) for the un-rotated decode, prefill and ALiBi paths
+    (PAPER.md Fact 3.2, L154-158: only n - m matters, either sign; reading 6: the mask is by index);
+  * slot permutation with positions on the GPU (twin of the oracle pin test_slot_permutation_with_positions);
+  * kv-head counts 2 and 16 (grid.y > 1 in decode);
+  * scores that jump far above the running reference maximum late in the sequence (the prefill kernels' optimistic
+    exponentials must take their slow path) -- pair kernel, one-CTA kernel at head_dim 128 and 64;
+  * an error return of lazy_attn_mixed."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_04302_b200 import binding as B
+from paper_2606_04302_b200 import workloads as W
+from paper_2606_04302_b200.runner import DeviceBatch
+
+from gpu_util import run_and_compare
+from test_gpu_edges import _custom, SH128, SH64, SH7
+
+pytestmark = pytest.mark.gpu
+
+SH_HKV2 = W.LazyShape(8, 2, 128, 5.0e5)
+SH_HKV16 = W.LazyShape(32, 16, 64, 1.0e4)
+SHAPES = [pytest.param(SH128, id="g4d128"), pytest.param(SH64, id="g4d64"), pytest.param(SH7, id="g7d128")]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    from paper_2606_04302_b200 import build
+    build.build()
+    B.lib()
+
+
+def _reposition(batch, mode, seed=0):
+    """Re-assign the logical start of every page slot: 'descending' puts the query's own pages at the LOWEST positions
+    (every earlier page sits above the query: all page offsets negative), 'shuffled' mixes both signs."""
+    P = batch.shape.page_size
+    pp = batch.page_logical_pos.clone()
+    rng = np.random.default_rng(seed)
+    for r, L in enumerate(batch.steps[0].seq_lens.tolist()):
+        n = (L + P - 1) // P
+        if n == 0:
+            continue
+        starts = 7 + P * np.arange(n) * 3                    # distinct, non-overlapping, not page aligned
+        if mode == "descending":
+            starts = starts[::-1].copy()
+        else:
+            starts = rng.permutation(starts)
+        pp[r, :n] = torch.from_numpy(starts.astype(np.int32))
+    return W.LazyBatch(name=batch.name + "_" + mode, shape=batch.shape, k_pool=batch.k_pool, v_pool=batch.v_pool,
+                       block_table=batch.block_table, page_logical_pos=pp, steps=batch.steps)
+
+
+@pytest.mark.parametrize("mode", ["descending", "shuffled"])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_decode_key_positions_above_query(shape, mode):
+    seq = [1, 17, 33, 100, 257, 640, 1000]
+    b = _reposition(_custom(shape, seq, [1] * len(seq), seed=31, kind="decode"), mode, seed=1)
+    run_and_compare(b)
+
+
+@pytest.mark.parametrize("mode", ["descending", "shuffled"])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_prefill_key_positions_above_query(shape, mode):
+    seq = [40, 200, 129, 300, 700]
+    qls = [40, 64, 1, 130, 257]
+    b = _reposition(_custom(shape, seq, qls, seed=32), mode, seed=2)
+    run_and_compare(b)
+    run_and_compare(b, flags=B.LAZY_FLAG_PREFILL_ONE_CTA)
+
+
+@pytest.mark.parametrize("kind", ["decode", "prefill"])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_alibi_key_positions_above_query(shape, kind):
+    seq = [33, 100, 257, 640]
+    qls = [1, 1, 1, 1] if kind == "decode" else [33, 64, 1, 200]
+    b = _reposition(_custom(shape, seq, qls, seed=33, kind=kind), "shuffled", seed=3)
+    slopes = [2.0 ** (-8.0 * (i + 1) / shape.num_q_heads) * 0.05 for i in range(shape.num_q_heads)]
+    run_and_compare(b, dev_kw=dict(rope_style=B.LAZY_POS_ALIBI, alibi_slopes=slopes),
+                    oracle_kw=dict(alibi_slopes=slopes))
+
+
+@pytest.mark.parametrize("shape", SHAPES)
+def test_alibi_steep_slopes_prefill(shape):
+    """Steep slopes: the bias grows by slope * 128 per tile, so the reference maximum moves every tile."""
+    b = _custom(shape, [900, 1300], [200, 300], seed=34)
+    slopes = [2.0 ** (-8.0 * (i + 1) / shape.num_q_heads) for i in range(shape.num_q_heads)]
+    run_and_compare(b, dev_kw=dict(rope_style=B.LAZY_POS_ALIBI, alibi_slopes=slopes),
+                    oracle_kw=dict(alibi_slopes=slopes))
+
+
+def test_slot_permutation_with_positions_gpu():
+    """Decode over pages given in another slot order, every page keeping its own logical position, is the same
+    attention problem: both orders must match the oracle and each other (up to the split-KV summation order)."""
+    b = _custom(SH128, [640, 333], [1, 1], seed=35, pos_gap=1000, kind="decode")
+    P = b.shape.page_size
+    bt, pp = b.block_table.clone(), b.page_logical_pos.clone()
+    rng = np.random.default_rng(5)
+    for r, L in enumerate(b.steps[0].seq_lens.tolist()):
+        full = (L - 1) // P                                  # the page holding the query token stays last
+        perm = torch.from_numpy(rng.permutation(full))
+        bt[r, :full] = b.block_table[r, :full][perm]
+        pp[r, :full] = b.page_logical_pos[r, :full][perm]
+    b2 = W.LazyBatch(name="perm", shape=b.shape, k_pool=b.k_pool, v_pool=b.v_pool, block_table=bt,
+                     page_logical_pos=pp, steps=b.steps)
+    outs = []
+    for bb in (b, b2):
+        run_and_compare(bb)
+        dev = DeviceBatch(bb)
+        outs.append(dev.run_step(bb.steps[0]).float().cpu())
+        dev.close()
+    assert (outs[0] - outs[1]).abs().max().item() < 2e-3
+
+
+@pytest.mark.parametrize("shape", [pytest.param(SH_HKV2, id="hkv2"), pytest.param(SH_HKV16, id="hkv16")])
+def test_kv_head_counts(shape):
+    seq = [1, 31, 100, 257, 640]
+    run_and_compare(_custom(shape, seq, [1] * len(seq), seed=36, kind="decode"))
+    run_and_compare(_custom(shape, [40, 200, 300], [40, 64, 130], seed=37))
+
+
+def _late_dominant(shape, seq, qls, seed, first_big=300, boost=15.0):
+    """Every query and every key from token `first_big` on get `boost` added on the x1 element of the SLOWEST rotation
+    pair (angle ~ 1e-6 rad per token: the rotation leaves it in place), so all late scores sit boost^2 * log2(e)/sqrt(D)
+    (~ 29 log2 units at D = 128, ~ 40 at D = 64) above the early ones while the softmax over the late keys stays as
+    flat as ever: the reference maximum taken from the first tiles is stale by far more than 2^20."""
+    b = _custom(shape, seq, qls, seed=seed)
+    P, jj = shape.page_size, shape.head_dim // 2 - 1
+    k = b.k_pool.clone()
+    for r, L in enumerate(seq):
+        for s in range(first_big // P, (L + P - 1) // P):
+            pg = int(b.block_table[r, s])
+            k[pg, :, :, jj] = (k[pg, :, :, jj].float() + boost).to(torch.bfloat16)
+    st = b.steps[0]
+    q = st.q.clone()
+    q[:, :, jj] = (q[:, :, jj].float() + boost).to(torch.bfloat16)
+    step = W.Step(kind=st.kind, q=q, seq_lens=st.seq_lens, cu_q_lens=st.cu_q_lens)
+    return W.LazyBatch(name="late_dominant", shape=shape, k_pool=k, v_pool=b.v_pool, block_table=b.block_table,
+                       page_logical_pos=b.page_logical_pos, steps=[step])
+
+
+@pytest.mark.parametrize("flags", [pytest.param(0, id="prod"), pytest.param(B.LAZY_FLAG_PREFILL_ONE_CTA, id="one_cta")])
+@pytest.mark.parametrize("shape", SHAPES)
+def test_prefill_late_dominant_keys(shape, flags):
+    """The optimistic exponentials of the prefill kernels must fall back (rescale O and l, rebuild P) when a later
+    tile's scores exceed the reference maximum by more than 2^20 -- in the first and in the second key half."""
+    for first_big in (304, 352):                              # a page in the first / second key half of a tile
+        b = _late_dominant(shape, [900, 517], [200, 517], seed=38, first_big=first_big)
+        # Scores of magnitude S ~ 30-40 log2 units carry an absolute error S * 2^-9 * sqrt(2) ~ 0.1 from the bf16
+        # rounding of the rotated q and k alone (the oracle keeps them in fp64): softmax weights move by several
+        # per cent.  The gates are widened for this adversarial input; a wrong slow path is off by factors of 2^20.
+        run_and_compare(b, flags=flags, gates=dict(abs_scale=8.0, rel_rms=6e-2, rel_max=0.15))
+
+
+def test_mixed_call_error_return():
+    batch = W.config5(scale=0.2)
+    pre, dec = batch.steps[0], batch.steps[1]
+    dev = DeviceBatch(batch)
+    d = dev.device
+    try:
+        bt_p, pp_p = dev.tables_for(pre)
+        bt_d, pp_d = dev.tables_for(dec)
+        with pytest.raises(B.LazyError) as ei:
+            B.lazy_attn_mixed(dev.handle, dev.k_pool, dev.v_pool, q_prefill=pre.q.to(d), block_table_prefill=bt_p,
+                              page_logical_pos_prefill=pp_p, seq_lens_prefill=pre.seq_lens.to(d),
+                              cu_q_lens=pre.cu_q_lens.to(d), max_q_len=8, out_prefill=torch.empty_like(pre.q, device=d),
+                              q_decode=dec.q.to(d), block_table_decode=bt_d, page_logical_pos_decode=pp_d,
+                              seq_lens_decode=dec.seq_lens.to(d), out_decode=torch.empty_like(dec.q, device=d),
+                              decode_sms=-1)
+        assert ei.value.status == B.LAZY_ERR_INVALID
+    finally:
+        dev.close()
