@@ -100,3 +100,21 @@ def test_pool_pins_and_errors():
         pool.close()
     with pytest.raises(B.LazyError):
         B.LazyPool(0)
+
+
+def test_table1_simulation_small_instance():
+    """The Table 1 sweep on a small instance: at every budget and skew the position-free pool hits
+    at least as often as the position-aware one, more budget never hurts, and the LRU simulation tracks Eq. 1 / Eq. 2."""
+    from paper_2606_04302_b200 import table1_sim as T
+    rows = T.simulate(queries=1500, pool_docs=3000, doc_tokens=64, budgets_gb=[("s", 0.2), ("m", 0.8)],
+                      skews=[("Low", 1.1), ("High", 2.1)])
+    assert len(rows) == 4
+    by = {(r["budget"], r["skew"]): r for r in rows}
+    for r in rows:
+        assert r["lazy_sim"] >= r["aware_sim"] and r["lazy_eq1"] >= r["aware_eq2"]
+        assert r["lazy_sim"] <= r["lazy_eq1"] + 2.0                      # an LRU pool cannot beat the ideal top-C cache
+        assert r["lazy_sim"] >= 0.45 * r["lazy_eq1"]                     # ... and LRU with 10 pinned documents sits below it
+    for skew in ("Low", "High"):
+        assert by[("m", skew)]["lazy_sim"] >= by[("s", skew)]["lazy_sim"]
+        assert by[("m", skew)]["aware_sim"] >= by[("s", skew)]["aware_sim"]
+    assert by[("s", "Low")]["lazy_sim"] > 1.3 * by[("s", "Low")]["aware_sim"]
