@@ -6,7 +6,10 @@
 A step = one pass of the whole hot path over one synthetic Zipf-shared RAG batch: lazy_cache_write of the
 step's new tokens, then the attention call(s) (decode for cfg2/cfg4, prefill for cfg3, prefill + decode for
 cfg5).  Default workload: BASELINE.json configs[1] (decode at the Llama-3-8B layer shape); unless
---no-secondary, the prefill headline (configs[2]) is measured in the same run and reported under "prefill".
+--no-secondary, configs[2..4] (prefill, long-context decode, mixed step) are measured in the same run and
+reported kernel by kernel under "configs".  The decode `roofline` is taken on the noshare variant of the
+workload (every drawn document distinct, so algorithmic bytes are DRAM bytes); the Zipf-shared numbers, where
+the L2 serves repeated pages, sit under roofline.shared.
 `--impl reference` times the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -98,9 +101,9 @@ class ClockSampler:
 def make_batch(workload: str, rank: int, noshare: bool = False):
     from paper_2606_04302_b200 import workloads as W
     idx = int(workload[3:])
-    if idx == 5:
-        return W.config5()
     kw = dict(noshare=True) if noshare else {}
+    if idx == 5:
+        return W.config5(**kw)
     b = W.CONFIGS[idx](**kw)
     if rank:
         # weak scaling: every rank owns a batch of the same shape drawn from its own seed
@@ -184,7 +187,8 @@ class GpuJob:
         self.flush_buf.fill_(1)
         self.sweep_buf.sum()
 
-    def run(self, ev_mid=None):
+    def run(self, ev_mid=None, call_evs=None):
+        """call_evs: list that receives one (start, end) event pair per attention call (separate calls only)."""
         B, dev = self.B, self.dev
         for rec in self.timed:
             B.lazy_cache_write(dev.handle, rec["k_new"], rec["v_new"], rec["slots"], dev.k_pool, dev.v_pool)
@@ -201,12 +205,42 @@ class GpuJob:
                               out_decode=rd["out"])
             return
         for rec in self.timed:
+            if call_evs is not None:
+                e0 = torch.cuda.Event(enable_timing=True); e0.record()
             if rec["step"].kind == "decode":
                 B.lazy_attn_decode(dev.handle, rec["q"], dev.k_pool, dev.v_pool, rec["bt"], rec["pp"], rec["sl"],
                                    rec["out"])
             else:
                 B.lazy_attn_prefill(dev.handle, rec["q"], dev.k_pool, dev.v_pool, rec["bt"], rec["pp"], rec["sl"],
                                     rec["cu"], rec["max_q"], rec["out"])
+            if call_evs is not None:
+                e1 = torch.cuda.Event(enable_timing=True); e1.record()
+                call_evs.append((rec["step"].kind, e0, e1))
+
+    def time_calls(self, steps, warmup):
+        """Per attention call (separate calls), L2 flushed before EVERY call: {kind: mean kernel ms}."""
+        keep = getattr(self, "separate_calls", False)
+        self.separate_calls = True
+        try:
+            acc = {}
+            for i in range(warmup + steps):
+                for rec in self.timed:
+                    self.B.lazy_cache_write(self.dev.handle, rec["k_new"], rec["v_new"], rec["slots"], self.dev.k_pool,
+                                            self.dev.v_pool)
+                evs = []
+                for rec in self.timed:
+                    self.flush_l2()
+                    one = GpuJob.__new__(GpuJob)
+                    one.__dict__.update(self.__dict__)
+                    one.timed = [dict(rec, k_new=rec["k_new"][:0], v_new=rec["v_new"][:0], slots=rec["slots"][:0])]
+                    one.run(call_evs=evs)
+                torch.cuda.synchronize()
+                if i >= warmup:
+                    for kind, e0, e1 in evs:
+                        acc.setdefault(kind, []).append(e0.elapsed_time(e1))
+            return {k: float(np.mean(v)) for k, v in acc.items()}
+        finally:
+            self.separate_calls = keep
 
     def time_steps(self, steps, warmup, barrier):
         for _ in range(warmup):
@@ -224,35 +258,43 @@ class GpuJob:
         attn = sum(e[1].elapsed_time(e[2]) for e in evs)
         return total, attn, self.dev.handle.launch_count() - n0
 
-    # -------- end to end through lazy_host_step (HOST buffers; copies inside the timed region)
+    # -------- end to end through lazy_host_step_packed (HOST buffers; copies inside the timed region)
     def prepare_e2e(self):
+        """Every step's inputs live in ONE pinned host block laid out by lazy_host_step_layout (where a serving engine's
+        scheduler would write them): the step is one H2D copy, the kernels, one D2H copy of the outputs."""
         B, dev = self.B, self.dev
-        pin = lambda t: t.contiguous().pin_memory()
         self.e2e = []
         for rec in self.timed:
             st = rec["step"]
             bt = self.batch.block_table if st.req_ids is None else self.batch.block_table[st.req_ids]
             pp = self.batch.page_logical_pos if st.req_ids is None else self.batch.page_logical_pos[st.req_ids]
             R, tq, nn = st.seq_lens.shape[0], st.q.shape[0], st.k_new.shape[0]
-            host = dict(q=pin(st.q), k=pin(st.k_new), v=pin(st.v_new), s=pin(st.slot_mapping), bt=pin(bt), pp=pin(pp),
-                        sl=pin(st.seq_lens), cu=pin(st.cu_q_lens), out=torch.empty_like(st.q).pin_memory())
-            nbytes = B.lazy_host_step_staging_bytes(dev.handle, R, tq, nn)
-            staging = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev.device)
-            base = (staging.data_ptr() + 255) // 256 * 256
+            lay = B.lazy_host_step_layout(dev.handle, R, tq, nn)
+            packed = torch.zeros(int(lay.in_bytes), dtype=torch.uint8).pin_memory()
+            h2d = 0
+
+            def put(off, t):
+                nonlocal h2d
+                raw = t.contiguous().view(torch.uint8).reshape(-1)
+                packed[off:off + raw.numel()] = raw
+                h2d += raw.numel()
+            put(lay.q, st.q); put(lay.k_new, st.k_new); put(lay.v_new, st.v_new); put(lay.slot_mapping, st.slot_mapping)
+            put(lay.block_table, bt.to(torch.int32)); put(lay.page_logical_pos, pp.to(torch.int32))
+            put(lay.seq_lens, st.seq_lens)
             kind = 0 if st.kind == "decode" else 1
-            args = B.HostStep(kind, R, tq, rec.get("max_q", 1), nn, 0, host["q"].data_ptr(), host["k"].data_ptr(),
-                              host["v"].data_ptr(), host["s"].data_ptr(), host["bt"].data_ptr(),
-                              host["pp"].data_ptr(), host["sl"].data_ptr(), host["cu"].data_ptr(),
-                              host["out"].data_ptr(), dev.k_pool.data_ptr(), dev.v_pool.data_ptr(), base, nbytes)
-            h2d = sum(host[k].numel() * host[k].element_size() for k in ("q", "k", "v", "s", "bt", "pp", "sl"))
             if kind == 1:
-                h2d += host["cu"].numel() * 4
-            d2h = host["out"].numel() * 2
-            self.e2e.append(dict(args=args, host=host, staging=staging, h2d=h2d, d2h=d2h))
+                put(lay.cu_q_lens, st.cu_q_lens)
+            out = torch.empty_like(st.q).pin_memory()
+            staging = torch.empty(int(lay.staging_bytes) + 256, dtype=torch.uint8, device=dev.device)
+            base = (staging.data_ptr() + 255) // 256 * 256
+            args = B.HostStepPacked(kind, R, tq, rec.get("max_q", 1), nn, 0, packed.data_ptr(), out.data_ptr(),
+                                    dev.k_pool.data_ptr(), dev.v_pool.data_ptr(), base, int(lay.staging_bytes))
+            self.e2e.append(dict(args=args, packed=packed, out=out, staging=staging, h2d=int(lay.in_bytes),
+                                 h2d_payload=h2d, d2h=out.numel() * 2))
 
     def run_e2e(self):
         for e in self.e2e:
-            self.B.lazy_host_step(self.dev.handle, e["args"])
+            self.B.lazy_host_step_packed(self.dev.handle, e["args"])
 
     def time_e2e(self, steps, warmup, barrier):
         for _ in range(warmup):
@@ -469,6 +511,117 @@ def oracle_sample(workload, batch, budget_s=20.0):
     return v, t_total, "; ".join(desc), O.num_threads()
 
 
+def _timed_job(workload, device, steps, noshare=False, warmup=3):
+    b = make_batch(workload, 0, noshare)
+    j = GpuJob(b, device)
+    w = step_work(b, [r["step"] for r in j.timed])
+    return b, j, w
+
+
+def decode_noshare_leg(workload, device, steps, barrier):
+    b, j, w = _timed_job(workload, device, steps, noshare=True)
+    _, a_ms, _ = j.time_steps(steps, 3, barrier)
+    j.dev.close()
+    return dict(kernel_ms=a_ms / steps, bytes=w["logical_bytes"])
+
+
+def decode_leg(workload, device, steps, peaks, barrier):
+    """Decode config as a side leg: Zipf-shared batch (logical GB/s) and its noshare variant (the HBM fraction)."""
+    b, j, w = _timed_job(workload, device, steps)
+    t_ms, a_ms, _ = j.time_steps(steps, 3, barrier)
+    ub = unique_bytes(b, [r["step"] for r in j.timed])
+    j.dev.close()
+    del j, b
+    torch.cuda.empty_cache()
+    ns = decode_noshare_leg(workload, device, steps, barrier)
+    gb = ns["bytes"] / (ns["kernel_ms"] * 1e-3) / 1e9
+    a = a_ms / steps
+    return {"workload": workload, "bound": "hbm",
+            "noshare": {"kernel_ms": ns["kernel_ms"], "algorithmic_bytes_per_launch": ns["bytes"], "GBps": gb,
+                        "frac_of_hbm_peak": gb / peaks["hbm"], "traffic": ncu_traffic("decode", workload + "_noshare")},
+            "shared": {"kernel_ms": a, "ms_per_step": t_ms / steps, "logical_GBps": w["logical_bytes"] / (a * 1e-3) / 1e9,
+                       "logical_over_hbm_peak": w["logical_bytes"] / (a * 1e-3) / 1e9 / peaks["hbm"],
+                       "unique_GBps": ub / (a * 1e-3) / 1e9, "traffic": ncu_traffic("decode", workload)}}
+
+
+def prefill_leg(workload, device, steps, peaks, barrier, sustained_s=2.0):
+    """Prefill config: burst (L2 flushed between launches, vs the burst peak) and a seconds-long back-to-back run with
+    its own clock record (vs the sustained peak measured under the power cap)."""
+    b, j, w = _timed_job(workload, device, steps)
+    t_ms, a_ms, _ = j.time_steps(steps, 3, barrier)
+    a = a_ms / steps
+    tf = w["flops"] / (a * 1e-3) / 1e12
+    res = {"workload": workload, "bound": "tensor", "kernel_ms": a, "ms_per_step": t_ms / steps, "TFLOPs": tf,
+           "frac_of_bf16_peak": tf / peaks["tensor"], "traffic": ncu_traffic("prefill", workload),
+           "query_tokens_per_s": w["q_tokens"] / (t_ms / steps * 1e-3)}
+    rec = [r for r in j.timed if r["step"].kind == "prefill"][0]
+    call = lambda: j.B.lazy_attn_prefill(j.dev.handle, rec["q"], j.dev.k_pool, j.dev.v_pool, rec["bt"], rec["pp"],
+                                         rec["sl"], rec["cu"], rec["max_q"], rec["out"])
+    n = max(50, int(sustained_s * 1e3 / a))
+    sampler = ClockSampler(torch.cuda.current_device())
+    sampler.start()
+    for _ in range(20):
+        call()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(n):
+        call()
+    e1.record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / n
+    tfs = w["flops"] / (ms * 1e-3) / 1e12
+    res["sustained"] = {"launches": n, "seconds": ms * n * 1e-3, "kernel_ms": ms, "TFLOPs": tfs,
+                        "frac_of_bf16_sustained": tfs / peaks["tensor_sustained"],
+                        "frac_of_bf16_peak": tfs / peaks["tensor"], "clocks": clocks,
+                        "note": "back-to-back launches, no L2 flush (the K/V working set of 1.1 GB exceeds the L2)"}
+    j.dev.close()
+    return res
+
+
+def cfg5_leg(device, steps, peaks, job=None):
+    """configs[4], kernel by kernel (separate calls, L2 flushed before each): the block-local prefill of the 4 miss
+    documents (tensor roofline; 464 one-CTA work items = 232 CTA pairs on 74 SM pairs, causal: 1..8 KV tiles per pair)
+    and the decode of the 16 running requests (HBM roofline, on the noshare variant), plus the mixed-step time."""
+    own = job is None
+    if own:
+        b, job, _ = _timed_job("cfg5", device, steps)
+    per = job.time_calls(steps, 3)
+    works = {r["step"].kind: step_work(job.batch, [r["step"]]) for r in job.timed}
+    t_ms, a_ms, _ = job.time_steps(steps, 3, lambda: None)
+    if own:
+        job.dev.close()
+        del job
+        torch.cuda.empty_cache()
+    bn, jn, _ = _timed_job("cfg5", device, steps, noshare=True)
+    per_ns = jn.time_calls(steps, 3)
+    wn = {r["step"].kind: step_work(bn, [r["step"]]) for r in jn.timed}
+    jn.dev.close()
+    tf = works["prefill"]["flops"] / (per["prefill"] * 1e-3) / 1e12
+    sh = bn.shape
+    grp = sh.num_q_heads // sh.num_kv_heads
+    tpt = 128 // grp
+    pst = [r["step"] for r in jn.timed if r["step"].kind == "prefill"][0]
+    nq = (pst.cu_q_lens[1:] - pst.cu_q_lens[:-1]).numpy()
+    pairs = int(sum(-(-int(n) // (4 * tpt)) for n in nq)) * sh.num_kv_heads
+    occ = (f"{pairs} CTA pairs ({len(nq)} documents x {sh.num_kv_heads} kv heads x blocks of {4 * tpt} query tokens) on 74 SM "
+           f"pairs, one pair per SM pair; causal: a pair runs 1..{-(-int(nq.max()) // 128)} KV tiles; {tpt * grp} of 128 rows "
+           f"of a Q tile used (group {grp})")
+    gb_ns = wn["decode"]["logical_bytes"] / (per_ns["decode"] * 1e-3) / 1e9
+    gb_sh = works["decode"]["logical_bytes"] / (per["decode"] * 1e-3) / 1e9
+    return {"workload": "cfg5",
+            "prefill": {"bound": "tensor", "kernel_ms": per["prefill"], "flops_per_launch": works["prefill"]["flops"],
+                        "TFLOPs": tf, "frac_of_bf16_peak": tf / peaks["tensor"],
+                        "occupancy": occ},
+            "decode_noshare": {"bound": "hbm", "kernel_ms": per_ns["decode"], "bytes": wn["decode"]["logical_bytes"],
+                               "GBps": gb_ns, "frac_of_hbm_peak": gb_ns / peaks["hbm"]},
+            "decode_shared": {"kernel_ms": per["decode"], "logical_GBps": gb_sh,
+                              "logical_over_hbm_peak": gb_sh / peaks["hbm"]},
+            "mixed_step_ms": t_ms / steps, "mixed_attention_ms": a_ms / steps,
+            "separate_kernels_sum_ms": per["prefill"] + per["decode"]}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -568,29 +721,44 @@ def main():
     value, e2e_value = value1 * world, e2e1 * world           # whole-job aggregate (weak scaling: same work per rank)
 
     wl_name = args.workload + ("_noshare" if args.noshare else "")
-    if args.workload in ("cfg2", "cfg4", "cfg5"):
-        ach = work["logical_bytes"] / (ms_attn * 1e-3) / 1e9 if args.workload != "cfg5" else None
     roof = None
     if args.workload in ("cfg2", "cfg4"):
+        # The HBM roofline of the decode kernel is taken on the `noshare` variant of the workload (every drawn
+        # document distinct: algorithmic bytes == distinct bytes == DRAM bytes).  On the Zipf-shared batch the L2
+        # serves the repeated pages, so logical bytes / time can exceed the HBM peak: reported under "shared".
         ub = unique_bytes(batch, [r["step"] for r in job.timed])
+        shared = {"kernel_ms": ms_attn, "logical_bytes_per_launch": work["logical_bytes"],
+                  "logical_GBps": work["logical_bytes"] / (ms_attn * 1e-3) / 1e9,
+                  "logical_over_hbm_peak": work["logical_bytes"] / (ms_attn * 1e-3) / 1e9 / peaks["hbm"],
+                  "unique_bytes_per_launch": ub, "unique_GBps": ub / (ms_attn * 1e-3) / 1e9,
+                  "traffic": ncu_traffic("decode", args.workload)}
+        if args.noshare:
+            ns = dict(kernel_ms=ms_attn, bytes=work["logical_bytes"])
+        else:
+            ns = decode_noshare_leg(args.workload, device, max(5, args.steps // 2), barrier)
+        ach = ns["bytes"] / (ns["kernel_ms"] * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": "lazy_attn_decode (split-KV + combine)", "achieved": ach,
                 "peak": peaks["hbm"], "unit": "GB/s", "frac": ach / peaks["hbm"],
-                "traffic": ncu_traffic("decode", wl_name),
-                "note": ("algorithmic bytes = K and V once per (token, kv head) per request; with Zipf page sharing the "
-                         "L2 serves repeats, so achieved can exceed the HBM peak -- the HBM-bound fraction is the "
-                         "noshare variant's (logical == unique == DRAM bytes), reported under decode_noshare"),
-                "peak_source": peaks["source"], "algorithmic_bytes_per_launch": work["logical_bytes"],
-                "unique_bytes_per_launch": ub, "achieved_unique": ub / (ms_attn * 1e-3) / 1e9,
-                "kernel_ms": ms_attn}
+                "traffic": ncu_traffic("decode", args.workload + "_noshare"), "peak_source": peaks["source"],
+                "workload": args.workload + " noshare (every drawn document distinct: algorithmic == DRAM bytes)",
+                "algorithmic_bytes_per_launch": ns["bytes"], "kernel_ms": ns["kernel_ms"]}
+        if not args.noshare:
+            roof["shared"] = shared
     elif args.workload == "cfg3":
         ach = work["flops"] / (ms_attn * 1e-3) / 1e12
         roof = {"bound": "tensor", "kernel": "lazy_attn_prefill", "achieved": ach, "peak": peaks["tensor"],
                 "unit": "TFLOP/s", "frac": ach / peaks["tensor"], "traffic": ncu_traffic("prefill", wl_name),
-                "peak_source": peaks["source"],
+                "peak_source": peaks["source"] + " (burst: the kernel is timed alone, L2 flushed between launches)",
                 "algorithmic_flops_per_launch": work["flops"], "kernel_ms": ms_attn}
     else:
-        roof = {"bound": "hbm", "kernel": "mixed step (prefill + decode)", "achieved": None, "peak": peaks["hbm"],
-                "unit": "GB/s", "frac": None, "traffic": None, "kernel_ms": ms_attn}
+        # mixed step: the dominant kernel by bytes is the decode kernel; both kernels are reported per call
+        leg = cfg5_leg(device, max(5, args.steps // 2), peaks, job=job)
+        d = leg["decode_noshare"]
+        roof = {"bound": "hbm", "kernel": "lazy_attn_decode (split-KV + combine) of the mixed step",
+                "achieved": d["GBps"], "peak": peaks["hbm"], "unit": "GB/s", "frac": d["frac_of_hbm_peak"],
+                "traffic": ncu_traffic("decode", "cfg5_noshare"), "peak_source": peaks["source"],
+                "workload": "cfg5 decode requests, noshare variant", "kernel_ms": d["kernel_ms"],
+                "algorithmic_bytes_per_launch": d["bytes"], "step": leg}
 
     out = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -607,7 +775,8 @@ def main():
         "roofline": roof,
         "e2e": {"value": e2e_value, "unit": unit, "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": int(sum(e["h2d"] for e in job.e2e)),
-                "d2h_bytes_per_step": int(sum(e["d2h"] for e in job.e2e))},
+                "d2h_bytes_per_step": int(sum(e["d2h"] for e in job.e2e)),
+                "api": "lazy_host_step_packed: one H2D copy of the packed inputs, the kernels, one D2H copy"},
         "gpu_launches": int(launches), "clocks": clocks,
     }
     if args.mixed and rank == 0 and world == 1 and args.workload == "cfg5":
@@ -671,32 +840,19 @@ def main():
     torch.cuda.empty_cache()
 
     if rank == 0 and world == 1 and not args.no_secondary and args.workload == "cfg2":
-        # side measurements in the same run: the prefill headline (configs[2]) and the noshare decode variant
+        # side measurements in the same run, so that the driver's record carries all five configs: the prefill headline
+        # (configs[2]) as a burst and as a seconds-long run, the long-context decode (configs[3]) and the mixed step
+        # (configs[4]) kernel by kernel.  configs[0] is the parity-test case.
         side = {}
-        for name, wl, ns in (("decode_noshare", "cfg2", True), ("prefill", "cfg3", False)):
+        for name, fn in (("cfg3", lambda: prefill_leg("cfg3", device, max(5, args.steps // 3), peaks, barrier)),
+                         ("cfg4", lambda: decode_leg("cfg4", device, max(5, args.steps // 2), peaks, barrier)),
+                         ("cfg5", lambda: cfg5_leg(device, max(5, args.steps // 2), peaks))):
             try:
-                b2 = make_batch(wl, 0, ns)
-                j2 = GpuJob(b2, device)
-                w2 = step_work(b2, [r["step"] for r in j2.timed])
-                k = max(5, args.steps // 3)
-                t_ms, a_ms, _ = j2.time_steps(k, 3, barrier)
-                a = a_ms / k
-                if wl == "cfg3":
-                    tf = w2["flops"] / (a * 1e-3) / 1e12
-                    side[name] = {"workload": "cfg3", "kernel_ms": a, "ms_per_step": t_ms / k, "TFLOPs": tf,
-                                  "frac_of_bf16_peak": tf / peaks["tensor"],
-                                  "frac_of_bf16_sustained": tf / peaks["tensor_sustained"],
-                                  "query_tokens_per_s": w2["q_tokens"] / (t_ms / k * 1e-3)}
-                else:
-                    gb = w2["logical_bytes"] / (a * 1e-3) / 1e9
-                    side[name] = {"workload": "cfg2 noshare", "kernel_ms": a, "GBps": gb,
-                                  "frac_of_hbm_peak": gb / peaks["hbm"]}
-                j2.dev.close()
-                del j2, b2
-                torch.cuda.empty_cache()
+                side[name] = fn()
             except Exception as e:  # a side measurement must not lose the headline
                 side[name] = {"error": repr(e)}
-        out.update(side)
+            torch.cuda.empty_cache()
+        out["configs"] = side
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, t, sample, cores = oracle_sample(args.workload, batch)

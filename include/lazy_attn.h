@@ -231,6 +231,36 @@ size_t lazy_host_step_staging_bytes(const lazy_handle* h, int32_t num_reqs, int3
                                     int32_t num_new_tokens);
 int lazy_host_step(lazy_handle* h, const lazy_host_step_args* a, void* stream);
 
+/* d'. The same step with the inputs PACKED by the caller into one pinned host block laid out like the device staging
+ * area, so that the whole step costs ONE host-to-device copy, the kernels and ONE device-to-host copy (with seven
+ * separate copies of a few KB to 1 MB each, copy issue latency -- not bandwidth -- was half of cfg 2's end-to-end
+ * time).  lazy_host_step_layout fills the byte offsets of each section inside the block (all 256-byte aligned; a
+ * section the step does not use keeps its slot) and `in_bytes`, the length of the single H2D copy; the output section
+ * starts at `out` in the DEVICE staging area only (h_out is a separate host buffer).  Sections hold exactly what the
+ * h_* pointers of lazy_host_step_args hold.  Returns LAZY_ERR_INVALID on bad counts. */
+typedef struct lazy_host_step_layout_t {
+  size_t q, k_new, v_new, slot_mapping, block_table, page_logical_pos, seq_lens, cu_q_lens, out;
+  size_t in_bytes;           /* bytes of the packed host block == offset of `out`            */
+  size_t staging_bytes;      /* == lazy_host_step_staging_bytes(...)                        */
+} lazy_host_step_layout_t;
+int lazy_host_step_layout(const lazy_handle* h, int32_t num_reqs, int32_t total_q, int32_t num_new_tokens,
+                          lazy_host_step_layout_t* out);
+typedef struct lazy_host_step_packed_args {
+  int32_t kind;              /* 0 = decode, 1 = prefill                                   */
+  int32_t num_reqs;
+  int32_t total_q;
+  int32_t max_q_len;
+  int32_t num_new_tokens;
+  int32_t reserved;
+  const void* h_packed;      /* HOST (pinned), in_bytes long, laid out per lazy_host_step_layout */
+  void* h_out;               /* HOST, [total_q][Hq][D] bf16                                */
+  void* d_k_cache;
+  void* d_v_cache;
+  void* d_staging;           /* DEVICE scratch, 256-byte aligned, >= staging_bytes          */
+  size_t staging_bytes;
+} lazy_host_step_packed_args;
+int lazy_host_step_packed(lazy_handle* h, const lazy_host_step_packed_args* a, void* stream);
+
 /* f4. One serving step's attention for a MIXED batch: the block-local prefill of cache-miss documents (or any
  * prefill chunk) and the decode of the running requests, issued together (Fig. 5 phases 1-3 happen in one
  * engine step).  Same results as lazy_attn_prefill followed by lazy_attn_decode; the two

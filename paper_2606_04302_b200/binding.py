@@ -21,7 +21,8 @@ LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
            "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_alibi_slopes", "lazy_set_page_stored_pos",
-           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step", "lazy_attn_mixed", "lazy_debug_validate",
+           "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step", "lazy_host_step_layout", "lazy_host_step_packed",
+           "lazy_attn_mixed", "lazy_debug_validate",
            "lazy_pool_create", "lazy_pool_destroy", "lazy_pool_acquire", "lazy_pool_release", "lazy_pool_stats",
            "lazy_hit_ratio_model"]
 LAZY_POOL_AGNOSTIC, LAZY_POOL_POSITION_AWARE = 0, 1
@@ -75,6 +76,10 @@ def lib() -> ctypes.CDLL:
         L.lazy_host_step_staging_bytes.argtypes = [vp, i32, i32, i32]
         L.lazy_host_step.restype = ctypes.c_int
         L.lazy_host_step.argtypes = [vp, ctypes.POINTER(HostStep), vp]
+        L.lazy_host_step_layout.restype = ctypes.c_int
+        L.lazy_host_step_layout.argtypes = [vp, i32, i32, i32, ctypes.POINTER(HostStepLayout)]
+        L.lazy_host_step_packed.restype = ctypes.c_int
+        L.lazy_host_step_packed.argtypes = [vp, ctypes.POINTER(HostStepPacked), vp]
         L.lazy_attn_mixed.restype = ctypes.c_int
         L.lazy_attn_mixed.argtypes = [vp, ctypes.POINTER(MixedArgs), vp, vp, vp]
         L.lazy_debug_validate.restype = i64
@@ -272,6 +277,20 @@ def lazy_attn_mixed(h: LazyHandle, k_cache, v_cache, *, q_prefill, block_table_p
         raise LazyError("lazy_attn_mixed", rc)
 
 
+class HostStepLayout(ctypes.Structure):
+    """Mirror of lazy_host_step_layout_t: byte offsets of the sections of the packed host block."""
+    _fields_ = [(n, ctypes.c_size_t) for n in ("q", "k_new", "v_new", "slot_mapping", "block_table", "page_logical_pos",
+                                               "seq_lens", "cu_q_lens", "out", "in_bytes", "staging_bytes")]
+
+
+class HostStepPacked(ctypes.Structure):
+    """Mirror of lazy_host_step_packed_args."""
+    _fields_ = [("kind", ctypes.c_int32), ("num_reqs", ctypes.c_int32), ("total_q", ctypes.c_int32),
+                ("max_q_len", ctypes.c_int32), ("num_new_tokens", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("h_packed", ctypes.c_void_p), ("h_out", ctypes.c_void_p), ("d_k_cache", ctypes.c_void_p),
+                ("d_v_cache", ctypes.c_void_p), ("d_staging", ctypes.c_void_p), ("staging_bytes", ctypes.c_size_t)]
+
+
 class HostStep(ctypes.Structure):
     """Mirror of lazy_host_step_args (include/lazy_attn.h): one serving step with HOST buffers."""
     _fields_ = [("kind", ctypes.c_int32), ("num_reqs", ctypes.c_int32), ("total_q", ctypes.c_int32),
@@ -292,6 +311,20 @@ def lazy_host_step(h: LazyHandle, args: HostStep, stream=None) -> None:
     rc = lib().lazy_host_step(h.ptr, ctypes.byref(args), _stream(stream))
     if rc != 0:
         raise LazyError("lazy_host_step", rc)
+
+
+def lazy_host_step_layout(h: LazyHandle, num_reqs: int, total_q: int, num_new_tokens: int) -> "HostStepLayout":
+    out = HostStepLayout()
+    rc = lib().lazy_host_step_layout(h.ptr, num_reqs, total_q, num_new_tokens, ctypes.byref(out))
+    if rc != 0:
+        raise LazyError("lazy_host_step_layout", rc)
+    return out
+
+
+def lazy_host_step_packed(h: LazyHandle, args: "HostStepPacked", stream=None) -> None:
+    rc = lib().lazy_host_step_packed(h.ptr, ctypes.byref(args), _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_host_step_packed", rc)
 
 
 class LazyPool:

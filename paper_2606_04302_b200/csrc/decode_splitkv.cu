@@ -64,15 +64,6 @@ struct DecodeCfg {
   static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGES * 8 + 16 + 1024;  // + alignment slack
 };
 
-// Optional timeline probe (compile with -DLAZY_TRACE): every CTA records %globaltimer (ns) at a few points.
-#ifdef LAZY_TRACE
-__device__ long long g_dtrace[1024 * 8];
-__device__ __forceinline__ long long gtime() { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t; }
-#define LAZY_DT(slot) do { g_dtrace[blockIdx.x * 8 + (slot)] = gtime(); } while (0)
-#else
-#define LAZY_DT(slot) do { } while (0)
-#endif
-
 struct DecodeArgs {
   const __nv_bfloat16* q;
   const int* block_table;
@@ -112,7 +103,6 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
   int* s_flag = reinterpret_cast<int*>(smem + C::OFF_BAR + 2 * C::NSTAGES * 8);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  if (tid == 0) LAZY_DT(0);
   const int R = a.num_reqs;
   const int hg = blockIdx.y;                       // kv-head group of this CTA
   const int HG = gridDim.y;
@@ -166,7 +156,6 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
     }
   }
   __syncthreads();
-  if (tid == 0) LAZY_DT(1);
 
   const long long U = s_cum[R];
   if (U < G) G = (int)U;
@@ -350,7 +339,6 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
       const int stage = it % C::NSTAGES;
       const uint32_t parity = (it / C::NSTAGES) & 1;
       ptx::mbar_wait(bar_full + 8 * stage, parity);
-      if (tid == 0 && it == 0) LAZY_DT(2);
       const int p = ul * C::PPS + pl;
       const int nv = min(kPageSize, L - p * kPageSize);      // valid tokens of this page (<= 0: no page)
       if (nv > 0) {
@@ -461,7 +449,6 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
       if (lane == 0) ptx::mbar_arrive(bar_empty + 8 * stage);
     }
 
-    if (tid == 0) LAZY_DT(3);                       // (last) segment's page loop done
     // ---- segment done: this warp's partial (o, m, l) for its kv head -> workspace (a8)
 #pragma unroll
     for (int o = 4; o < 32; o <<= 1) {
@@ -545,19 +532,10 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
       }
     }
     ptx::named_bar_sync(1, kConsumerWarps * 32);    // s_flag is reused by the next segment
-    if (tid == 0) LAZY_DT(4);                       // (last) segment's partial write / combine done
     u = s_cum[r] + seg_hi;
     ++r;
   }
 }
-
-#ifdef LAZY_TRACE
-}  // namespace
-extern "C" int lazy_debug_decode_trace(long long* host_out) {
-  return cudaMemcpyFromSymbol(host_out, g_dtrace, sizeof(long long) * 1024 * 8) == cudaSuccess ? 0 : -1;
-}
-namespace {
-#endif
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,

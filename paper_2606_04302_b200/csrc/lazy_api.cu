@@ -400,3 +400,43 @@ extern "C" int lazy_host_step(lazy_handle* h, const lazy_host_step_args* a, void
     return LAZY_ERR_CUDA;
   return LAZY_OK;
 }
+
+
+extern "C" int lazy_host_step_layout(const lazy_handle* h, int32_t num_reqs, int32_t total_q, int32_t num_new_tokens,
+                                     lazy_host_step_layout_t* out) {
+  if (!h || !out || num_reqs < 0 || total_q < 0 || num_new_tokens < 0) return LAZY_ERR_INVALID;
+  const StagePlan p = stage_plan(h, num_reqs, total_q, num_new_tokens);
+  out->q = p.q; out->k_new = p.k_new; out->v_new = p.v_new; out->slot_mapping = p.slots;
+  out->block_table = p.bt; out->page_logical_pos = p.pp; out->seq_lens = p.sl; out->cu_q_lens = p.cu;
+  out->out = p.out; out->in_bytes = p.out; out->staging_bytes = p.total;
+  return LAZY_OK;
+}
+
+extern "C" int lazy_host_step_packed(lazy_handle* h, const lazy_host_step_packed_args* a, void* stream) {
+  if (!h || !a) return LAZY_ERR_INVALID;
+  if (a->num_reqs < 0 || a->total_q < 0 || a->num_new_tokens < 0) return LAZY_ERR_INVALID;
+  if (a->num_reqs == 0 || a->total_q == 0) return LAZY_OK;
+  if (!a->h_packed || !a->h_out || !a->d_k_cache || !a->d_v_cache || !a->d_staging) return LAZY_ERR_INVALID;
+  const StagePlan p = stage_plan(h, a->num_reqs, a->total_q, a->num_new_tokens);
+  if ((reinterpret_cast<uintptr_t>(a->d_staging) & 255u) || a->staging_bytes < p.total) return LAZY_ERR_WORKSPACE;
+  cudaStream_t s = static_cast<cudaStream_t>(stream);
+  char* d = static_cast<char*>(a->d_staging);
+  if (cudaMemcpyAsync(d, a->h_packed, p.out, cudaMemcpyHostToDevice, s) != cudaSuccess) return LAZY_ERR_CUDA;
+  int rc = LAZY_OK;
+  if (a->num_new_tokens > 0)
+    rc = lazy_cache_write(h, d + p.k_new, d + p.v_new, reinterpret_cast<const int64_t*>(d + p.slots),
+                          a->num_new_tokens, a->d_k_cache, a->d_v_cache, stream);
+  if (rc != LAZY_OK) return rc;
+  if (a->kind == 1)
+    rc = lazy_attn_prefill(h, d + p.q, a->d_k_cache, a->d_v_cache, reinterpret_cast<const int32_t*>(d + p.bt),
+                           reinterpret_cast<const int32_t*>(d + p.pp), reinterpret_cast<const int32_t*>(d + p.sl),
+                           reinterpret_cast<const int32_t*>(d + p.cu), a->num_reqs, a->total_q, a->max_q_len,
+                           d + p.out, stream);
+  else
+    rc = lazy_attn_decode(h, d + p.q, a->d_k_cache, a->d_v_cache, reinterpret_cast<const int32_t*>(d + p.bt),
+                          reinterpret_cast<const int32_t*>(d + p.pp), reinterpret_cast<const int32_t*>(d + p.sl),
+                          a->num_reqs, d + p.out, stream);
+  if (rc != LAZY_OK) return rc;
+  if (cudaMemcpyAsync(a->h_out, d + p.out, p.q_bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) return LAZY_ERR_CUDA;
+  return LAZY_OK;
+}

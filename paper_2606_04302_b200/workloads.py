@@ -269,7 +269,7 @@ def config4(scale: float = 1.0, **kw) -> LazyBatch:
                           prefill_question=False, **kw)
 
 
-def config5(scale: float = 1.0, q_scale: float = 1.0) -> LazyBatch:
+def config5(scale: float = 1.0, q_scale: float = 1.0, noshare: bool = False) -> LazyBatch:
     """Mixed serving step (Hq=28, Hkv=4, theta 1e6): 16 decode requests over 20 cached docs x 512
     (pool 2000, Zipf 0.8) + 4 cache-miss docs x 1024 prefilled block-locally (positions from 0, causal)
     and written un-rotated into new pages.  Steps: prefill (writes the 4 miss documents, then attends
@@ -285,7 +285,7 @@ def config5(scale: float = 1.0, q_scale: float = 1.0) -> LazyBatch:
     miss_pages = (miss_len + P - 1) // P
     dec = make_rag_batch("cfg5_mixed", shape, seed=seed, pool_docs=pool, doc_len=512, num_reqs=R_dec,
                          docs_per_req=20, alpha=0.8, replace=False, question_len=0, decode=True,
-                         prefill_question=False, q_scale=q_scale)
+                         prefill_question=False, q_scale=q_scale, noshare=noshare)
     gen = torch.Generator().manual_seed(seed + 1000)
     base_pages = dec.num_pages
     # new pages: miss documents + 1 private page for the follow-up request's decode token
