@@ -18,7 +18,7 @@ struct PrefillArgs {
   const float* alibi;      // kKmAlibi: [Hq] slopes * log2(e)
   int num_reqs;
   int q_interleaved;    // LAZY_ROPE_INTERLEAVED: q arrives with pairs (2j, 2j+1); de-interleaved while it is rotated
-  int mblocks;          // CTAs per (request, kv head)
+  int mblocks;          // CTAs (pair kernel: CTA pairs) per (request, kv head)
   int tokens_per_tile;  // 128 / group
   Shape sh;
 };

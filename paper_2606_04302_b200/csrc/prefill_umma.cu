@@ -376,12 +376,19 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     const int lim_min = max(0, L - n_q + min(i0 + t * TPT, n_q - 1));
 
     // ---- Q tile: rotate by the query position, fold in log2(e)/sqrt(D), in place ----------------------------
+    // the row's cos/sin (one table row: D/4 16-byte chunks) is fetched BEFORE waiting for the Q tile, all loads in
+    // flight at once: chunk by chunk behind the wait, the dependent global loads cost ~3 us per CTA
+    float4 csr[D / 4];
+    if (valid && KM != kKmAlibi) {
+      const int pos = ppos[sq / kPageSize] + sq % kPageSize;
+      const float4* p = reinterpret_cast<const float4*>(a.cs + (size_t)pos * (D / 2));
+#pragma unroll
+      for (int x = 0; x < D / 4; ++x) csr[x] = __ldg(p + x);
+    }
     ptx::mbar_wait(bar(B_QFULL + t), 0);
     {
       const uint32_t qb = sQ + t * C::TILE_BYTES;
       if (valid) {
-        const int pos = ppos[sq / kPageSize] + sq % kPageSize;
-        const float2* cs_row = a.cs + (size_t)pos * (D / 2);
         uint4 src[2 * C::CPR];                      // LAZY_ROPE_INTERLEAVED: the whole row first (in-place hazard)
         if (a.q_interleaved) {
 #pragma unroll
@@ -394,9 +401,12 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 #pragma unroll
             for (int e = 0; e < 8; ++e) { co[e] = sh.scale_log2; si[e] = 0.f; }
           } else {
-            load_cs8<D>(cs_row, c, co, si);
 #pragma unroll
-            for (int e = 0; e < 8; ++e) { co[e] *= sh.scale_log2; si[e] *= sh.scale_log2; }
+            for (int x = 0; x < 4; ++x) {
+              const float4 v = csr[cs_f4_index<D>(c, x)];
+              co[2 * x] = v.x * sh.scale_log2; co[2 * x + 1] = v.y * sh.scale_log2;
+              si[2 * x] = v.z * sh.scale_log2; si[2 * x + 1] = v.w * sh.scale_log2;
+            }
           }
           const uint32_t pa = qb + chunk_off(row, c), pb = qb + chunk_off(row, c + C::CPR);
           uint4 va, vb;
