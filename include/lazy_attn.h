@@ -145,7 +145,10 @@ int lazy_attn_prefill(lazy_handle* h, const void* q, const void* k_cache, const 
 
 /* Decode: one query per request (its last token) over the whole sequence (Fig. 3c;
  * T_decode ~ 2LD/B, L204-209).  Split-KV flash-decoding with an in-kernel combine.
- *   q, out : [num_reqs][Hq][D] bf16.  Other arguments as for prefill. */
+ *   q, out : [num_reqs][Hq][D] bf16.  Other arguments as for prefill.
+ * ONE decode call in flight per handle: the split-KV partials, the per-request arrival counters and the scheduling
+ * words live in the handle's workspace, so a second lazy_attn_decode (or lazy_attn_mixed / lazy_host_step*) on the
+ * same handle may only be enqueued on the SAME stream, behind the first.  Use one handle per concurrent stream. */
 int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                      const int32_t* block_table, const int32_t* page_logical_pos,
                      const int32_t* seq_lens, int32_t num_reqs, void* out, void* stream);

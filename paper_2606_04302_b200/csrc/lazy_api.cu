@@ -262,10 +262,19 @@ int lazy_attn_mixed(lazy_handle* h, const lazy_mixed_args* a, const void* k_cach
     return rc;
   }
   if (!h->side_stream) {
-    if (cudaStreamCreateWithFlags(&h->side_stream, cudaStreamNonBlocking) != cudaSuccess) return LAZY_ERR_CUDA;
-    if (cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&h->ev_join, cudaEventDisableTiming) != cudaSuccess)
+    // all three host resources or none: a half-built set would be used (null events) by the next call
+    cudaStream_t st = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    const bool ok = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&e0, cudaEventDisableTiming) == cudaSuccess &&
+                    cudaEventCreateWithFlags(&e1, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) {
+      if (e1) cudaEventDestroy(e1);
+      if (e0) cudaEventDestroy(e0);
+      if (st) cudaStreamDestroy(st);
       return LAZY_ERR_CUDA;
+    }
+    h->side_stream = st; h->ev_fork = e0; h->ev_join = e1;
   }
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   if (cudaEventRecord(h->ev_fork, s) != cudaSuccess || cudaStreamWaitEvent(h->side_stream, h->ev_fork, 0) != cudaSuccess)

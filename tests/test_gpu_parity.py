@@ -52,7 +52,13 @@ def test_configs_peaked_queries(cfg):
 def test_configs_full_size_sampled(cfg, rows):
     """BASELINE.json sizes, the launch configuration bench.py times; oracle on sampled query rows
     (decode configs have few rows and are compared in full)."""
-    _run(W.CONFIGS[cfg](), sample_rows=rows, seed=cfg)
+    stats = _run(W.CONFIGS[cfg](), sample_rows=rows, seed=cfg)
+    # a correct kernel sits an order of magnitude inside the contract (DESIGN.md "Tolerances": outputs shrink like
+    # sqrt(e/L), bf16 rounding of the rotated operands and of P dominates the error)
+    # (cfg5's block-local prefill has rows that see a handful of keys: outputs of magnitude |v|, whose bf16 rounding
+    # alone is up to 2^-9 * 4 = 8e-3 -- there the mean error is the meaningful gate)
+    max_b, mean_b = {2: (2e-3, 2e-4), 3: (2e-3, 2e-4), 4: (1e-3, 1e-4), 5: (1.5e-2, 5e-4)}[cfg]
+    assert all(s["max_abs"] < max_b and s["mean_abs"] < mean_b for s in stats), stats
 
 
 def test_shift_invariance_gpu():
