@@ -271,7 +271,11 @@ int lazy_host_step_packed(lazy_handle* h, const lazy_host_step_packed_args* a, v
  * stream forked from and joined back into `stream` with events, the prefill kernel (tensor-bound) takes the other
  * SMs and, as decode CTAs retire, theirs too.  No host synchronisation; capturable in a CUDA graph.  The side stream
  * and two events are host-side resources created at the first call and released by lazy_destroy.
- * Field meanings are those of the two calls above; the two request sets use separate tables. */
+ * Field meanings are those of the two calls above; the two request sets use separate tables.
+ * For the product configuration (head_dim 128, un-rotated K, RoPE, 4 or 8 kv heads) the step is ONE launch: the first
+ * `decode_sms` CTAs of the grid run the decode body, CTA pairs behind them the prefill work items (mixed_fused.cu);
+ * decode_sms = 0 picks 7/16 of the SMs (64 of 148).  Bit 0 of `reserved0` forces the two-stream path described above
+ * (the A/B arm); other configurations always take it. */
 typedef struct lazy_mixed_args {
   const void* q_prefill;  const int32_t* block_table_prefill;  const int32_t* page_logical_pos_prefill;
   const int32_t* seq_lens_prefill;  const int32_t* cu_q_lens;

@@ -261,6 +261,25 @@ int lazy_attn_mixed(lazy_handle* h, const lazy_mixed_args* a, const void* k_cach
                             a->seq_lens_decode, a->num_reqs_decode, a->out_decode, stream);
     return rc;
   }
+  if (lazy::mixed_fused_supported(h, a->num_reqs_decode) && !(a->reserved0 & 1)) {
+    // one launch: decode CTAs first, prefill CTA pairs behind them (mixed_fused.cu).  Same argument checks as the
+    // separate calls.
+    int rc = check_attn_args(h, a->q_prefill, k_cache, v_cache, a->block_table_prefill, a->page_logical_pos_prefill,
+                             a->seq_lens_prefill, a->num_reqs_prefill, a->out_prefill);
+    if (rc == LAZY_OK)
+      rc = check_attn_args(h, a->q_decode, k_cache, v_cache, a->block_table_decode, a->page_logical_pos_decode,
+                           a->seq_lens_decode, a->num_reqs_decode, a->out_decode);
+    if (rc != LAZY_OK) return rc;
+    if (a->total_q < 0 || a->max_q_len <= 0 || !a->cu_q_lens || (reinterpret_cast<uintptr_t>(a->cu_q_lens) & 3u))
+      return LAZY_ERR_INVALID;
+    // decode is HBM-bound and saturates the memory system from a fraction of the SMs; the prefill pairs get the rest
+    // (cfg 5 on B200: 142.5 us at 64 decode CTAs, 143.5 at 56, 145.5 at 96, 148 at 128; 177 us as two separate calls)
+    const int n_dec = a->decode_sms > 0 ? (a->decode_sms < h->num_sms ? a->decode_sms : h->num_sms) : h->num_sms * 7 / 16;
+    const int n = lazy::launch_mixed_fused(h, a, k_cache, v_cache, n_dec, static_cast<cudaStream_t>(stream));
+    if (n < 0) return n;
+    h->launches += n;
+    return LAZY_OK;
+  }
   if (!h->side_stream) {
     // all three host resources or none: a half-built set would be used (null events) by the next call
     cudaStream_t st = nullptr;

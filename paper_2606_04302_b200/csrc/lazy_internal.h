@@ -83,6 +83,10 @@ int launch_rowwise(lazy_handle* h, const void* q, const void* k_cache, const voi
 int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                   const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                   int num_reqs, void* out, cudaStream_t stream);
+// one launch for a mixed prefill + decode step (mixed_fused.cu); supported for the product configuration only
+bool mixed_fused_supported(const lazy_handle* h, int num_reqs_decode);
+int launch_mixed_fused(lazy_handle* h, const lazy_mixed_args* m, const void* k_cache, const void* v_cache, int decode_ctas,
+                       cudaStream_t stream);
 int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                    const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                    const int32_t* cu_q_lens, int num_reqs, int total_q, int max_q_len, void* out,
