@@ -294,18 +294,23 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
     }
   } else if (warp >= 8) {
     // ================================ K-rotate warpgroup ======================================================
-    // this CTA's 64 keys of every tile.  thread = (page, group of 4 consecutive tokens, chunk pair c = 8 rotation
-    // pairs): the page's table row w = e^{i p0 theta_j} is read once, composed with the group's first in-page offset,
-    // and the tokens are walked with z <- z * e^{i theta_j} (at most 3 fp32 complex products from a table value).
+    // this CTA's 64 keys of every tile.  thread = (page, token group tg, chunk pair c = 8 rotation pairs): it takes the
+    // tokens tg, tg+4, tg+8, tg+12 of the page.  The page's table row w = e^{i p0 theta_j} is read once, composed with
+    // e^{i tg theta_j}, and the tokens are walked with z <- z * e^{i 4 theta_j} (at most 3 fp32 complex products from
+    // a table value).  Lane -> (c, tg) is chosen so that the 8 lanes of a quarter warp (one shared-memory wavefront of
+    // a 16-byte access) hold the four c of one parity x two ADJACENT tokens: their table chunks are 4 distinct
+    // 16-byte words (broadcast across the two tokens; chunk pairs c and c+1 would collide, they sit 256 B apart), and
+    // their K chunks, swizzled by (row & 7), fall into disjoint bank groups because adjacent rows differ in parity.
     ptx::setmaxnreg_dec<kRegsRotate>();
     constexpr int TOK = 4;
     const int wtid = tid - 256;
     const int i = wtid >> 5;                        // page of this CTA's half tile
-    const int t0 = ((wtid & 31) >> 3) * TOK, c = wtid & 7;
-    float2 u0c[4], u0s[4], u1c[4], u1s[4];          // e^{i t0 theta_j}, e^{i theta_j} for this thread's 8 pairs
+    const int c = 2 * (lane & 3) + ((lane >> 3) & 1);
+    const int tg = ((lane >> 2) & 1) + 2 * (lane >> 4);
+    float2 u0c[4], u0s[4], u1c[4], u1s[4];          // e^{i tg theta_j}, e^{i 4 theta_j} for this thread's 8 pairs
     if (KM == LAZY_K_UNROTATED) {
-      const float4* r0 = reinterpret_cast<const float4*>(a.cs + (size_t)t0 * (D / 2));
-      const float4* r1 = reinterpret_cast<const float4*>(a.cs + (size_t)1 * (D / 2));
+      const float4* r0 = reinterpret_cast<const float4*>(a.cs + (size_t)tg * (D / 2));
+      const float4* r1 = reinterpret_cast<const float4*>(a.cs + (size_t)4 * (D / 2));
 #pragma unroll
       for (int x = 0; x < 4; ++x) {
         const float4 v0 = __ldg(r0 + cs_f4_index<D>(c, x)), v1 = __ldg(r1 + cs_f4_index<D>(c, x));
@@ -329,7 +334,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
           zc[x] = make_float2(f32(v.x), f32(v.y));
           zs[x] = make_float2(f32(v.z), f32(v.w));
         }
-        if (KM == LAZY_K_UNROTATED) {               // first token of the group: z = w * u0
+        if (KM == LAZY_K_UNROTATED) {               // first token of the thread: z = w * u0
 #pragma unroll
           for (int x = 0; x < 4; ++x) {
             const float2 wc = zc[x], ws = zs[x];
@@ -341,19 +346,19 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
 #pragma unroll
           for (int x = 0; x < 4; ++x) zs[x] = __fmul2_rn(zs[x], make_float2(sgn, sgn));
         }
-        const int row0 = i * kPageSize + t0;
+        const int row0 = i * kPageSize + tg;
         uint4 va[TOK], vb[TOK];
 #pragma unroll
         for (int tt = 0; tt < TOK; ++tt) {
-          va[tt] = ptx::lds128(kb + kchunk_off(row0 + tt, c));
-          vb[tt] = ptx::lds128(kb + kchunk_off(row0 + tt, c + 8));
+          va[tt] = ptx::lds128(kb + kchunk_off(row0 + 4 * tt, c));
+          vb[tt] = ptx::lds128(kb + kchunk_off(row0 + 4 * tt, c + 8));
         }
 #pragma unroll
         for (int tt = 0; tt < TOK; ++tt) {
           rotate8_packed(va[tt], vb[tt], zc, zs);
-          ptx::sts128(kb + kchunk_off(row0 + tt, c), va[tt]);
-          ptx::sts128(kb + kchunk_off(row0 + tt, c + 8), vb[tt]);
-          if (KM == LAZY_K_UNROTATED && tt + 1 < TOK) {          // next token: z <- z * e^{i theta_j}
+          ptx::sts128(kb + kchunk_off(row0 + 4 * tt, c), va[tt]);
+          ptx::sts128(kb + kchunk_off(row0 + 4 * tt, c + 8), vb[tt]);
+          if (KM == LAZY_K_UNROTATED && tt + 1 < TOK) {          // next token (4 further): z <- z * e^{i 4 theta_j}
 #pragma unroll
             for (int x = 0; x < 4; ++x) {
               const float2 wc = zc[x], ws = zs[x];
