@@ -60,25 +60,6 @@ __device__ __forceinline__ int cs_f4_index(int c, int x) {
   const int j0 = 8 * c;
   return ((j0 % JT) / 2 + x) * 4 + j0 / JT;
 }
-// (cos, sin) of the 8 rotation pairs j = 8c .. 8c+7 from one table row in global memory / in shared memory.
-template <int D>
-__device__ __forceinline__ void load_cs8(const float2* __restrict__ cs_row, int c, float (&co)[8], float (&si)[8]) {
-  const float4* p = reinterpret_cast<const float4*>(cs_row);
-#pragma unroll
-  for (int x = 0; x < 4; ++x) {
-    float4 v = __ldg(p + cs_f4_index<D>(c, x));
-    co[2 * x] = v.x; co[2 * x + 1] = v.y; si[2 * x] = v.z; si[2 * x + 1] = v.w;
-  }
-}
-template <int D>
-__device__ __forceinline__ void load_cs8_smem(uint32_t row_addr, int c, float (&co)[8], float (&si)[8]) {
-#pragma unroll
-  for (int x = 0; x < 4; ++x) {
-    uint4 v = ptx::lds128(row_addr + 16 * cs_f4_index<D>(c, x));
-    co[2 * x] = f32(v.x); co[2 * x + 1] = f32(v.y); si[2 * x] = f32(v.z); si[2 * x + 1] = f32(v.w);
-  }
-}
-
 // byte offset of 16-byte chunk `ci` (8 dims: 8ci .. 8ci+7) of row `row` inside a 128-row, 128B-swizzled tile
 __device__ __forceinline__ uint32_t chunk_off(int row, int ci) {
   return (ci >> 3) * kHalfBytes + row * 128 + (((ci & 7) ^ (row & 7)) << 4);
