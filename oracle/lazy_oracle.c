@@ -23,7 +23,9 @@
  * only RoPE; scale 1/sqrt(D).
  *
  * Pins: tests/test_oracle_pins.py (brute force, closed forms, shift invariance,
- * SDPA reduction, sharing equivalence, golden worked examples).  No function here is
+ * SDPA reduction, sharing equivalence, golden worked examples) and tests/test_oracle_fp8.py
+ * (FP8 pages: the E4M3 code table, nearest-value and tie rules, round trips, scale closed form,
+ * equality with the pinned fp64 path on dequantised pools).  No function here is
  * "parity unpinned".
  */
 #include <math.h>
@@ -33,6 +35,7 @@
 
 #define DT_F64 0
 #define DT_BF16 1
+#define DT_E4M3 2
 
 /* exact bf16 -> double (bf16 is the top 16 bits of an IEEE fp32) */
 static double bf16_to_double(uint16_t b) {
@@ -42,8 +45,37 @@ static double bf16_to_double(uint16_t b) {
     return (double)f;
 }
 
+/* OCP 8-bit floating point, E4M3 ("FN" flavour: no infinities): bit 7 sign, bits 6-3 exponent E (bias 7), bits 2-0
+ * mantissa M.  E = 0: subnormal, value M/8 * 2^-6.  Otherwise (1 + M/8) * 2^(E-7), except E = 15, M = 7, which is
+ * NaN; the largest finite value is therefore 1.75 * 2^8 = 448 (code 0x7e). */
+double lazy_oracle_e4m3_to_double(uint8_t c) {
+    int E = (c >> 3) & 15, M = c & 7;
+    double v;
+    if (E == 15 && M == 7) return NAN;
+    if (E == 0) v = ldexp((double)M / 8.0, -6);
+    else v = ldexp(1.0 + (double)M / 8.0, E - 7);
+    return (c & 0x80) ? -v : v;
+}
+
+/* Nearest E4M3 code of x: round to nearest, ties to the code with an even mantissa bit, magnitudes beyond 448
+ * saturate to +-448 (never NaN, never infinity); NaN gives the NaN code.  Written as a search over the 127
+ * non-negative finite values (codes 0x00..0x7e are increasing in value), not as bit manipulation. */
+uint8_t lazy_oracle_e4m3_from_float(float x) {
+    if (x != x) return 0x7f;
+    uint8_t sign = (x < 0.0f || (x == 0.0f && 1.0f / x < 0.0f)) ? 0x80 : 0x00;
+    double a = fabs((double)x);
+    if (a >= 448.0) return sign | 0x7e;
+    int c = 0;                                   /* largest code whose value is <= a */
+    while (c < 0x7e && lazy_oracle_e4m3_to_double((uint8_t)(c + 1)) <= a) ++c;
+    double lo = lazy_oracle_e4m3_to_double((uint8_t)c), hi = lazy_oracle_e4m3_to_double((uint8_t)(c + 1));
+    double dl = a - lo, dh = hi - a;             /* exact: fp32 and E4M3 values are dyadic, differences fit in fp64 */
+    if (dh < dl || (dh == dl && (c & 1))) ++c;
+    return sign | (uint8_t)c;
+}
+
 static inline double load_elem(const void* base, int dtype, int64_t idx) {
     if (dtype == DT_BF16) return bf16_to_double(((const uint16_t*)base)[idx]);
+    if (dtype == DT_E4M3) return lazy_oracle_e4m3_to_double(((const uint8_t*)base)[idx]);
     return ((const double*)base)[idx];
 }
 
@@ -240,6 +272,15 @@ int lazy_oracle_attend_paged_stored(const void* q, int dtype_q, const void* k_po
 }
 
 /* ... and with a positional variant (lazy_oracle_variant above). */
+static int attend_paged_impl(const void* q, int dtype_q, const void* k_pool, const void* v_pool,
+                             int dtype_kv, const float* k_scale, const float* v_scale,
+                             const int32_t* block_table, const int32_t* page_logical_pos,
+                             int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
+                             int num_reqs, int Hq, int Hkv, int D, int P, double theta,
+                             int k_storage, const int32_t* page_stored_pos,
+                             int rope_style, const double* inv_freq, double scale, const double* alibi_slopes,
+                             const uint8_t* row_select, double* out);
+
 int lazy_oracle_attend_paged_variant(const void* q, int dtype_q, const void* k_pool, const void* v_pool,
                                      int dtype_kv, const int32_t* block_table, const int32_t* page_logical_pos,
                                      int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
@@ -247,6 +288,39 @@ int lazy_oracle_attend_paged_variant(const void* q, int dtype_q, const void* k_p
                                      int k_storage, const int32_t* page_stored_pos,
                                      int rope_style, const double* inv_freq, double scale, const double* alibi_slopes,
                                      const uint8_t* row_select, double* out) {
+    if (dtype_kv == DT_E4M3) return -1;     /* FP8 pages need their scales: lazy_oracle_attend_paged_fp8 */
+    return attend_paged_impl(q, dtype_q, k_pool, v_pool, dtype_kv, NULL, NULL, block_table, page_logical_pos,
+                             table_stride, seq_lens, cu_q_lens, num_reqs, Hq, Hkv, D, P, theta, k_storage,
+                             page_stored_pos, rope_style, inv_freq, scale, alibi_slopes, row_select, out);
+}
+
+/* FP8 KV pages (the paper's cache holds "purely content-based keys and values", PAPER.md
+ * L108, which is what makes a quantised page shareable at any position; decode traffic is the 2LD of L204-209).
+ * The paper defines no quantised format; the format is this repository's: pages hold OCP FP8 E4M3
+ * codes of the un-rotated K and of V, with one fp32 scale per (page, kv head, token) in k_scale / v_scale
+ * [num_pages][Hkv][P].  The result is DEFINED as: dequantise every element exactly (code value x scale, exact in
+ * fp64), then the unchanged definition above.  Nothing else differs. */
+int lazy_oracle_attend_paged_fp8(const void* q, int dtype_q, const uint8_t* k_codes, const uint8_t* v_codes,
+                                 const float* k_scale, const float* v_scale,
+                                 const int32_t* block_table, const int32_t* page_logical_pos,
+                                 int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
+                                 int num_reqs, int Hq, int Hkv, int D, int P, double theta,
+                                 int rope_style, const double* inv_freq, double scale, const double* alibi_slopes,
+                                 const uint8_t* row_select, double* out) {
+    if (!k_scale || !v_scale) return -1;
+    return attend_paged_impl(q, dtype_q, k_codes, v_codes, DT_E4M3, k_scale, v_scale, block_table, page_logical_pos,
+                             table_stride, seq_lens, cu_q_lens, num_reqs, Hq, Hkv, D, P, theta, 0, NULL,
+                             rope_style, inv_freq, scale, alibi_slopes, row_select, out);
+}
+
+static int attend_paged_impl(const void* q, int dtype_q, const void* k_pool, const void* v_pool,
+                             int dtype_kv, const float* k_scale, const float* v_scale,
+                             const int32_t* block_table, const int32_t* page_logical_pos,
+                             int64_t table_stride, const int32_t* seq_lens, const int32_t* cu_q_lens,
+                             int num_reqs, int Hq, int Hkv, int D, int P, double theta,
+                             int k_storage, const int32_t* page_stored_pos,
+                             int rope_style, const double* inv_freq, double scale, const double* alibi_slopes,
+                             const uint8_t* row_select, double* out) {
     lazy_oracle_variant var;
     var.rope_style = rope_style; var.inv_freq = inv_freq; var.scale = scale; var.alibi_slopes = alibi_slopes;
     if (k_storage < 0 || k_storage > 2 || (k_storage == 1 && !page_stored_pos)) return -1;
@@ -284,9 +358,12 @@ int lazy_oracle_attend_paged_variant(const void* q, int dtype_q, const void* k_p
             else rot[s] = 0.0;
             for (int hk = 0; hk < Hkv; ++hk) {
                 int64_t base = (((int64_t)page * Hkv + hk) * P + t) * D;
+                /* FP8 pages: exact dequantisation, code value x the (page, head, token) scale */
+                double sk = k_scale ? (double)k_scale[((int64_t)page * Hkv + hk) * P + t] : 1.0;
+                double sv = v_scale ? (double)v_scale[((int64_t)page * Hkv + hk) * P + t] : 1.0;
                 for (int d = 0; d < D; ++d) {
-                    kg[((size_t)s * Hkv + hk) * D + d] = load_elem(k_pool, dtype_kv, base + d);
-                    vg[((size_t)s * Hkv + hk) * D + d] = load_elem(v_pool, dtype_kv, base + d);
+                    kg[((size_t)s * Hkv + hk) * D + d] = load_elem(k_pool, dtype_kv, base + d) * sk;
+                    vg[((size_t)s * Hkv + hk) * D + d] = load_elem(v_pool, dtype_kv, base + d) * sv;
                 }
             }
         }
@@ -321,6 +398,47 @@ int lazy_oracle_cache_write(const uint16_t* k_new, const uint16_t* v_new, const 
             int64_t src = (t * Hkv + hk) * D;
             memcpy(k_pool + dst, k_new + src, sizeof(uint16_t) * D);
             memcpy(v_pool + dst, v_new + src, sizeof(uint16_t) * D);
+        }
+    }
+    return 0;
+}
+
+/* lazy_cache_write for FP8 pages: quantise each new (token, kv head) row of K and of V on its own.
+ *   amax  = max_d |x[d]|                        (bf16 inputs, exact)
+ *   scale = amax / 448 in fp32 (round to nearest), or 1 if that is not a positive number (an all-zero row)
+ *   code[d] = nearest E4M3 code of  x[d] / scale  (the quotient formed in fp32, round to nearest)
+ * so the row's largest element lands on +-448, the top of the E4M3 range.  Both decisions that produce integers
+ * (the scale's fp32 bits and the codes) are taken in fp32, the precision the CUDA kernel uses; IEEE division is
+ * correctly rounded on both sides, so codes and scales must agree bit for bit.  Inputs are finite.
+ *   k_new/v_new [T][Hkv][D] bf16 words; code pools [num_pages][Hkv][P][D] bytes; scale pools [num_pages][Hkv][P]. */
+int lazy_oracle_cache_write_fp8(const uint16_t* k_new, const uint16_t* v_new, const int64_t* slot_mapping,
+                                int64_t num_tokens, int Hkv, int D, int P, int64_t num_pages,
+                                uint8_t* k_codes, uint8_t* v_codes, float* k_scale, float* v_scale) {
+    for (int64_t t = 0; t < num_tokens; ++t) {
+        int64_t slot = slot_mapping[t];
+        if (slot < 0) continue;
+        int64_t page = slot / P, off = slot % P;
+        if (page >= num_pages) return -1;
+        for (int hk = 0; hk < Hkv; ++hk) {
+            int64_t dst = ((page * Hkv + hk) * P + off) * D;
+            int64_t src = (t * Hkv + hk) * D;
+            for (int which = 0; which < 2; ++which) {
+                const uint16_t* x = (which ? v_new : k_new) + src;
+                uint8_t* codes = (which ? v_codes : k_codes) + dst;
+                float* sc = (which ? v_scale : k_scale) + (page * Hkv + hk) * P + off;
+                float amax = 0.0f;
+                for (int d = 0; d < D; ++d) {
+                    float a = fabsf((float)bf16_to_double(x[d]));
+                    if (a > amax) amax = a;
+                }
+                volatile float scale = amax / 448.0f;       /* volatile: keep the quotient in fp32 (no excess precision) */
+                if (!(scale > 0.0f)) scale = 1.0f;
+                *sc = scale;
+                for (int d = 0; d < D; ++d) {
+                    volatile float y = (float)bf16_to_double(x[d]) / scale;
+                    codes[d] = lazy_oracle_e4m3_from_float(y);
+                }
+            }
         }
     }
     return 0;

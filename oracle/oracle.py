@@ -179,6 +179,105 @@ def cache_write(k_new, v_new, slot_mapping, k_pool, v_pool, page_size: int) -> N
         raise RuntimeError(f"lazy_oracle_cache_write failed: {rc}")
 
 
+# ---- FP8 KV pages: E4M3 codes + one fp32 scale per (page, kv head, token) -------------------
+def e4m3_to_double(codes) -> np.ndarray:
+    c = np.ascontiguousarray(np.asarray(codes, dtype=np.uint8))
+    f = lib().lazy_oracle_e4m3_to_double
+    f.restype = ctypes.c_double
+    f.argtypes = [ctypes.c_uint8]
+    return np.array([f(int(x)) for x in c.ravel()], dtype=np.float64).reshape(c.shape)
+
+
+def e4m3_from_float(x) -> np.ndarray:
+    a = np.ascontiguousarray(np.asarray(x, dtype=np.float32))
+    f = lib().lazy_oracle_e4m3_from_float
+    f.restype = ctypes.c_uint8
+    f.argtypes = [ctypes.c_float]
+    return np.array([f(float(v)) for v in a.ravel()], dtype=np.uint8).reshape(a.shape)
+
+
+class Fp8Pools:
+    """The oracle's own FP8 page pools (numpy): codes [num_pages,Hkv,P,D] uint8, scales [num_pages,Hkv,P] float32.
+    Unwritten rows hold the NaN code 0x7f and a NaN scale, so that a kernel reading past a tail is caught."""
+
+    def __init__(self, num_pages: int, Hkv: int, P: int, D: int):
+        self.k_codes = np.full((num_pages, Hkv, P, D), 0x7f, dtype=np.uint8)
+        self.v_codes = np.full((num_pages, Hkv, P, D), 0x7f, dtype=np.uint8)
+        self.k_scale = np.full((num_pages, Hkv, P), np.nan, dtype=np.float32)
+        self.v_scale = np.full((num_pages, Hkv, P), np.nan, dtype=np.float32)
+
+
+def cache_write_fp8(k_new, v_new, slot_mapping, pools: Fp8Pools) -> None:
+    """Quantise bf16 rows [T,Hkv,D] (torch) into the FP8 pools, in place."""
+    import torch
+    kn = np.ascontiguousarray(k_new.contiguous().view(torch.int16).numpy()).view(np.uint16)
+    vn = np.ascontiguousarray(v_new.contiguous().view(torch.int16).numpy()).view(np.uint16)
+    sm = np.ascontiguousarray(np.asarray(slot_mapping, dtype=np.int64))
+    T, Hkv, D = kn.shape
+    num_pages, _, P, _ = pools.k_codes.shape
+    f = lib().lazy_oracle_cache_write_fp8
+    f.restype = ctypes.c_int
+    rc = f(_p(kn), _p(vn), _p(sm), ctypes.c_int64(T), ctypes.c_int(Hkv), ctypes.c_int(D), ctypes.c_int(P),
+           ctypes.c_int64(num_pages), _p(pools.k_codes), _p(pools.v_codes), _p(pools.k_scale), _p(pools.v_scale))
+    if rc != 0:
+        raise RuntimeError(f"lazy_oracle_cache_write_fp8 failed: {rc}")
+
+
+def quantize_pool_fp8(k_pool, v_pool) -> Fp8Pools:
+    """FP8 pools holding the quantised content of whole bf16 pools [num_pages,Hkv,P,D]: every slot whose K and V
+    rows are finite is written once; poisoned (NaN) slots of the bf16 pools stay poisoned (skipped)."""
+    import torch
+    num_pages, Hkv, P, D = k_pool.shape
+    pools = Fp8Pools(num_pages, Hkv, P, D)
+    kn = k_pool.permute(0, 2, 1, 3).reshape(num_pages * P, Hkv, D)
+    vn = v_pool.permute(0, 2, 1, 3).reshape(num_pages * P, Hkv, D)
+    ok = torch.isfinite(kn.float()).all(dim=(1, 2)) & torch.isfinite(vn.float()).all(dim=(1, 2))
+    slots = np.where(ok.numpy(), np.arange(num_pages * P, dtype=np.int64), -1)
+    cache_write_fp8(kn, vn, slots, pools)
+    return pools
+
+
+def attend_paged_fp8(q, pools: Fp8Pools, block_table, page_logical_pos, seq_lens, cu_q_lens, *,
+                     num_q_heads: int, num_kv_heads: int, head_dim: int, page_size: int, theta: float,
+                     row_select=None, rope_style: int = 0, inv_freq=None, scale: float = 0.0,
+                     alibi_slopes=None) -> np.ndarray:
+    """attend_paged over FP8 pages: exact dequantisation, then the unchanged definition."""
+    qa, dq = _as_kernel_input(q)
+    bt = np.ascontiguousarray(np.asarray(block_table, dtype=np.int32))
+    pp = np.ascontiguousarray(np.asarray(page_logical_pos, dtype=np.int32))
+    assert bt.shape == pp.shape and bt.ndim == 2
+    sl = np.ascontiguousarray(np.asarray(seq_lens, dtype=np.int32))
+    cu = np.ascontiguousarray(np.asarray(cu_q_lens, dtype=np.int32))
+    out = np.zeros((int(cu[-1]), num_q_heads, head_dim), dtype=np.float64)
+    rs = None if row_select is None else np.ascontiguousarray(np.asarray(row_select, dtype=np.uint8))
+    fr = None if inv_freq is None else np.ascontiguousarray(np.asarray(inv_freq, dtype=np.float64))
+    al = None if alibi_slopes is None else np.ascontiguousarray(np.asarray(alibi_slopes, dtype=np.float64))
+    f = lib().lazy_oracle_attend_paged_fp8
+    f.restype = ctypes.c_int
+    rc = f(_p(qa), ctypes.c_int(dq), _p(pools.k_codes), _p(pools.v_codes), _p(pools.k_scale), _p(pools.v_scale),
+           _p(bt), _p(pp), ctypes.c_int64(bt.shape[1]), _p(sl), _p(cu), ctypes.c_int(sl.shape[0]),
+           ctypes.c_int(num_q_heads), ctypes.c_int(num_kv_heads), ctypes.c_int(head_dim), ctypes.c_int(page_size),
+           ctypes.c_double(theta), ctypes.c_int(rope_style), _p(fr), ctypes.c_double(scale), _p(al), _p(rs), _p(out))
+    if rc != 0:
+        raise RuntimeError(f"lazy_oracle_attend_paged_fp8 failed: {rc}")
+    return out
+
+
+def run_step_fp8(batch, step, pools: Fp8Pools, row_select=None, **variant) -> Optional[np.ndarray]:
+    """run_step over FP8 pools: quantising cache write, then attention over the dequantised pages."""
+    sh = batch.shape
+    if step.k_new is not None:
+        cache_write_fp8(step.k_new, step.v_new, step.slot_mapping.numpy(), pools)
+    if step.kind == "write_only":
+        return None
+    bt, pp = batch.block_table, batch.page_logical_pos
+    if step.req_ids is not None:
+        bt, pp = bt[step.req_ids], pp[step.req_ids]
+    return attend_paged_fp8(step.q, pools, bt.numpy(), pp.numpy(), step.seq_lens.numpy(), step.cu_q_lens.numpy(),
+                            num_q_heads=sh.num_q_heads, num_kv_heads=sh.num_kv_heads, head_dim=sh.head_dim,
+                            page_size=sh.page_size, theta=sh.rope_theta, row_select=row_select, **variant)
+
+
 def run_step(batch, step, k_pool, v_pool, row_select=None, **variant) -> Optional[np.ndarray]:
     """Apply one workloads.Step with the oracle: cache write (in place on the given pool copies),
     then the attention call.  Returns the fp64 output or None for write-only steps."""
