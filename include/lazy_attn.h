@@ -59,7 +59,7 @@ typedef struct lazy_config {
   int32_t max_pages_per_req; /* row stride (in entries) of block_table and page_logical_pos     */
   double  rope_theta;        /* 1e4, 5e5, 1e6 ...                                               */
   int32_t rope_style;        /* LAZY_ROPE_* : pairing of the rotated dimensions (0 = half-split)  */
-  int32_t dtype;             /* 0 = bf16 (the only dtype)                                       */
+  int32_t dtype;             /* LAZY_KV_* : what the KV pages hold (0 = bf16; q, k_new, v_new, out are always bf16) */
   int32_t flags;             /* LAZY_FLAG_* (0 for production)                                  */
   int32_t k_storage;         /* LAZY_K_* : how the pages hold K (0 = un-rotated, the product)    */
 } lazy_config;
@@ -96,6 +96,22 @@ typedef struct lazy_config {
 #define LAZY_K_UNROTATED  0
 #define LAZY_K_STORED_POS 1
 #define LAZY_K_ABSOLUTE   2
+
+/* dtype: storage format of the KV pages (SURVEY.md 8.0 row f4 "FP8 KV pages").  The paper's cache holds "purely
+ * content-based keys and values" -- a page carries no position, so a QUANTISED page is as shareable
+ * at any logical offset as a bf16 one -- and decode moves 2LD bytes (L204-209), which this halves.  The paper defines
+ * no quantised format; this one is the repository's:
+ *   LAZY_KV_BF16      the pool layout above.
+ *   LAZY_KV_FP8_E4M3  k_cache, v_cache : [num_pages][num_kv_heads][page_size][head_dim] bytes, OCP FP8 E4M3 codes of
+ *                     the un-rotated K row / of the V row divided by a per-row scale; the scales are two more device
+ *                     arrays [num_pages][num_kv_heads][page_size] fp32 registered with lazy_set_kv_scales (per token,
+ *                     because lazy_cache_write appends single tokens to half-filled pages).  lazy_cache_write
+ *                     quantises: scale = max|row| / 448 in fp32 (1 for an all-zero row), code = nearest E4M3 (ties
+ *                     to even, saturating) of the fp32 quotient row[d] / scale.  The attention calls compute what the
+ *                     bf16 calls would compute on the exactly dequantised pages (code value x scale).  Supported
+ *                     with LAZY_ROPE_HALF_SPLIT and LAZY_K_UNROTATED; lazy_materialize_pages is bf16-only. */
+#define LAZY_KV_BF16      0
+#define LAZY_KV_FP8_E4M3  1
 
 /* flags: debugging aids, never set by bench.py */
 #define LAZY_FLAG_ROWWISE_KERNELS 1  /* run the simple one-row-per-CTA CUDA kernels for prefill and decode */
@@ -169,6 +185,12 @@ int lazy_set_alibi_slopes(lazy_handle* h, const float* slopes, void* stream);
  * was rotated when it was stored.  The pointer is kept (not copied) and read by every later attention call;
  * it must stay valid until lazy_destroy or the next lazy_set_page_stored_pos.  Host-side, no launch. */
 int lazy_set_page_stored_pos(lazy_handle* h, const int32_t* page_stored_pos);
+
+/* LAZY_KV_FP8_E4M3 only: device arrays [num_pages][num_kv_heads][page_size] fp32 holding the per-row scales of the
+ * K and V code pools.  lazy_cache_write fills them, the attention calls read them.  The pointers are kept (not
+ * copied) and must stay valid until lazy_destroy or the next lazy_set_kv_scales; 16-byte aligned.  Host-side, no
+ * launch. */
+int lazy_set_kv_scales(lazy_handle* h, float* k_scale, float* v_scale);
 
 /* f2. Materialising re-encoding of whole pages: what a position-dependent cache does on a position mismatch
  * ("allocate + copy + rotate", App. B; "read-modify-write ... doubling HBM traffic", L447) and

@@ -414,11 +414,14 @@ int lazy_oracle_cache_write(const uint16_t* k_new, const uint16_t* v_new, const 
 int lazy_oracle_cache_write_fp8(const uint16_t* k_new, const uint16_t* v_new, const int64_t* slot_mapping,
                                 int64_t num_tokens, int Hkv, int D, int P, int64_t num_pages,
                                 uint8_t* k_codes, uint8_t* v_codes, float* k_scale, float* v_scale) {
+    for (int64_t t = 0; t < num_tokens; ++t)
+        if (slot_mapping[t] >= 0 && slot_mapping[t] / P >= num_pages) return -1;
+    /* tokens are independent (distinct slots): OpenMP only distributes them over host cores */
+#pragma omp parallel for schedule(static)
     for (int64_t t = 0; t < num_tokens; ++t) {
         int64_t slot = slot_mapping[t];
         if (slot < 0) continue;
         int64_t page = slot / P, off = slot % P;
-        if (page >= num_pages) return -1;
         for (int hk = 0; hk < Hkv; ++hk) {
             int64_t dst = ((page * Hkv + hk) * P + off) * D;
             int64_t src = (t * Hkv + hk) * D;

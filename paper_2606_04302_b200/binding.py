@@ -18,9 +18,11 @@ LAZY_FLAG_ROWWISE_KERNELS = 1
 LAZY_FLAG_PREFILL_ONE_CTA = 2
 LAZY_K_UNROTATED, LAZY_K_STORED_POS, LAZY_K_ABSOLUTE = 0, 1, 2
 LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
+LAZY_KV_BF16, LAZY_KV_FP8_E4M3 = 0, 1
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
            "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_alibi_slopes", "lazy_set_page_stored_pos",
+           "lazy_set_kv_scales",
            "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step", "lazy_host_step_layout", "lazy_host_step_packed",
            "lazy_attn_mixed", "lazy_debug_validate",
            "lazy_pool_create", "lazy_pool_destroy", "lazy_pool_acquire", "lazy_pool_release", "lazy_pool_stats",
@@ -66,6 +68,8 @@ def lib() -> ctypes.CDLL:
         L.lazy_set_alibi_slopes.argtypes = [vp, vp, vp]
         L.lazy_set_page_stored_pos.restype = ctypes.c_int
         L.lazy_set_page_stored_pos.argtypes = [vp, vp]
+        L.lazy_set_kv_scales.restype = ctypes.c_int
+        L.lazy_set_kv_scales.argtypes = [vp, vp, vp]
         L.lazy_materialize_pages.restype = ctypes.c_int
         L.lazy_materialize_pages.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp, vp, i32, vp]
         L.lazy_status_string.restype = ctypes.c_char_p
@@ -164,10 +168,10 @@ class LazyHandle:
 
 def lazy_create(num_q_heads: int, num_kv_heads: int, head_dim: int, *, num_pages: int, max_position: int,
                 max_reqs: int, max_pages_per_req: int, rope_theta: float, page_size: int = 16, flags: int = 0,
-                k_storage: int = LAZY_K_UNROTATED, rope_style: int = LAZY_ROPE_HALF_SPLIT, device="cuda",
-                stream=None) -> LazyHandle:
+                k_storage: int = LAZY_K_UNROTATED, rope_style: int = LAZY_ROPE_HALF_SPLIT, dtype: int = LAZY_KV_BF16,
+                device="cuda", stream=None) -> LazyHandle:
     cfg = LazyConfig(num_q_heads, num_kv_heads, head_dim, page_size, num_pages, max_position, max_reqs,
-                     max_pages_per_req, float(rope_theta), rope_style, 0, flags, k_storage)
+                     max_pages_per_req, float(rope_theta), rope_style, dtype, flags, k_storage)
     return LazyHandle(cfg, device=device, stream=stream)
 
 
@@ -232,6 +236,13 @@ def lazy_set_page_stored_pos(h: LazyHandle, page_stored_pos) -> None:
     if rc != 0:
         raise LazyError("lazy_set_page_stored_pos", rc)
     h._stored_pos = page_stored_pos          # the library keeps the pointer: keep the tensor alive with the handle
+
+
+def lazy_set_kv_scales(h: LazyHandle, k_scale, v_scale) -> None:
+    rc = lib().lazy_set_kv_scales(h.ptr, _ptr(k_scale), _ptr(v_scale))
+    if rc != 0:
+        raise LazyError("lazy_set_kv_scales", rc)
+    h._kv_scales = (k_scale, v_scale)        # the library keeps the pointers: keep the tensors alive with the handle
 
 
 def lazy_materialize_pages(h: LazyHandle, k_src, v_src, src_pages, rot_pos, per_token: bool, k_dst, v_dst,

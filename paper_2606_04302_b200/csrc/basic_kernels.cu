@@ -84,6 +84,8 @@ __global__ void cache_write_kernel(const uint4* __restrict__ k_new, const uint4*
 
 int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
                        int num_tokens, void* k_cache, void* v_cache, cudaStream_t stream) {
+  if (h->cfg.dtype == LAZY_KV_FP8_E4M3)
+    return launch_cache_write_fp8(h, k_new, v_new, slot_mapping, num_tokens, k_cache, v_cache, stream);
   int chunks_per_row = h->cfg.head_dim / 8;
   long long num_chunks = (long long)num_tokens * h->cfg.num_kv_heads * chunks_per_row;
   int threads = 256;
@@ -298,6 +300,9 @@ int launch_rowwise(lazy_handle* h, const void* q, const void* k_cache, const voi
                    const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                    const int32_t* cu_q_lens, int num_reqs, int total_q, int /*max_q_len*/, void* out,
                    cudaStream_t stream) {
+  if (h->cfg.dtype == LAZY_KV_FP8_E4M3)
+    return launch_rowwise_fp8(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, cu_q_lens, num_reqs,
+                              total_q, out, stream);
   dim3 grid(total_q, h->cfg.num_q_heads);
   auto qp = static_cast<const __nv_bfloat16*>(q);
   auto kp = static_cast<const __nv_bfloat16*>(k_cache);

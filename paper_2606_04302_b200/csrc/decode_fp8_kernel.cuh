@@ -1,0 +1,423 @@
+// decode_fp8_kernel.cuh -- the split-KV decode CTA over LAZY_KV_FP8_E4M3 pages (head_dim 128, un-rotated K).
+//
+// Same decomposition, pipeline, rotation identity and in-kernel combine as decode_kernel.cuh (see decode_splitkv.cu);
+// what changes is the arithmetic type of a tile, chosen so that a tile of HALF the bytes does not cost MORE
+// instructions than a bf16 tile (the bf16 kernel's streaming rate is set by its consumer warps):
+//   * K codes are widened e4m3x2 -> f16x2 (exact, one instruction per two elements) and rotated by the in-page offset
+//     IN F16 on packed halves (HMUL2 / HFMA2: |code| <= 448, cos/sin rounded to f16 -- relative 2^-11, finer than the
+//     bf16 rounding the bf16 kernel applies to the rotated K) -- no unpack to fp32, no repack;
+//   * q is re-rotated per page in fp32 as before and rounded to f16; QK^T and PV are mma.sync m16n8k16 f16 -> fp32;
+//   * the K scale of a token (a row of S) multiplies the fp32 score together with log2(e)/sqrt(D);
+//   * V codes come out of shared memory already transposed AND still 8-bit with the 8-bit transposing ldmatrix
+//     (m16n16.b8: thread (g, tq) gets tokens 4tq..4tq+3 of dims g, g+8), are widened to f16x2 and used as the A
+//     operand; that fixes which MMA k-slot holds which token, and the token -> MMA-row order of the QK^T product is
+//     chosen to match (row i <-> token (i>>1) + 4(i&1) + (i&8)), which also makes the K loads bank-conflict-free;
+//   * the V scale of a token multiplies P (fp32, then f16) relative to a running reference scale c_run carried like
+//     the softmax maximum: P' = p * sv / c_run, O accumulates in units of c_run and is rescaled only when a page's
+//     largest V scale leaves [c_run/64, 64 c_run] (f16 has the range: P' <= 64).
+#pragma once
+#include <cuda_fp16.h>
+
+#include "decode_kernel.cuh"
+
+namespace lazy {
+namespace {
+
+template <int HKV_CTA>
+struct DecodeFp8Cfg {
+  static constexpr int D = 128;
+  static constexpr int PPS = kConsumerWarps / HKV_CTA;  // pages per pipeline stage
+  static constexpr int BOX_ROWS = 16 * HKV_CTA;
+  static constexpr int PAGE_BYTES = BOX_ROWS * 128;     // K (or V) codes of one page, HKV_CTA heads: rows of 128 B
+  static constexpr int CS_ROW_BYTES = D / 2 * 8;
+  static constexpr int SC_BYTES = HKV_CTA * 64;         // K (or V) scales of one page, HKV_CTA heads
+  static constexpr int OFF_V = PPS * PAGE_BYTES;
+  static constexpr int OFF_CS = 2 * PPS * PAGE_BYTES;
+  static constexpr int OFF_SK = OFF_CS + PPS * CS_ROW_BYTES;
+  static constexpr int OFF_SV = OFF_SK + PPS * SC_BYTES;
+  static constexpr int OFF_META = OFF_SV + PPS * SC_BYTES;
+  static constexpr int STAGE_BYTES = (OFF_META + PPS * 4 + 1023) / 1024 * 1024;
+  static constexpr int NSTAGES = 5;
+  static constexpr int NL = 8;                          // words of 2 rotation pairs per thread per half
+  static constexpr int NC = D / 16;
+  static constexpr int OFF_CUM = NSTAGES * STAGE_BYTES;
+  static constexpr int OFF_LEN = OFF_CUM + (kMaxReqsSmem + 4) * 4;
+  static constexpr int OFF_BAR = OFF_LEN + kMaxReqsSmem * 4;
+  static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGES * 8 + 16 + 1024;
+};
+
+struct DecodeFp8Args {
+  DecodeArgs d;            // q, tables, out, cs, partials (stored_pos / alibi unused)
+  const float* k_scale;    // [num_pages][Hkv][16]
+  const float* v_scale;
+};
+
+__device__ __forceinline__ uint32_t h2mul(uint32_t a, uint32_t b) {
+  const __half2 r = __hmul2(*reinterpret_cast<const __half2*>(&a), *reinterpret_cast<const __half2*>(&b));
+  return *reinterpret_cast<const uint32_t*>(&r);
+}
+__device__ __forceinline__ uint32_t h2fma(uint32_t a, uint32_t b, uint32_t c) {
+  const __half2 r = __hfma2(*reinterpret_cast<const __half2*>(&a), *reinterpret_cast<const __half2*>(&b),
+                            *reinterpret_cast<const __half2*>(&c));
+  return *reinterpret_cast<const uint32_t*>(&r);
+}
+__device__ __forceinline__ uint32_t h2neg(uint32_t a) { return a ^ 0x80008000u; }
+
+template <int HKV_CTA>
+__device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const CUtensorMap& tmap_v,
+                                               const DecodeFp8Args& fa, const int bid, const int G_in, const int hg,
+                                               const int HG, unsigned char* smem_raw) {
+  using C = DecodeFp8Cfg<HKV_CTA>;
+  constexpr int D = C::D;
+  const DecodeArgs& a = fa.d;
+  unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const uint32_t smem_base = ptx::smem_u32(smem);
+  int* s_cum = reinterpret_cast<int*>(smem + C::OFF_CUM);
+  int* s_len = reinterpret_cast<int*>(smem + C::OFF_LEN);
+  const uint32_t bar_full = smem_base + C::OFF_BAR;
+  const uint32_t bar_empty = bar_full + C::NSTAGES * 8;
+  int* s_flag = reinterpret_cast<int*>(smem + C::OFF_BAR + 2 * C::NSTAGES * 8);
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int R = a.num_reqs;
+  int G = G_in;
+  const Shape sh = a.sh;
+
+  // ---- prologue: barriers, unit prefix sums ---------------------------------------------------------------
+  if (tid == 0) {
+    for (int s = 0; s < C::NSTAGES; ++s) {
+      ptx::mbar_init(bar_full + 8 * s, 1);
+      ptx::mbar_init(bar_empty + 8 * s, kConsumerWarps);
+    }
+    ptx::fence_mbar_init();
+  }
+  if (warp == kConsumerWarps && lane == 0) {
+    ptx::prefetch_tmap(&tmap_k);
+    ptx::prefetch_tmap(&tmap_v);
+  }
+  if (warp == 0) {
+    int carry = 0;
+    if (lane == 0) s_cum[0] = 0;
+    for (int base = 0; base < R; base += 32) {
+      int r = base + lane;
+      int L = (r < R) ? a.seq_lens[r] : 0;
+      if (L < 0) L = 0;
+      int np = (L + kPageSize - 1) / kPageSize;
+      int nu = (r < R) ? max(1, (np + C::PPS - 1) / C::PPS) : 0;
+      int x = nu;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += y;
+      }
+      if (r < R) { s_cum[r + 1] = carry + x; s_len[r] = L; }
+      carry += __shfl_sync(0xffffffffu, x, 31);
+    }
+  }
+  __syncthreads();
+
+  const long long U = s_cum[R];
+  if (U < G) G = (int)U;
+  if (bid >= G) return;
+  const int u_begin = (int)(((long long)bid * U) / G);
+  const int u_end = (int)(((long long)(bid + 1) * U) / G);
+  if (u_begin >= u_end) return;
+  int r0;
+  {
+    int lo = 0, hi = R;
+    while (lo < hi) { int mid = (lo + hi) >> 1; if (s_cum[mid + 1] > u_begin) hi = mid; else lo = mid + 1; }
+    r0 = lo;
+  }
+
+  if (warp >= kConsumerWarps) {
+    ptx::setmaxnreg_dec<kRegsProducer>();
+    if (warp > kConsumerWarps) return;
+    // ================================= producer warp =====================================================
+    const int pl = lane;
+    int r = r0, u = u_begin;
+    int it = 0;
+    auto load_unit = [&](int rr, int uu, int& pg, int& delta, int& nvalid) {
+      int L = s_len[rr];
+      int np = (L + kPageSize - 1) / kPageSize;
+      int ul = uu - s_cum[rr];
+      int p = ul * C::PPS + pl;
+      nvalid = min(C::PPS, max(0, np - ul * C::PPS));
+      pg = 0; delta = 0;
+      if (pl < C::PPS && p < np) {
+        const int* bt = a.block_table + (size_t)rr * sh.table_stride;
+        const int* pp = a.page_pos + (size_t)rr * sh.table_stride;
+        int mq = pp[(L - 1) / kPageSize] + (L - 1) % kPageSize;
+        pg = bt[p];
+        delta = mq - pp[p];
+      }
+    };
+    int pg, delta, nvalid;
+    load_unit(r, u, pg, delta, nvalid);
+    while (u < u_end) {
+      int rn = r, un = u + 1;
+      if (un >= s_cum[rn + 1]) rn++;
+      int pg_n = 0, delta_n = 0, nvalid_n = 0;
+      if (un < u_end) load_unit(rn, un, pg_n, delta_n, nvalid_n);
+
+      const int stage = it % C::NSTAGES;
+      const uint32_t parity = (it / C::NSTAGES) & 1;
+      ptx::mbar_wait(bar_empty + 8 * stage, parity ^ 1);
+      unsigned char* st = smem + stage * C::STAGE_BYTES;
+      const uint32_t st_u32 = smem_base + stage * C::STAGE_BYTES;
+      const uint32_t full = bar_full + 8 * stage;
+      const bool active = pl < nvalid;
+      if (pl < C::PPS) reinterpret_cast<int*>(st + C::OFF_META)[pl] = delta;
+      __syncwarp();
+      if (lane == 0)
+        ptx::mbar_arrive_expect_tx(full, nvalid * (2 * C::PAGE_BYTES + C::CS_ROW_BYTES + 2 * C::SC_BYTES));
+      __syncwarp();
+      if (active) {
+        const int row0 = (pg * sh.Hkv + hg * HKV_CTA) * kPageSize;
+        ptx::tma_load_2d(st_u32 + pl * C::PAGE_BYTES, &tmap_k, full, 0, row0);
+        ptx::tma_load_2d(st_u32 + C::OFF_V + pl * C::PAGE_BYTES, &tmap_v, full, 0, row0);
+        const int ad = delta < 0 ? -delta : delta;
+        ptx::bulk_load_1d(st_u32 + C::OFF_CS + pl * C::CS_ROW_BYTES, a.cs + (size_t)ad * (D / 2), C::CS_ROW_BYTES, full);
+        ptx::bulk_load_1d(st_u32 + C::OFF_SK + pl * C::SC_BYTES, fa.k_scale + row0, C::SC_BYTES, full);
+        ptx::bulk_load_1d(st_u32 + C::OFF_SV + pl * C::SC_BYTES, fa.v_scale + row0, C::SC_BYTES, full);
+      }
+      pg = pg_n; delta = delta_n; nvalid = nvalid_n;
+      r = rn; u = un; ++it;
+    }
+    return;
+  }
+
+  // =================================== consumer warps ====================================================
+  ptx::setmaxnreg_inc<kRegsConsumer>();
+  const int g = lane >> 2, tq = lane & 3;
+  const int pl = warp / HKV_CTA;
+  const int hl = warp % HKV_CTA;
+  const int hk = hg * HKV_CTA + hl;
+  const int group = sh.group;
+  // MMA row g of the QK^T tile is token t0, row g + 8 token t0 + 8 (see the header: the order the V fragments fix)
+  const int t0 = (g >> 1) + 4 * (g & 1);
+
+  // in-page rotation constants of this thread's two tokens and 16 pairs, as f16x2 (cos j, cos j+1) / (sin j, sin j+1)
+  uint32_t ctc[2][C::NL], cts[2][C::NL];
+  {
+    const float4* cs4 = reinterpret_cast<const float4*>(a.cs);
+#pragma unroll
+    for (int rw = 0; rw < 2; ++rw)
+#pragma unroll
+      for (int w = 0; w < C::NL; ++w) {
+        const float4 v = __ldg(cs4 + (size_t)(t0 + 8 * rw) * (D / 4) + w * 4 + tq);
+        ctc[rw][w] = ptx::pack_f16(v.x, v.y);
+        cts[rw][w] = ptx::pack_f16(v.z, v.w);
+      }
+  }
+  // ldmatrix row address of this lane inside a (page, head) V tile: matrix row i = lane & 15 is token (i>>2) + 4(i&3)
+  const int vtok = ((lane & 15) >> 2) + 4 * (lane & 3);
+  const int vrow = hl * 16 + vtok;
+  const int vmat = lane >> 4;                       // which of the two 16-dim tiles of an x2 load this lane addresses
+
+  int r = r0, u = u_begin, it = 0;
+  while (u < u_end) {
+    const int L = s_len[r];
+    const int seg_lo = u - s_cum[r];
+    const int seg_hi = min(u_end, s_cum[r + 1]) - s_cum[r];
+
+    // un-rotated q of head g of this kv head's group, widened to fp32 once per segment
+    float qf[2][C::NL][2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int w = 0; w < C::NL; ++w) { qf[h][w][0] = 0.f; qf[h][w][1] = 0.f; }
+    if (g < group) {
+      const uint4* qp = reinterpret_cast<const uint4*>(a.q + ((size_t)r * sh.Hq + hk * group + g) * D);
+#pragma unroll
+      for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int x = 0; x < 2; ++x) {
+          const uint4 v = qp[(h * (D / 2) + 16 * tq) / 8 + x];
+          const uint32_t ww[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+          for (int y = 0; y < 4; ++y) {
+            qf[h][4 * x + y][0] = ptx::bf16_lo(ww[y]);
+            qf[h][4 * x + y][1] = ptx::bf16_hi(ww[y]);
+          }
+        }
+    }
+    uint32_t qhat[2][C::NL];
+
+    float oacc[C::NC][4];
+#pragma unroll
+    for (int i = 0; i < C::NC; ++i) { oacc[i][0] = oacc[i][1] = oacc[i][2] = oacc[i][3] = 0.f; }
+    float m_run[2] = {-INFINITY, -INFINITY};
+    float l_run[2] = {0.f, 0.f};
+    // reference V scale: O is accumulated in units of c_run; (c_lo, c_hi) = the band a page's largest scale may
+    // move in before O is re-referenced (empty at first: the first page sets it)
+    float c_run = 1.f, inv_c = 1.f, c_lo = 0.f, c_hi = 0.f;
+    for (int ul = seg_lo; ul < seg_hi; ++ul, ++it) {
+      const int stage = it % C::NSTAGES;
+      const uint32_t parity = (it / C::NSTAGES) & 1;
+      ptx::mbar_wait(bar_full + 8 * stage, parity);
+      const int p = ul * C::PPS + pl;
+      const int nv = min(kPageSize, L - p * kPageSize);      // valid tokens of this page (<= 0: no page)
+      if (nv > 0) {
+        const uint32_t st = smem_base + stage * C::STAGE_BYTES;
+        const int delta = ptx::lds32(st + C::OFF_META + pl * 4);
+        // ---- K codes -> registers: 16 bytes per (half, token row): dims 64h + 16tq .. +15
+        uint4 kc[2][2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+          for (int rw = 0; rw < 2; ++rw) {
+            const int Rr = hl * 16 + t0 + 8 * rw;
+            kc[h][rw] = ptx::lds128(st + pl * C::PAGE_BYTES + Rr * 128 + (((4 * h + tq) ^ (Rr & 7)) * 16));
+          }
+        // scales of this thread's two tokens: K (times log2(e)/sqrt(D)) and V
+        const uint32_t sc_off = pl * C::SC_BYTES + (hl * 16 + t0) * 4;
+        const float sk0 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off)) * sh.scale_log2;
+        const float sk1 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off + 32)) * sh.scale_log2;
+        float sv0 = __int_as_float(ptx::lds32(st + C::OFF_SV + sc_off));
+        float sv1 = __int_as_float(ptx::lds32(st + C::OFF_SV + sc_off + 32));
+        // ---- q re-rotated for this page: Qhat = R_{m - p0} q in fp32, rounded to f16 (a3/a4)
+        {
+          const uint32_t qcs = st + C::OFF_CS + pl * C::CS_ROW_BYTES + tq * 16;
+          const float sgn = delta < 0 ? -1.f : 1.f;
+#pragma unroll
+          for (int w = 0; w < C::NL; ++w) {
+            const float4 c = ptx::lds128f(qcs + w * 64);
+            const float2 cc = make_float2(c.x, c.y);
+            const float2 ss = __fmul2_rn(make_float2(c.z, c.w), make_float2(sgn, sgn));
+            const float2 x1 = make_float2(qf[0][w][0], qf[0][w][1]), x2 = make_float2(qf[1][w][0], qf[1][w][1]);
+            const float2 y1 = __ffma2_rn(make_float2(-x2.x, -x2.y), ss, __fmul2_rn(x1, cc));
+            const float2 y2 = __ffma2_rn(x2, cc, __fmul2_rn(x1, ss));
+            qhat[0][w] = ptx::pack_f16(y1.x, y1.y);
+            qhat[1][w] = ptx::pack_f16(y2.x, y2.y);
+          }
+        }
+        // ---- Khat = R_t k on packed f16 lanes (codes, un-scaled: the token's scale goes to the score)
+        uint32_t kreg[2][2][C::NL];
+#pragma unroll
+        for (int rw = 0; rw < 2; ++rw) {
+          const uint32_t a1[4] = {kc[0][rw].x, kc[0][rw].y, kc[0][rw].z, kc[0][rw].w};
+          const uint32_t a2[4] = {kc[1][rw].x, kc[1][rw].y, kc[1][rw].z, kc[1][rw].w};
+#pragma unroll
+          for (int w = 0; w < C::NL; ++w) {
+            const uint32_t x1 = (w & 1) ? ptx::e4m3x2_hi_to_f16x2(a1[w >> 1]) : ptx::e4m3x2_lo_to_f16x2(a1[w >> 1]);
+            const uint32_t x2 = (w & 1) ? ptx::e4m3x2_hi_to_f16x2(a2[w >> 1]) : ptx::e4m3x2_lo_to_f16x2(a2[w >> 1]);
+            kreg[0][rw][w] = h2fma(h2neg(x2), cts[rw][w], h2mul(x1, ctc[rw][w]));
+            kreg[1][rw][w] = h2fma(x2, ctc[rw][w], h2mul(x1, cts[rw][w]));
+          }
+        }
+        // ---- S = Khat Qhat^T : rows = tokens (t0, t0 + 8), cols = heads (2tq, 2tq+1)
+        float s[4] = {0.f, 0.f, 0.f, 0.f}, s_b[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+        for (int cc = 0; cc < C::NC / 2; ++cc) {
+          ptx::mma_f16_16816(s, kreg[0][0][2 * cc], kreg[0][1][2 * cc], kreg[0][0][2 * cc + 1],
+                             kreg[0][1][2 * cc + 1], qhat[0][2 * cc], qhat[0][2 * cc + 1]);
+          ptx::mma_f16_16816(s_b, kreg[1][0][2 * cc], kreg[1][1][2 * cc], kreg[1][0][2 * cc + 1],
+                             kreg[1][1][2 * cc + 1], qhat[1][2 * cc], qhat[1][2 * cc + 1]);
+        }
+        s[0] = (s[0] + s_b[0]) * sk0; s[1] = (s[1] + s_b[1]) * sk0;
+        s[2] = (s[2] + s_b[2]) * sk1; s[3] = (s[3] + s_b[3]) * sk1;
+        if (t0 >= nv) { s[0] = -INFINITY; s[1] = -INFINITY; sv0 = 0.f; }
+        if (t0 + 8 >= nv) { s[2] = -INFINITY; s[3] = -INFINITY; sv1 = 0.f; }
+        // ---- online softmax over the 16 tokens (a6)
+        float mx0 = fmaxf(s[0], s[2]), mx1 = fmaxf(s[1], s[3]);
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+          mx0 = fmaxf(mx0, __shfl_xor_sync(0xffffffffu, mx0, o));
+          mx1 = fmaxf(mx1, __shfl_xor_sync(0xffffffffu, mx1, o));
+        }
+        const float mn0 = fmaxf(m_run[0], mx0), mn1 = fmaxf(m_run[1], mx1);
+        if (__any_sync(0xffffffffu, mn0 > m_run[0] || mn1 > m_run[1])) {
+          const float corr0 = exp2f(m_run[0] - mn0), corr1 = exp2f(m_run[1] - mn1);
+          m_run[0] = mn0; m_run[1] = mn1;
+          l_run[0] *= corr0; l_run[1] *= corr1;
+#pragma unroll
+          for (int i = 0; i < C::NC; ++i) {
+            oacc[i][0] *= corr0; oacc[i][1] *= corr1; oacc[i][2] *= corr0; oacc[i][3] *= corr1;
+          }
+        }
+        const float p0 = exp2f(s[0] - mn0), p1 = exp2f(s[1] - mn1);
+        const float p2 = exp2f(s[2] - mn0), p3 = exp2f(s[3] - mn1);
+        l_run[0] += p0 + p2;
+        l_run[1] += p1 + p3;
+        // ---- V scales: P' = p * sv / c_run; re-reference O when the page's largest scale leaves the band
+        const float svmax = __uint_as_float(__reduce_max_sync(0xffffffffu, __float_as_uint(fmaxf(sv0, sv1))));
+        if (svmax > c_hi || svmax < c_lo) {          // warp-uniform; the first page, then rare
+          const float f = c_run / svmax;
+          c_run = svmax; inv_c = 1.f / svmax; c_lo = svmax * (1.f / 64.f); c_hi = svmax * 64.f;
+#pragma unroll
+          for (int i = 0; i < C::NC; ++i) { oacc[i][0] *= f; oacc[i][1] *= f; oacc[i][2] *= f; oacc[i][3] *= f; }
+        }
+        const float w0 = sv0 * inv_c, w1 = sv1 * inv_c;
+        // ---- P' (f16) transposed into the B-fragment layout: k = tokens, n = heads
+        const uint32_t pb0 = ptx::movmatrix_trans(ptx::pack_f16(p0 * w0, p1 * w0));
+        const uint32_t pb1 = ptx::movmatrix_trans(ptx::pack_f16(p2 * w1, p3 * w1));
+        // ---- O^T += V^T P'  (a7): 8-bit transposing ldmatrix, two 16-dim tiles per load; byte b of a register is
+        // token tq + 4b -- bytes past the tail are cleared (their codes may be NaN)
+        uint32_t vmask = 0xffffffffu;
+        if (nv < kPageSize)
+          vmask = (tq < nv ? 0xffu : 0u) | (tq + 4 < nv ? 0xff00u : 0u) | (tq + 8 < nv ? 0xff0000u : 0u) |
+                  (tq + 12 < nv ? 0xff000000u : 0u);
+        const uint32_t vbase = st + C::OFF_V + pl * C::PAGE_BYTES + vrow * 128;
+#pragma unroll
+        for (int i = 0; i < C::NC; i += 2) {
+          uint32_t r0, r1, r2, r3;
+          ptx::ldmatrix_b8_x2_trans(r0, r1, r2, r3, vbase + ((((i + vmat)) ^ (vrow & 7)) * 16));
+          if (nv < kPageSize) { r0 &= vmask; r1 &= vmask; r2 &= vmask; r3 &= vmask; }
+          ptx::mma_f16_16816(oacc[i], ptx::e4m3x2_lo_to_f16x2(r0), ptx::e4m3x2_lo_to_f16x2(r1),
+                             ptx::e4m3x2_hi_to_f16x2(r0), ptx::e4m3x2_hi_to_f16x2(r1), pb0, pb1);
+          ptx::mma_f16_16816(oacc[i + 1], ptx::e4m3x2_lo_to_f16x2(r2), ptx::e4m3x2_lo_to_f16x2(r3),
+                             ptx::e4m3x2_hi_to_f16x2(r2), ptx::e4m3x2_hi_to_f16x2(r3), pb0, pb1);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(bar_empty + 8 * stage);
+    }
+
+    // ---- segment done: O back to true units, then this warp's partial (o, m, l) -> workspace (a8)
+#pragma unroll
+    for (int i = 0; i < C::NC; ++i) { oacc[i][0] *= c_run; oacc[i][1] *= c_run; oacc[i][2] *= c_run; oacc[i][3] *= c_run; }
+#pragma unroll
+    for (int o = 4; o < 32; o <<= 1) {
+      l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], o);
+      l_run[1] += __shfl_xor_sync(0xffffffffu, l_run[1], o);
+    }
+    const int slot = (r + bid) * C::PPS + pl;
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const int n = 2 * tq + e;
+      if (n < group) {
+        const int hq = hk * group + n;
+        float* po = a.part_o + ((size_t)slot * sh.Hq + hq) * D;
+#pragma unroll
+        for (int i = 0; i < C::NC; ++i) {
+          po[16 * i + g] = oacc[i][e];
+          po[16 * i + g + 8] = oacc[i][2 + e];
+        }
+        if (g == 0) a.part_ml[(size_t)slot * sh.Hq + hq] = make_float2(m_run[e], l_run[e]);
+      }
+    }
+    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    const long long c0 = s_cum[r], c1 = s_cum[r + 1];
+    const int b_first = (int)(((c0 + 1) * G + U - 1) / U) - 1;
+    const int b_last = (int)((c1 * G + U - 1) / U) - 1;
+    const int n_parts = b_last - b_first + 1;
+    if (tid == 0) {
+      __threadfence();
+      int old = atomicAdd(&a.req_counter[r * HG + hg], 1);
+      int last = (old == n_parts - 1);
+      if (last) a.req_counter[r * HG + hg] = 0;
+      *s_flag = last;
+    }
+    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    if (*s_flag) {
+      __threadfence();
+      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane);
+    }
+    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    u = s_cum[r] + seg_hi;
+    ++r;
+  }
+}
+
+}  // namespace
+}  // namespace lazy

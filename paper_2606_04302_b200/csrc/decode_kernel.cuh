@@ -60,6 +60,54 @@ struct DecodeArgs {
   Shape sh;
 };
 
+// Split-KV combine (a8) + epilogue (a9) of request r by the LAST CTA to finish a piece of it: warp w takes q heads
+// w, w+8, ... of the CTA's head group (heads_cta of them) and merges the n_slots partials (o, m, l) that start at slot0.
+template <int D>
+__device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r, const int hg, const int heads_cta,
+                                                const int n_slots, const int slot0, const int warp, const int lane) {
+  const Shape& sh = a.sh;
+  for (int hh = warp; hh < heads_cta; hh += kConsumerWarps) {
+    const int hq = hg * heads_cta + hh;
+    // single pass with a running max; the loads of four partials are issued together so that their L2
+    // latencies overlap (the partials were written by other SMs)
+    float mstar = -INFINITY, lsum = 0.f;
+    float acc[D / 32];
+#pragma unroll
+    for (int x = 0; x < D / 32; ++x) acc[x] = 0.f;
+    for (int base = 0; base < n_slots; base += 4) {
+      float2 ml[4];
+      float2 pv[4][D / 64];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int sidx = min(base + i, n_slots - 1);
+        ml[i] = __ldcg(&a.part_ml[(size_t)(slot0 + sidx) * sh.Hq + hq]);
+        const float2* po = reinterpret_cast<const float2*>(a.part_o + ((size_t)(slot0 + sidx) * sh.Hq + hq) * D +
+                                                           lane * (D / 32));
+#pragma unroll
+        for (int x = 0; x < D / 64; ++x) pv[i][x] = __ldcg(po + x);
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        if (base + i >= n_slots || ml[i].x == -INFINITY) continue;
+        const float mnew = fmaxf(mstar, ml[i].x);
+        const float f = exp2f(mstar - mnew), w = exp2f(ml[i].x - mnew);   // mstar = -inf on the first: f = 0
+        mstar = mnew;
+        lsum = lsum * f + w * ml[i].y;
+#pragma unroll
+        for (int x = 0; x < D / 64; ++x) {
+          acc[2 * x] = acc[2 * x] * f + w * pv[i][x].x;
+          acc[2 * x + 1] = acc[2 * x + 1] * f + w * pv[i][x].y;
+        }
+      }
+    }
+    const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
+    __nv_bfloat16* op = a.out + ((size_t)r * sh.Hq + hq) * D + lane * (D / 32);
+#pragma unroll
+    for (int x = 0; x < D / 32; x += 2)
+      *reinterpret_cast<uint32_t*>(op + x) = ptx::pack_bf16(acc[x] * inv, acc[x + 1] * inv);
+  }
+}
+
 // KM = lazy_config.k_storage.  LAZY_K_UNROTATED: the identity above.  LAZY_K_STORED_POS (Eq. 6,
 // L175-182: "rotate Q" by the page's relative offset): K is consumed as stored, q is re-rotated once per page
 // by m - (p0 - stored[page]).  LAZY_K_ABSOLUTE: K as stored, q rotated once per request by m (no table rows
@@ -465,50 +513,7 @@ __device__ __forceinline__ void decode_cta(const CUtensorMap& tmap_k, const CUte
     ptx::named_bar_sync(1, kConsumerWarps * 32);
     if (*s_flag) {
       __threadfence();
-      // ---- combine (a8) + epilogue (a9): warp w takes q heads w, w+8, ... of this CTA's head group
-      const int heads_cta = HKV_CTA * group;
-      for (int hh = warp; hh < heads_cta; hh += kConsumerWarps) {
-        const int hq = hg * heads_cta + hh;
-        const int n_slots = n_parts * C::PPS;
-        const int slot0 = (r + b_first) * C::PPS;
-        // single pass with a running max; the loads of four partials are issued together so that their L2
-        // latencies overlap (the partials were written by other SMs)
-        float mstar = -INFINITY, lsum = 0.f;
-        float acc[D / 32];
-#pragma unroll
-        for (int x = 0; x < D / 32; ++x) acc[x] = 0.f;
-        for (int base = 0; base < n_slots; base += 4) {
-          float2 ml[4];
-          float2 pv[4][D / 64];
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            const int sidx = min(base + i, n_slots - 1);
-            ml[i] = __ldcg(&a.part_ml[(size_t)(slot0 + sidx) * sh.Hq + hq]);
-            const float2* po = reinterpret_cast<const float2*>(a.part_o + ((size_t)(slot0 + sidx) * sh.Hq + hq) * D +
-                                                               lane * (D / 32));
-#pragma unroll
-            for (int x = 0; x < D / 64; ++x) pv[i][x] = __ldcg(po + x);
-          }
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            if (base + i >= n_slots || ml[i].x == -INFINITY) continue;
-            const float mnew = fmaxf(mstar, ml[i].x);
-            const float f = exp2f(mstar - mnew), w = exp2f(ml[i].x - mnew);   // mstar = -inf on the first: f = 0
-            mstar = mnew;
-            lsum = lsum * f + w * ml[i].y;
-#pragma unroll
-            for (int x = 0; x < D / 64; ++x) {
-              acc[2 * x] = acc[2 * x] * f + w * pv[i][x].x;
-              acc[2 * x + 1] = acc[2 * x + 1] * f + w * pv[i][x].y;
-            }
-          }
-        }
-        const float inv = lsum > 0.f ? 1.f / lsum : 0.f;
-        __nv_bfloat16* op = a.out + ((size_t)r * sh.Hq + hq) * D + lane * (D / 32);
-#pragma unroll
-        for (int x = 0; x < D / 32; x += 2)
-          *reinterpret_cast<uint32_t*>(op + x) = ptx::pack_bf16(acc[x] * inv, acc[x + 1] * inv);
-      }
+      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane);
     }
     ptx::named_bar_sync(1, kConsumerWarps * 32);    // s_flag is reused by the next segment
     u = s_cum[r] + seg_hi;

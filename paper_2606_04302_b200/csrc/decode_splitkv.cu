@@ -24,6 +24,7 @@
 #include <climits>
 
 #include "decode_kernel.cuh"
+#include "decode_fp8_kernel.cuh"
 
 namespace lazy {
 namespace {
@@ -34,6 +35,15 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
                       const DecodeArgs a) {
   extern __shared__ unsigned char smem_raw[];
   decode_cta<D, HKV_CTA, KM>(tmap_k, tmap_v, a, (int)blockIdx.x, (int)gridDim.x, (int)blockIdx.y, (int)gridDim.y, smem_raw);
+}
+
+// LAZY_KV_FP8_E4M3 pages (decode_fp8_kernel.cuh), head_dim 128
+template <int HKV_CTA>
+__global__ void __launch_bounds__(kDecodeThreads, 1)
+decode_fp8_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
+                  const DecodeFp8Args a) {
+  extern __shared__ unsigned char smem_raw[];
+  decode_fp8_cta<HKV_CTA>(tmap_k, tmap_v, a, (int)blockIdx.x, (int)gridDim.x, (int)blockIdx.y, (int)gridDim.y, smem_raw);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -66,6 +76,21 @@ bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, in
                    const_cast<void*>(pool), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return rc == CUDA_SUCCESS;
+}
+
+// FP8 code pool: rows of D bytes; box = [box_rows][D bytes] (D = 128: one 128-byte swizzle span per row)
+bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D, int box_rows) {
+  EncodeTiledFn fn = get_encode_fn();
+  if (!fn) return false;
+  cuuint64_t gdim[2] = {(cuuint64_t)D, (cuuint64_t)rows};
+  cuuint64_t gstride[1] = {(cuuint64_t)D};
+  cuuint32_t box[2] = {(cuuint32_t)D, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1u, 1u};
+  CUresult rc = fn(reinterpret_cast<CUtensorMap*>(out_map), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
+                   const_cast<void*>(pool), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                   D == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return rc == CUDA_SUCCESS;
 }
 
@@ -107,6 +132,18 @@ static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, i
   }
 }
 
+template <int HKV_CTA>
+static int launch_decode_fp8_t(lazy_handle* h, const DecodeFp8Args& args, int grid_x, int grid_y, cudaStream_t stream) {
+  using C = DecodeFp8Cfg<HKV_CTA>;
+  auto kern = decode_fp8_kernel<HKV_CTA>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
+    return LAZY_ERR_CUDA;
+  const CUtensorMap* mk = reinterpret_cast<const CUtensorMap*>(h->tmap_k);
+  const CUtensorMap* mv = reinterpret_cast<const CUtensorMap*>(h->tmap_v);
+  kern<<<dim3(grid_x, grid_y), kDecodeThreads, C::SMEM_BYTES, stream>>>(*mk, *mv, args);
+  return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
+}
+
 int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                   const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                   int num_reqs, void* out, cudaStream_t stream) {
@@ -114,12 +151,18 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
   const int hkv_cta = c.num_kv_heads >= 8 ? 8 : c.num_kv_heads;
   const int HG = c.num_kv_heads / hkv_cta;
   const long long rows = (long long)c.num_pages * c.num_kv_heads * kPageSize;
+  const bool fp8 = c.dtype == LAZY_KV_FP8_E4M3;
+  if (fp8 && c.head_dim != 128) return LAZY_ERR_UNSUPPORTED;   // the caller routes head_dim 64 to the row-wise kernel
   if (h->tmap_k_ptr != k_cache) {
-    if (!encode_pool_tmap(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta)) return LAZY_ERR_CUDA;
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta)
+              : encode_pool_tmap(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta)))
+      return LAZY_ERR_CUDA;
     h->tmap_k_ptr = k_cache;
   }
   if (h->tmap_v_ptr != v_cache) {
-    if (!encode_pool_tmap(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta)) return LAZY_ERR_CUDA;
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta)
+              : encode_pool_tmap(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta)))
+      return LAZY_ERR_CUDA;
     h->tmap_v_ptr = v_cache;
   }
   int launches = 0;
@@ -144,7 +187,16 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
     if (gx < 1) gx = 1;
     if (gx > kMaxDecodeCtas) gx = kMaxDecodeCtas;
     int rc;
-    if (c.head_dim == 128) {
+    if (fp8) {
+      DecodeFp8Args fa;
+      fa.d = a;
+      fa.k_scale = h->k_scale;
+      fa.v_scale = h->v_scale;
+      if (hkv_cta == 8) rc = launch_decode_fp8_t<8>(h, fa, gx, HG, stream);
+      else if (hkv_cta == 4) rc = launch_decode_fp8_t<4>(h, fa, gx, HG, stream);
+      else if (hkv_cta == 2) rc = launch_decode_fp8_t<2>(h, fa, gx, HG, stream);
+      else rc = launch_decode_fp8_t<1>(h, fa, gx, HG, stream);
+    } else if (c.head_dim == 128) {
       if (hkv_cta == 8) rc = launch_decode_t<128, 8>(h, a, gx, HG, stream);
       else if (hkv_cta == 4) rc = launch_decode_t<128, 4>(h, a, gx, HG, stream);
       else if (hkv_cta == 2) rc = launch_decode_t<128, 2>(h, a, gx, HG, stream);

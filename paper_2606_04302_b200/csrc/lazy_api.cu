@@ -20,7 +20,9 @@ bool config_supported(const lazy_config* c) {
   if (c->num_q_heads / c->num_kv_heads > 8) return false;
   int hkv = c->num_kv_heads;
   if (!(hkv == 1 || hkv == 2 || hkv == 4 || hkv % 8 == 0)) return false;
-  if (c->dtype != 0) return false;
+  if (c->dtype != LAZY_KV_BF16 && c->dtype != LAZY_KV_FP8_E4M3) return false;
+  if (c->dtype == LAZY_KV_FP8_E4M3 && (c->rope_style != LAZY_ROPE_HALF_SPLIT || c->k_storage != LAZY_K_UNROTATED))
+    return false;
   if (c->rope_style < LAZY_ROPE_HALF_SPLIT || c->rope_style > LAZY_POS_ALIBI) return false;
   if (c->rope_style == LAZY_POS_ALIBI && (c->k_storage != LAZY_K_UNROTATED || c->num_q_heads > lazy::kMaxAlibiHeads))
     return false;
@@ -129,6 +131,7 @@ int lazy_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const
   if (!h || num_tokens < 0) return LAZY_ERR_INVALID;
   if (num_tokens == 0) return LAZY_OK;
   if (!k_new || !v_new || !slot_mapping || !k_cache || !v_cache) return LAZY_ERR_INVALID;
+  if (h->cfg.dtype == LAZY_KV_FP8_E4M3 && !h->k_scale) return LAZY_ERR_INVALID;
   if (misaligned(k_new) || misaligned(v_new) || misaligned(k_cache) || misaligned(v_cache) ||
       (reinterpret_cast<uintptr_t>(slot_mapping) & 7u))
     return LAZY_ERR_INVALID;
@@ -172,10 +175,19 @@ int lazy_set_page_stored_pos(lazy_handle* h, const int32_t* page_stored_pos) {
   return LAZY_OK;
 }
 
+int lazy_set_kv_scales(lazy_handle* h, float* k_scale, float* v_scale) {
+  if (!h || !k_scale || !v_scale || misaligned(k_scale) || misaligned(v_scale)) return LAZY_ERR_INVALID;
+  if (h->cfg.dtype != LAZY_KV_FP8_E4M3) return LAZY_ERR_UNSUPPORTED;
+  h->k_scale = k_scale;
+  h->v_scale = v_scale;
+  return LAZY_OK;
+}
+
 int lazy_materialize_pages(lazy_handle* h, const void* k_src, const void* v_src, const int32_t* src_pages,
                            const int32_t* rot_pos, int32_t per_token, void* k_dst, void* v_dst,
                            const int32_t* dst_pages, int32_t num, void* stream) {
   if (!h || num < 0) return LAZY_ERR_INVALID;
+  if (h->cfg.dtype != LAZY_KV_BF16) return LAZY_ERR_UNSUPPORTED;
   if (num == 0) return LAZY_OK;
   if (!k_src || !k_dst || !src_pages || !rot_pos || !dst_pages) return LAZY_ERR_INVALID;
   if (misaligned(k_src) || misaligned(k_dst) || misaligned(v_src) || misaligned(v_dst) ||
@@ -194,6 +206,7 @@ static int check_attn_args(lazy_handle* h, const void* q, const void* k_cache, c
                            const int32_t* seq_lens, int32_t num_reqs, void* out) {
   if (!h || num_reqs < 0) return LAZY_ERR_INVALID;
   if (h->cfg.k_storage == LAZY_K_STORED_POS && !h->page_stored_pos) return LAZY_ERR_INVALID;
+  if (h->cfg.dtype == LAZY_KV_FP8_E4M3 && !h->k_scale) return LAZY_ERR_INVALID;
   if (num_reqs > h->cfg.max_reqs) return LAZY_ERR_INVALID;
   if (num_reqs == 0) return LAZY_OK;
   if (!q || !k_cache || !v_cache || !block_table || !page_logical_pos || !seq_lens || !out)
@@ -216,7 +229,7 @@ int lazy_attn_prefill(lazy_handle* h, const void* q, const void* k_cache, const 
   if (!cu_q_lens || (reinterpret_cast<uintptr_t>(cu_q_lens) & 3u) || max_q_len == 0) return LAZY_ERR_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   int n;
-  if (h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS)
+  if ((h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS) || h->cfg.dtype == LAZY_KV_FP8_E4M3)
     n = lazy::launch_rowwise(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, cu_q_lens,
                              num_reqs, total_q, max_q_len, out, s);
   else
@@ -235,7 +248,8 @@ int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const v
   if (num_reqs == 0) return LAZY_OK;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   int n;
-  if (h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS)
+  // FP8 pages at head_dim 64 have no split-KV kernel: they run on the row-wise CUDA kernel
+  if ((h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS) || (h->cfg.dtype == LAZY_KV_FP8_E4M3 && h->cfg.head_dim != 128))
     n = lazy::launch_rowwise(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, nullptr,
                              num_reqs, num_reqs, 1, out, s);
   else

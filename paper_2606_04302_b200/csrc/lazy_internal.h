@@ -40,6 +40,8 @@ struct lazy_handle {
   int num_sms;
   int64_t launches;
   const int32_t* page_stored_pos;   // LAZY_K_STORED_POS: device [num_pages], caller-owned
+  float* k_scale;                   // LAZY_KV_FP8_E4M3: device [num_pages][Hkv][16] per-row scales, caller-owned
+  float* v_scale;
   int decode_cta_limit;             // > 0: lazy_attn_mixed confines the decode kernel to this many CTAs (= SMs)
   cudaStream_t side_stream;         // lazy_attn_mixed: library-owned fork stream and its two events (host resources)
   cudaEvent_t ev_fork, ev_join;
@@ -65,12 +67,19 @@ namespace lazy {
 //   q    : 4-D view (D, group, Hkv, total_q) of q [total_q][Hq][D], box = (64, group, 1, tokens_per_tile):
 //          lands as rows token*group + head-in-group of one kv head's GQA group.
 bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, int box_rows);
+bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D, int box_rows);
 bool encode_q_tmap(void* out_map, const void* q, int total_q, int Hq, int Hkv, int D, int tokens_per_tile);
 
 // Each launcher enqueues on `stream` and returns the number of kernels launched (<0: LAZY_ERR_*).
 int launch_build_tables(lazy_handle* h, const double* inv_freq_host, cudaStream_t stream);
 int launch_cache_write(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
                        int num_tokens, void* k_cache, void* v_cache, cudaStream_t stream);
+// LAZY_KV_FP8_E4M3 (fp8_kernels.cu): quantising cache write, row-wise debug attention over FP8 pages
+int launch_cache_write_fp8(lazy_handle* h, const void* k_new, const void* v_new, const int64_t* slot_mapping,
+                           int num_tokens, void* k_cache, void* v_cache, cudaStream_t stream);
+int launch_rowwise_fp8(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
+                       const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
+                       const int32_t* cu_q_lens, int num_reqs, int total_q, void* out, cudaStream_t stream);
 int launch_materialize(lazy_handle* h, const void* k_src, const void* v_src, const int32_t* src_pages,
                        const int32_t* rot_pos, int per_token, void* k_dst, void* v_dst, const int32_t* dst_pages,
                        int num, cudaStream_t stream);

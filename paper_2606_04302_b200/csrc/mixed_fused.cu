@@ -54,7 +54,7 @@ int launch_mixed_t(const lazy_handle* h, const DecodeArgs& da, const PrefillArgs
 
 bool mixed_fused_supported(const lazy_handle* h, int num_reqs_decode) {
   const lazy_config& c = h->cfg;
-  return c.head_dim == 128 && c.k_storage == LAZY_K_UNROTATED && c.rope_style != LAZY_POS_ALIBI &&
+  return c.dtype == LAZY_KV_BF16 && c.head_dim == 128 && c.k_storage == LAZY_K_UNROTATED && c.rope_style != LAZY_POS_ALIBI &&
          (c.num_kv_heads == 4 || c.num_kv_heads == 8) && num_reqs_decode <= kMaxReqsSmem &&
          !(c.flags & (LAZY_FLAG_ROWWISE_KERNELS | LAZY_FLAG_PREFILL_ONE_CTA));
 }

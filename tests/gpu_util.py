@@ -66,3 +66,46 @@ def run_and_compare(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, 
     finally:
         dev.close()
     return all_stats
+
+
+def run_and_compare_fp8(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, scale_abs_by_output: bool = False,
+                        gates=None, dev_kw=None):
+    """FP8 KV pages (LAZY_KV_FP8_E4M3): the library quantises (lazy_cache_write), the oracle quantises its own copy;
+    codes and scales must agree BIT FOR BIT after every step (integer decisions taken in fp32 on both sides), and the
+    attention outputs must match the oracle's exact-dequantisation result under the same gates as the bf16 path."""
+    from paper_2606_04302_b200 import binding as B
+    dev = DeviceBatch(batch, flags=flags, dtype=B.LAZY_KV_FP8_E4M3, **(dev_kw or {}))
+    pools = O.quantize_pool_fp8(batch.k_pool, batch.v_pool)
+    rng = np.random.default_rng(seed)
+    all_stats = []
+
+    def check_pools(si):
+        kc, vc = dev.k_pool.cpu().numpy(), dev.v_pool.cpu().numpy()
+        ks, vs = dev.k_scale.cpu().numpy().view(np.uint32), dev.v_scale.cpu().numpy().view(np.uint32)
+        valid = ~np.isnan(pools.k_scale)
+        assert np.array_equal(np.isnan(dev.k_scale.cpu().numpy()), ~valid), f"step {si}: which rows are written"
+        assert np.array_equal(ks[valid], pools.k_scale.view(np.uint32)[valid]), f"step {si}: K scales"
+        assert np.array_equal(vs[valid], pools.v_scale.view(np.uint32)[valid]), f"step {si}: V scales"
+        assert np.array_equal(kc, pools.k_codes), f"step {si}: K codes"
+        assert np.array_equal(vc, pools.v_codes), f"step {si}: V codes"
+
+    try:
+        check_pools(-1)
+        for si, step in enumerate(batch.steps):
+            got = dev.run_step(step)
+            torch.cuda.synchronize()
+            sel = rows = None
+            if step.q is not None and sample_rows and step.q.shape[0] > sample_rows:
+                rows = np.sort(rng.choice(step.q.shape[0], size=sample_rows, replace=False))
+                sel = np.zeros(step.q.shape[0], dtype=np.uint8)
+                sel[rows] = 1
+            ref = O.run_step_fp8(batch, step, pools, row_select=sel)
+            check_pools(si)
+            if got is not None:
+                sc = max(1.0, float(np.abs(ref).max())) if scale_abs_by_output else 1.0
+                kw = dict(abs_scale=sc)
+                kw.update(gates or {})
+                all_stats.append(compare(got, ref, f"{batch.name} fp8 step {si} ({step.kind})", rows=rows, **kw))
+    finally:
+        dev.close()
+    return all_stats

@@ -1,0 +1,100 @@
+"""-m gpu parity tests of LAZY_KV_FP8_E4M3 pages: the quantising lazy_cache_write bit for bit
+against the oracle's, and the attention calls against the oracle's exact-dequantisation result.  The tolerance is the
+bf16 contract (max abs 2e-2, mean abs 2e-3) and the same normalised gates: both sides start from identical codes and
+scales, so the FP8 quantisation error itself is not part of the comparison."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_04302_b200 import binding as B
+from paper_2606_04302_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+FLAGS = [pytest.param(0, id="prod"), pytest.param(B.LAZY_FLAG_ROWWISE_KERNELS, id="rowwise")]
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    from paper_2606_04302_b200 import build
+    build.build()
+    B.lib()
+
+
+def _run(batch, **kw):
+    from gpu_util import run_and_compare_fp8
+    return run_and_compare_fp8(batch, **kw)
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+def test_fp8_config1_tiny(flags):
+    stats = _run(W.config1(), flags=flags)
+    assert len(stats) == 2
+    assert all(s["max_abs"] < 5e-3 for s in stats), stats
+
+
+@pytest.mark.parametrize("flags", FLAGS)
+@pytest.mark.parametrize("cfg,scale", [(2, 0.25), (3, 0.07), (4, 0.25), (5, 0.25)])
+def test_fp8_configs_reduced_full_compare(cfg, scale, flags):
+    _run(W.CONFIGS[cfg](scale=scale), flags=flags)
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_fp8_configs_peaked_queries(cfg):
+    scale = {2: 0.1, 3: 0.07, 4: 0.25, 5: 0.25}[cfg]
+    _run(W.CONFIGS[cfg](scale=scale, q_scale=4.0), scale_abs_by_output=True)
+
+
+def test_fp8_cache_write_edge_rows():
+    """All-zero rows (scale 1, codes 0), huge and tiny magnitudes, skipped slots, a partially written page."""
+    from oracle import oracle as O
+    torch.manual_seed(3)
+    Hkv, D, P, T = 2, 128, 16, 40
+    dev = torch.device("cuda")
+    h = B.lazy_create(4, Hkv, D, num_pages=4, max_position=256, max_reqs=1, max_pages_per_req=4, rope_theta=1e4,
+                      dtype=B.LAZY_KV_FP8_E4M3, device=dev)
+    kc = torch.full((4, Hkv, P, D), 0x7f, dtype=torch.uint8, device=dev)
+    vc = torch.full((4, Hkv, P, D), 0x7f, dtype=torch.uint8, device=dev)
+    ks = torch.full((4, Hkv, P), float("nan"), dtype=torch.float32, device=dev)
+    vs = torch.full((4, Hkv, P), float("nan"), dtype=torch.float32, device=dev)
+    B.lazy_set_kv_scales(h, ks, vs)
+    k = torch.randn(T, Hkv, D).to(torch.bfloat16)
+    v = torch.randn(T, Hkv, D).to(torch.bfloat16)
+    k[0] = 0
+    v[1] = 0
+    k[2] *= 1e30
+    v[3] *= 1e-30
+    k[4, 0, 5] = 3e38
+    v[5] = torch.where(torch.rand(Hkv, D) < 0.5, 1.0, -1.0).to(torch.bfloat16) * 7
+    slots = torch.arange(T, dtype=torch.int64) + 5
+    slots[7] = -1
+    B.lazy_cache_write(h, k.to(dev), v.to(dev), slots.to(dev), kc, vc)
+    torch.cuda.synchronize()
+    pools = O.Fp8Pools(4, Hkv, P, D)
+    O.cache_write_fp8(k, v, slots.numpy(), pools)
+    assert np.array_equal(kc.cpu().numpy(), pools.k_codes)
+    assert np.array_equal(vc.cpu().numpy(), pools.v_codes)
+    assert np.array_equal(ks.cpu().numpy().view(np.uint32), pools.k_scale.view(np.uint32))
+    assert np.array_equal(vs.cpu().numpy().view(np.uint32), pools.v_scale.view(np.uint32))
+    h.close()
+
+
+def test_fp8_needs_scales_and_rejects_unsupported_modes():
+    dev = torch.device("cuda")
+    with pytest.raises(B.LazyError):
+        B.lazy_create(4, 1, 64, num_pages=4, max_position=256, max_reqs=1, max_pages_per_req=4, rope_theta=1e4,
+                      dtype=B.LAZY_KV_FP8_E4M3, k_storage=B.LAZY_K_STORED_POS, device=dev)
+    h = B.lazy_create(4, 1, 64, num_pages=4, max_position=256, max_reqs=1, max_pages_per_req=4, rope_theta=1e4,
+                      dtype=B.LAZY_KV_FP8_E4M3, device=dev)
+    kc = torch.zeros(4, 1, 16, 64, dtype=torch.uint8, device=dev)
+    k = torch.zeros(1, 1, 64, dtype=torch.bfloat16, device=dev)
+    with pytest.raises(B.LazyError) as e:
+        B.lazy_cache_write(h, k, k, torch.zeros(1, dtype=torch.int64, device=dev), kc, kc)
+    assert e.value.status == B.LAZY_ERR_INVALID
+    h.close()
+    hb = B.lazy_create(4, 1, 64, num_pages=4, max_position=256, max_reqs=1, max_pages_per_req=4, rope_theta=1e4,
+                       device=dev)
+    with pytest.raises(B.LazyError) as e:
+        B.lazy_set_kv_scales(hb, torch.zeros(64, device=dev), torch.zeros(64, device=dev))
+    assert e.value.status == B.LAZY_ERR_UNSUPPORTED
+    hb.close()
