@@ -77,6 +77,8 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
   const uint32_t bar_full = smem_base + C::OFF_BAR;
   const uint32_t bar_empty = bar_full + C::NSTAGES * 8;
   int* s_flag = reinterpret_cast<int*>(smem + C::OFF_BAR + 2 * C::NSTAGES * 8);
+  const uint32_t bar_comb = bar_empty + C::NSTAGES * 8 + 8;     // bulk-copy combine (combine_request)
+  uint32_t comb_phase = 0;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int R = a.num_reqs;
@@ -89,6 +91,7 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
       ptx::mbar_init(bar_full + 8 * s, 1);
       ptx::mbar_init(bar_empty + 8 * s, kConsumerWarps);
     }
+    ptx::mbar_init(bar_empty + C::NSTAGES * 8 + 8, 1);
     ptx::fence_mbar_init();
   }
   if (warp == kConsumerWarps && lane == 0) {
@@ -411,7 +414,9 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
     ptx::named_bar_sync(1, kConsumerWarps * 32);
     if (*s_flag) {
       __threadfence();
-      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane);
+      // the ring is idle iff this segment ends the CTA's range (every issued stage has been consumed)
+      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane,
+                         s_cum[r] + seg_hi == u_end, smem_base, C::NSTAGES * C::STAGE_BYTES, bar_comb, comb_phase);
     }
     ptx::named_bar_sync(1, kConsumerWarps * 32);
     u = s_cum[r] + seg_hi;

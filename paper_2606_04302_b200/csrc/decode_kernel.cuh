@@ -62,10 +62,102 @@ struct DecodeArgs {
 
 // Split-KV combine (a8) + epilogue (a9) of request r by the LAST CTA to finish a piece of it: warp w takes q heads
 // w, w+8, ... of the CTA's head group (heads_cta of them) and merges the n_slots partials (o, m, l) that start at slot0.
+//
+// Two paths.  When the combining CTA has finished its whole range (the usual case: a request's last arriver is a CTA
+// whose piece of it ENDS its range) the pipeline ring is idle, and the partial outputs are pulled into it with bulk
+// async copies -- one per slot, all heads of the CTA's head group are contiguous there -- so that every byte of the
+// request's partials is in flight at once; the warps then merge out of shared memory.  (Round 1 / early round 2: the
+// warps loaded four slots at a time from L2 / HBM, ~0.9 us per dependent batch: 16 us for the 20 slots x 28 heads of a
+// cfg-5 request, which held that decode under 70 % of the HBM roofline.)  Otherwise (the ring still holds pages of the
+// CTA's next request) the register path below runs.
 template <int D>
 __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r, const int hg, const int heads_cta,
-                                                const int n_slots, const int slot0, const int warp, const int lane) {
+                                                const int n_slots, const int slot0, const int warp, const int lane,
+                                                const bool ring_free, const uint32_t ring_u32, const int ring_bytes,
+                                                const uint32_t cbar, uint32_t& cphase) {
   const Shape& sh = a.sh;
+  const int slot_bytes = heads_cta * D * 4;
+  if (ring_free && slot_bytes <= ring_bytes) {
+    const int cap = min(32, ring_bytes / slot_bytes);
+    const int hpw = (heads_cta + kConsumerWarps - 1) / kConsumerWarps;      // heads per warp (<= 8)
+    float mstar[8], lsum[8], acc[8][D / 32];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      mstar[k] = -INFINITY; lsum[k] = 0.f;
+#pragma unroll
+      for (int x = 0; x < D / 32; ++x) acc[k][x] = 0.f;
+    }
+    for (int base = 0; base < n_slots; base += cap) {
+      const int n = min(cap, n_slots - base);
+      if (warp == 0) {
+        if (lane == 0) {
+          ptx::fence_proxy_async();                 // the partials were written through the generic proxy
+          ptx::mbar_arrive_expect_tx(cbar, (uint32_t)(n * slot_bytes));
+        }
+        __syncwarp();
+        if (lane < n)
+          ptx::bulk_load_1d(ring_u32 + lane * slot_bytes,
+                            a.part_o + ((size_t)(slot0 + base + lane) * sh.Hq + hg * heads_cta) * D, slot_bytes, cbar);
+      }
+      // (m, l) of slot base + lane for each of this warp's heads, issued before the wait
+      float2 ml[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int hh = warp + k * kConsumerWarps;
+        ml[k] = make_float2(-INFINITY, 0.f);
+        if (k < hpw && hh < heads_cta && lane < n)
+          ml[k] = __ldcg(&a.part_ml[(size_t)(slot0 + base + lane) * sh.Hq + hg * heads_cta + hh]);
+      }
+      ptx::mbar_wait(cbar, cphase);
+      cphase ^= 1;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        const int hh = warp + k * kConsumerWarps;
+        if (k < hpw && hh < heads_cta) {
+          float mx = ml[k].x;
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+          const float mnew = fmaxf(mstar[k], mx);
+          if (mnew > -INFINITY) {                   // warp-uniform
+            const float f = exp2f(mstar[k] - mnew);                       // mstar = -inf on the first round: 0
+            const float w = ml[k].x == -INFINITY ? 0.f : exp2f(ml[k].x - mnew);
+            float wl = w * ml[k].y;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) wl += __shfl_xor_sync(0xffffffffu, wl, o);
+            mstar[k] = mnew;
+            lsum[k] = lsum[k] * f + wl;
+#pragma unroll
+            for (int x = 0; x < D / 32; ++x) acc[k][x] *= f;
+            const uint32_t src = ring_u32 + hh * (D * 4) + lane * (D / 32) * 4;
+            for (int i = 0; i < n; ++i) {
+              const float wi = __shfl_sync(0xffffffffu, w, i);
+              if (D == 128) {
+                const float4 v = ptx::lds128f(src + i * slot_bytes);
+                acc[k][0] += wi * v.x; acc[k][1] += wi * v.y; acc[k][D / 32 - 2] += wi * v.z; acc[k][D / 32 - 1] += wi * v.w;
+              } else {
+                const float4 v = ptx::lds128f((src + i * slot_bytes) & ~15u);   // 8-byte pieces: pick the lane's half
+                const bool hi = lane & 1;
+                acc[k][0] += wi * (hi ? v.z : v.x); acc[k][1] += wi * (hi ? v.w : v.y);
+              }
+            }
+          }
+        }
+      }
+      if (base + cap < n_slots) ptx::named_bar_sync(1, kConsumerWarps * 32);   // the next round overwrites the ring
+    }
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const int hh = warp + k * kConsumerWarps;
+      if (k < hpw && hh < heads_cta) {
+        const float inv = lsum[k] > 0.f ? 1.f / lsum[k] : 0.f;
+        __nv_bfloat16* op = a.out + ((size_t)r * sh.Hq + hg * heads_cta + hh) * D + lane * (D / 32);
+#pragma unroll
+        for (int x = 0; x < D / 32; x += 2)
+          *reinterpret_cast<uint32_t*>(op + x) = ptx::pack_bf16(acc[k][x] * inv, acc[k][x + 1] * inv);
+      }
+    }
+    return;
+  }
   for (int hh = warp; hh < heads_cta; hh += kConsumerWarps) {
     const int hq = hg * heads_cta + hh;
     // single pass with a running max; the loads of four partials are issued together so that their L2
@@ -130,6 +222,8 @@ __device__ __forceinline__ void decode_cta(const CUtensorMap& tmap_k, const CUte
   const uint32_t bar_full = smem_base + C::OFF_BAR;
   const uint32_t bar_empty = bar_full + C::NSTAGES * 8;
   int* s_flag = reinterpret_cast<int*>(smem + C::OFF_BAR + 2 * C::NSTAGES * 8);
+  const uint32_t bar_comb = bar_empty + C::NSTAGES * 8 + 8;     // bulk-copy combine (combine_request)
+  uint32_t comb_phase = 0;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int R = a.num_reqs;
@@ -142,6 +236,7 @@ __device__ __forceinline__ void decode_cta(const CUtensorMap& tmap_k, const CUte
       ptx::mbar_init(bar_full + 8 * s, 1);
       ptx::mbar_init(bar_empty + 8 * s, kConsumerWarps);
     }
+    ptx::mbar_init(bar_empty + C::NSTAGES * 8 + 8, 1);
     ptx::fence_mbar_init();
   }
   if (warp == kConsumerWarps && lane == 0) {
@@ -513,7 +608,9 @@ __device__ __forceinline__ void decode_cta(const CUtensorMap& tmap_k, const CUte
     ptx::named_bar_sync(1, kConsumerWarps * 32);
     if (*s_flag) {
       __threadfence();
-      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane);
+      // the ring is idle iff this segment ends the CTA's range (every issued stage has been consumed)
+      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane,
+                         s_cum[r] + seg_hi == u_end, smem_base, C::NSTAGES * C::STAGE_BYTES, bar_comb, comb_phase);
     }
     ptx::named_bar_sync(1, kConsumerWarps * 32);    // s_flag is reused by the next segment
     u = s_cum[r] + seg_hi;
