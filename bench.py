@@ -117,8 +117,9 @@ def make_batch(workload: str, rank: int, noshare: bool = False):
     return b
 
 
-def step_work(batch, steps):
-    """Algorithmic work of the timed attention calls."""
+def step_work(batch, steps, fp8=False):
+    """Algorithmic work of the timed attention calls.  fp8: LAZY_KV_FP8_E4M3
+    pages move D bytes of codes + one fp32 scale per (token, kv head), for K and for V: 2*(D + 4) B instead of 4*D."""
     sh = batch.shape
     logical = 0          # decode: K and V once per (token, kv head): 2*D*2 B, + q/out
     flops = 0            # prefill: 4*D FLOPs per visible (query, key) pair per q head
@@ -126,7 +127,7 @@ def step_work(batch, steps):
     for st in steps:
         L = st.seq_lens.numpy().astype(np.int64)
         if st.kind == "decode":
-            logical += int(L.sum()) * sh.num_kv_heads * sh.head_dim * 2 * 2
+            logical += int(L.sum()) * sh.num_kv_heads * (2 * (sh.head_dim + 4) if fp8 else sh.head_dim * 2 * 2)
             logical += len(L) * sh.num_q_heads * sh.head_dim * 2 * 2
             dec_tokens += len(L)
             kv_tokens += int(L.sum())
@@ -154,12 +155,12 @@ def unique_bytes(batch, steps):
 class GpuJob:
     """Holds the device-resident batch and replays its timed step."""
 
-    def __init__(self, batch, device):
+    def __init__(self, batch, device, fp8=False):
         from paper_2606_04302_b200.runner import DeviceBatch
         from paper_2606_04302_b200 import binding as B
         self.B = B
         self.batch = batch
-        self.dev = DeviceBatch(batch, device=device)
+        self.dev = DeviceBatch(batch, device=device, dtype=B.LAZY_KV_FP8_E4M3 if fp8 else B.LAZY_KV_BF16)
         d = self.dev.device
         self.timed = []
         for st in batch.steps:
@@ -511,18 +512,42 @@ def oracle_sample(workload, batch, budget_s=20.0):
     return v, t_total, "; ".join(desc), O.num_threads()
 
 
-def _timed_job(workload, device, steps, noshare=False, warmup=3):
+def _timed_job(workload, device, steps, noshare=False, warmup=3, fp8=False):
     b = make_batch(workload, 0, noshare)
-    j = GpuJob(b, device)
-    w = step_work(b, [r["step"] for r in j.timed])
+    j = GpuJob(b, device, fp8=fp8)
+    w = step_work(b, [r["step"] for r in j.timed], fp8=fp8)
     return b, j, w
 
 
-def decode_noshare_leg(workload, device, steps, barrier):
-    b, j, w = _timed_job(workload, device, steps, noshare=True)
+def decode_noshare_leg(workload, device, steps, barrier, fp8=False):
+    b, j, w = _timed_job(workload, device, steps, noshare=True, fp8=fp8)
     _, a_ms, _ = j.time_steps(steps, 3, barrier)
     j.dev.close()
     return dict(kernel_ms=a_ms / steps, bytes=w["logical_bytes"])
+
+
+def fp8_leg(device, steps, peaks, barrier):
+    """the decode configs on LAZY_KV_FP8_E4M3 pages (E4M3 codes + one fp32 scale per row), noshare
+    variants, against the HBM roofline on the HALVED algorithmic bytes (264 B per (token, kv head) at head_dim 128)."""
+    res = {"dtype": "fp8_e4m3 pages (bf16 q / out, f16 tensor operands, fp32 accumulate)",
+           "bytes_per_token_kv_head": 264}
+    for wl in ("cfg2", "cfg4", "cfg5"):
+        b, j, w = _timed_job(wl, device, steps, noshare=True, fp8=True)
+        if wl == "cfg5":
+            per = j.time_calls(steps, 3)
+            wd = step_work(b, [r["step"] for r in j.timed if r["step"].kind == "decode"], fp8=True)
+            ms, nbytes = per["decode"], wd["logical_bytes"]
+        else:
+            _, a_ms, _ = j.time_steps(steps, 3, barrier)
+            ms, nbytes = a_ms / steps, w["logical_bytes"]
+        j.dev.close()
+        del j, b
+        torch.cuda.empty_cache()
+        gb = nbytes / (ms * 1e-3) / 1e9
+        res[wl + "_noshare"] = {"kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes, "GBps": gb,
+                                "frac_of_hbm_peak": gb / peaks["hbm"],
+                                "traffic": ncu_traffic("decode_fp8", wl + "_noshare")}
+    return res
 
 
 def decode_leg(workload, device, steps, peaks, barrier):
@@ -630,6 +655,8 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--noshare", action="store_true", help="every drawn document distinct (logical == unique bytes)")
+    ap.add_argument("--kv-dtype", default="bf16", choices=["bf16", "fp8"],
+                    help="fp8: LAZY_KV_FP8_E4M3 pages (decode workloads cfg2 / cfg4; SURVEY 8.0 row f4)")
     ap.add_argument("--no-secondary", action="store_true", help="skip the prefill (cfg3) and noshare side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mixed", action="store_true",
@@ -694,9 +721,11 @@ def main():
         lazy_build.build()
     barrier()
 
+    fp8 = args.kv_dtype == "fp8"
+    assert not fp8 or args.workload in ("cfg2", "cfg4"), "--kv-dtype fp8 times the decode workloads (cfg2, cfg4)"
     batch = make_batch(args.workload, rank, args.noshare)
-    job = GpuJob(batch, device)
-    work = step_work(batch, [r["step"] for r in job.timed])
+    job = GpuJob(batch, device, fp8=fp8)
+    work = step_work(batch, [r["step"] for r in job.timed], fp8=fp8)
     sampler = ClockSampler(local_rank)
     sampler.start()
     total_ms, attn_ms, launches = job.time_steps(args.steps, args.warmup, barrier)
@@ -735,11 +764,12 @@ def main():
         if args.noshare:
             ns = dict(kernel_ms=ms_attn, bytes=work["logical_bytes"])
         else:
-            ns = decode_noshare_leg(args.workload, device, max(5, args.steps // 2), barrier)
+            ns = decode_noshare_leg(args.workload, device, max(5, args.steps // 2), barrier, fp8=fp8)
         ach = ns["bytes"] / (ns["kernel_ms"] * 1e-3) / 1e9
         roof = {"bound": "hbm", "kernel": "lazy_attn_decode (split-KV + combine)", "achieved": ach,
                 "peak": peaks["hbm"], "unit": "GB/s", "frac": ach / peaks["hbm"],
-                "traffic": ncu_traffic("decode", args.workload + "_noshare"), "peak_source": peaks["source"],
+                "traffic": ncu_traffic("decode_fp8" if fp8 else "decode", args.workload + "_noshare"),
+                "peak_source": peaks["source"],
                 "workload": args.workload + " noshare (every drawn document distinct: algorithmic == DRAM bytes)",
                 "algorithmic_bytes_per_launch": ns["bytes"], "kernel_ms": ns["kernel_ms"]}
         if not args.noshare:
@@ -762,8 +792,8 @@ def main():
 
     out = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-        "data": "synthetic",
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "fp8_e4m3 KV pages, bf16 q/out" if fp8 else "bf16", "data": "synthetic",
         "config": {"workload": args.workload + (" noshare" if args.noshare else ""), "batch": batch.name,
                    "heads": [batch.shape.num_q_heads, batch.shape.num_kv_heads, batch.shape.head_dim],
                    "num_reqs": int(sum(len(r["step"].seq_lens) for r in job.timed)),
@@ -839,14 +869,15 @@ def main():
     del job
     torch.cuda.empty_cache()
 
-    if rank == 0 and world == 1 and not args.no_secondary and args.workload == "cfg2":
+    if rank == 0 and world == 1 and not args.no_secondary and args.workload == "cfg2" and not fp8:
         # side measurements in the same run, so that the driver's record carries all five configs: the prefill headline
         # (configs[2]) as a burst and as a seconds-long run, the long-context decode (configs[3]) and the mixed step
         # (configs[4]) kernel by kernel.  configs[0] is the parity-test case.
         side = {}
         for name, fn in (("cfg3", lambda: prefill_leg("cfg3", device, max(5, args.steps // 3), peaks, barrier)),
                          ("cfg4", lambda: decode_leg("cfg4", device, max(5, args.steps // 2), peaks, barrier)),
-                         ("cfg5", lambda: cfg5_leg(device, max(5, args.steps // 2), peaks))):
+                         ("cfg5", lambda: cfg5_leg(device, max(5, args.steps // 2), peaks)),
+                         ("fp8_pages", lambda: fp8_leg(device, max(5, args.steps // 2), peaks, barrier))):
             try:
                 side[name] = fn()
             except Exception as e:  # a side measurement must not lose the headline

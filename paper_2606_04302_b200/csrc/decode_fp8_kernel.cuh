@@ -11,7 +11,8 @@
 //   * V codes come out of shared memory already transposed AND still 8-bit with the 8-bit transposing ldmatrix
 //     (m16n16.b8: thread (g, tq) gets tokens 4tq..4tq+3 of dims g, g+8), are widened to f16x2 and used as the A
 //     operand; that fixes which MMA k-slot holds which token, and the token -> MMA-row order of the QK^T product is
-//     chosen to match (row i <-> token (i>>1) + 4(i&1) + (i&8)), which also makes the K loads bank-conflict-free;
+//     chosen to match, with the ldmatrix row addresses permuted so that both the K loads and the V loads are
+//     bank-conflict-free (token order tau in the kernel);
 //   * the V scale of a token multiplies P (fp32, then f16) relative to a running reference scale c_run carried like
 //     the softmax maximum: P' = p * sv / c_run, O accumulates in units of c_run and is rescaled only when a page's
 //     largest V scale leaves [c_run/64, 64 c_run] (f16 has the range: P' <= 64).
@@ -61,7 +62,12 @@ __device__ __forceinline__ uint32_t h2fma(uint32_t a, uint32_t b, uint32_t c) {
                             *reinterpret_cast<const __half2*>(&c));
   return *reinterpret_cast<const uint32_t*>(&r);
 }
-__device__ __forceinline__ uint32_t h2neg(uint32_t a) { return a ^ 0x80008000u; }
+// a * b - c * d on packed halves (the negation folds into an operand modifier)
+__device__ __forceinline__ uint32_t h2mulsub(uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  const __half2 r = __hfma2(__hneg2(*reinterpret_cast<const __half2*>(&c)), *reinterpret_cast<const __half2*>(&d),
+                            __hmul2(*reinterpret_cast<const __half2*>(&a), *reinterpret_cast<const __half2*>(&b)));
+  return *reinterpret_cast<const uint32_t*>(&r);
+}
 
 template <int HKV_CTA>
 __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const CUtensorMap& tmap_v,
@@ -196,8 +202,8 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
   const int hl = warp % HKV_CTA;
   const int hk = hg * HKV_CTA + hl;
   const int group = sh.group;
-  // MMA row g of the QK^T tile is token t0, row g + 8 token t0 + 8 (see the header: the order the V fragments fix)
-  const int t0 = (g >> 1) + 4 * (g & 1);
+  // MMA row g of the QK^T tile is token t0, row g + 8 token t0 + 2 (see the header: the order the V fragments fix)
+  const int t0 = 8 * (g >> 2) + 4 * (g & 1) + ((g >> 1) & 1);
 
   // in-page rotation constants of this thread's two tokens and 16 pairs, as f16x2 (cos j, cos j+1) / (sin j, sin j+1)
   uint32_t ctc[2][C::NL], cts[2][C::NL];
@@ -207,13 +213,15 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
     for (int rw = 0; rw < 2; ++rw)
 #pragma unroll
       for (int w = 0; w < C::NL; ++w) {
-        const float4 v = __ldg(cs4 + (size_t)(t0 + 8 * rw) * (D / 4) + w * 4 + tq);
+        const float4 v = __ldg(cs4 + (size_t)(t0 + 2 * rw) * (D / 4) + w * 4 + tq);
         ctc[rw][w] = ptx::pack_f16(v.x, v.y);
         cts[rw][w] = ptx::pack_f16(v.z, v.w);
       }
   }
-  // ldmatrix row address of this lane inside a (page, head) V tile: matrix row i = lane & 15 is token (i>>2) + 4(i&3)
-  const int vtok = ((lane & 15) >> 2) + 4 * (lane & 3);
+  // ldmatrix row address of this lane inside a (page, head) V tile: matrix row i = 4a + b (lane & 15) is token
+  // tau(i) = 8(a>>1) + 4(b&1) + 2(b>>1) + (a&1): any 8 consecutive lanes address 8 different 16-byte columns of the
+  // swizzled tile (no bank conflicts), and the K rows of a quarter warp differ in bit 2 (ditto)
+  const int vtok = 8 * ((lane >> 3) & 1) + 4 * (lane & 1) + 2 * ((lane >> 1) & 1) + ((lane >> 2) & 1);
   const int vrow = hl * 16 + vtok;
   const int vmat = lane >> 4;                       // which of the two 16-dim tiles of an x2 load this lane addresses
 
@@ -269,15 +277,15 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
         for (int h = 0; h < 2; ++h)
 #pragma unroll
           for (int rw = 0; rw < 2; ++rw) {
-            const int Rr = hl * 16 + t0 + 8 * rw;
+            const int Rr = hl * 16 + t0 + 2 * rw;
             kc[h][rw] = ptx::lds128(st + pl * C::PAGE_BYTES + Rr * 128 + (((4 * h + tq) ^ (Rr & 7)) * 16));
           }
         // scales of this thread's two tokens: K (times log2(e)/sqrt(D)) and V
         const uint32_t sc_off = pl * C::SC_BYTES + (hl * 16 + t0) * 4;
         const float sk0 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off)) * sh.scale_log2;
-        const float sk1 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off + 32)) * sh.scale_log2;
+        const float sk1 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off + 8)) * sh.scale_log2;
         float sv0 = __int_as_float(ptx::lds32(st + C::OFF_SV + sc_off));
-        float sv1 = __int_as_float(ptx::lds32(st + C::OFF_SV + sc_off + 32));
+        float sv1 = __int_as_float(ptx::lds32(st + C::OFF_SV + sc_off + 8));
         // ---- q re-rotated for this page: Qhat = R_{m - p0} q in fp32, rounded to f16 (a3/a4)
         {
           const uint32_t qcs = st + C::OFF_CS + pl * C::CS_ROW_BYTES + tq * 16;
@@ -304,23 +312,25 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
           for (int w = 0; w < C::NL; ++w) {
             const uint32_t x1 = (w & 1) ? ptx::e4m3x2_hi_to_f16x2(a1[w >> 1]) : ptx::e4m3x2_lo_to_f16x2(a1[w >> 1]);
             const uint32_t x2 = (w & 1) ? ptx::e4m3x2_hi_to_f16x2(a2[w >> 1]) : ptx::e4m3x2_lo_to_f16x2(a2[w >> 1]);
-            kreg[0][rw][w] = h2fma(h2neg(x2), cts[rw][w], h2mul(x1, ctc[rw][w]));
+            kreg[0][rw][w] = h2mulsub(x1, ctc[rw][w], x2, cts[rw][w]);
             kreg[1][rw][w] = h2fma(x2, ctc[rw][w], h2mul(x1, cts[rw][w]));
           }
         }
         // ---- S = Khat Qhat^T : rows = tokens (t0, t0 + 8), cols = heads (2tq, 2tq+1)
+        // (four accumulator chains of 4 MMAs: with two warps per scheduler the MMA latency chain is exposed)
         float s[4] = {0.f, 0.f, 0.f, 0.f}, s_b[4] = {0.f, 0.f, 0.f, 0.f};
+        float s_c[4] = {0.f, 0.f, 0.f, 0.f}, s_d[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
         for (int cc = 0; cc < C::NC / 2; ++cc) {
-          ptx::mma_f16_16816(s, kreg[0][0][2 * cc], kreg[0][1][2 * cc], kreg[0][0][2 * cc + 1],
+          ptx::mma_f16_16816((cc & 1) ? s_c : s, kreg[0][0][2 * cc], kreg[0][1][2 * cc], kreg[0][0][2 * cc + 1],
                              kreg[0][1][2 * cc + 1], qhat[0][2 * cc], qhat[0][2 * cc + 1]);
-          ptx::mma_f16_16816(s_b, kreg[1][0][2 * cc], kreg[1][1][2 * cc], kreg[1][0][2 * cc + 1],
+          ptx::mma_f16_16816((cc & 1) ? s_d : s_b, kreg[1][0][2 * cc], kreg[1][1][2 * cc], kreg[1][0][2 * cc + 1],
                              kreg[1][1][2 * cc + 1], qhat[1][2 * cc], qhat[1][2 * cc + 1]);
         }
-        s[0] = (s[0] + s_b[0]) * sk0; s[1] = (s[1] + s_b[1]) * sk0;
-        s[2] = (s[2] + s_b[2]) * sk1; s[3] = (s[3] + s_b[3]) * sk1;
+        s[0] = ((s[0] + s_b[0]) + (s_c[0] + s_d[0])) * sk0; s[1] = ((s[1] + s_b[1]) + (s_c[1] + s_d[1])) * sk0;
+        s[2] = ((s[2] + s_b[2]) + (s_c[2] + s_d[2])) * sk1; s[3] = ((s[3] + s_b[3]) + (s_c[3] + s_d[3])) * sk1;
         if (t0 >= nv) { s[0] = -INFINITY; s[1] = -INFINITY; sv0 = 0.f; }
-        if (t0 + 8 >= nv) { s[2] = -INFINITY; s[3] = -INFINITY; sv1 = 0.f; }
+        if (t0 + 2 >= nv) { s[2] = -INFINITY; s[3] = -INFINITY; sv1 = 0.f; }
         // ---- online softmax over the 16 tokens (a6)
         float mx0 = fmaxf(s[0], s[2]), mx1 = fmaxf(s[1], s[3]);
 #pragma unroll
@@ -355,11 +365,13 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
         const uint32_t pb0 = ptx::movmatrix_trans(ptx::pack_f16(p0 * w0, p1 * w0));
         const uint32_t pb1 = ptx::movmatrix_trans(ptx::pack_f16(p2 * w1, p3 * w1));
         // ---- O^T += V^T P'  (a7): 8-bit transposing ldmatrix, two 16-dim tiles per load; byte b of a register is
-        // token tq + 4b -- bytes past the tail are cleared (their codes may be NaN)
+        // token tau(4tq + b) = vt + 4(b&1) + 2(b>>1) -- bytes past the tail are cleared (their codes may be NaN)
         uint32_t vmask = 0xffffffffu;
-        if (nv < kPageSize)
-          vmask = (tq < nv ? 0xffu : 0u) | (tq + 4 < nv ? 0xff00u : 0u) | (tq + 8 < nv ? 0xff0000u : 0u) |
-                  (tq + 12 < nv ? 0xff000000u : 0u);
+        if (nv < kPageSize) {
+          const int vt = 8 * (tq >> 1) + (tq & 1);
+          vmask = (vt < nv ? 0xffu : 0u) | (vt + 4 < nv ? 0xff00u : 0u) | (vt + 2 < nv ? 0xff0000u : 0u) |
+                  (vt + 6 < nv ? 0xff000000u : 0u);
+        }
         const uint32_t vbase = st + C::OFF_V + pl * C::PAGE_BYTES + vrow * 128;
 #pragma unroll
         for (int i = 0; i < C::NC; i += 2) {
