@@ -79,8 +79,9 @@ bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, in
   return rc == CUDA_SUCCESS;
 }
 
-// FP8 code pool: rows of D bytes; box = [box_rows][D bytes] (D = 128: one 128-byte swizzle span per row)
-bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D, int box_rows) {
+// FP8 code pool: rows of D bytes; box = [box_rows][D bytes] (swizzled for the decode kernel -- D = 128: one 128-byte
+// swizzle span per row -- plain rows for the prefill kernel, which re-writes the tile as bf16)
+bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D, int box_rows, bool swizzle) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return false;
   cuuint64_t gdim[2] = {(cuuint64_t)D, (cuuint64_t)rows};
@@ -89,7 +90,7 @@ bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D,
   cuuint32_t estr[2] = {1u, 1u};
   CUresult rc = fn(reinterpret_cast<CUtensorMap*>(out_map), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
                    const_cast<void*>(pool), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                   D == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
+                   !swizzle ? CU_TENSOR_MAP_SWIZZLE_NONE : D == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_64B,
                    CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return rc == CUDA_SUCCESS;
 }
@@ -154,13 +155,13 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
   const bool fp8 = c.dtype == LAZY_KV_FP8_E4M3;
   if (fp8 && c.head_dim != 128) return LAZY_ERR_UNSUPPORTED;   // the caller routes head_dim 64 to the row-wise kernel
   if (h->tmap_k_ptr != k_cache) {
-    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta)
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta, true)
               : encode_pool_tmap(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta)))
       return LAZY_ERR_CUDA;
     h->tmap_k_ptr = k_cache;
   }
   if (h->tmap_v_ptr != v_cache) {
-    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta)
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta, true)
               : encode_pool_tmap(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta)))
       return LAZY_ERR_CUDA;
     h->tmap_v_ptr = v_cache;

@@ -229,7 +229,7 @@ int lazy_attn_prefill(lazy_handle* h, const void* q, const void* k_cache, const 
   if (!cu_q_lens || (reinterpret_cast<uintptr_t>(cu_q_lens) & 3u) || max_q_len == 0) return LAZY_ERR_INVALID;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   int n;
-  if ((h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS) || h->cfg.dtype == LAZY_KV_FP8_E4M3)
+  if (h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS)
     n = lazy::launch_rowwise(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, cu_q_lens,
                              num_reqs, total_q, max_q_len, out, s);
   else

@@ -113,6 +113,8 @@ int launch_mixed_fused(lazy_handle* h, const lazy_mixed_args* m, const void* k_c
   pa.cs = h->ws.cs;
   pa.stored_pos = h->page_stored_pos;
   pa.alibi = h->ws.alibi;
+  pa.k_scale = nullptr;
+  pa.v_scale = nullptr;
   pa.num_reqs = m->num_reqs_prefill;
   pa.q_interleaved = c.rope_style == LAZY_ROPE_INTERLEAVED;
   pa.mblocks = (m->max_q_len + 4 * tpt - 1) / (4 * tpt);

@@ -16,6 +16,8 @@ struct PrefillArgs {
   const float2* cs;
   const int* stored_pos;   // LAZY_K_STORED_POS: [num_pages] position each physical page was stored at
   const float* alibi;      // kKmAlibi: [Hq] slopes * log2(e)
+  const float* k_scale;    // LAZY_KV_FP8_E4M3: [num_pages][Hkv][16] per-row scales of the code pools
+  const float* v_scale;
   int num_reqs;
   int q_interleaved;    // LAZY_ROPE_INTERLEAVED: q arrives with pairs (2j, 2j+1); de-interleaved while it is rotated
   int mblocks;          // CTAs (pair kernel: CTA pairs) per (request, kv head)

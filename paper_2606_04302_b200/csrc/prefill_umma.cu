@@ -19,6 +19,8 @@
 // TMEM (512 columns): S0 | S1 | O0 | O1, P_t aliases the first 64 columns of S_t.
 #include <climits>
 
+#include <cuda_fp16.h>
+
 #include "prefill_common.cuh"
 
 namespace lazy {
@@ -36,11 +38,12 @@ struct PrefillCfg {
   static constexpr int OFF_V = 4 * TILE_BYTES;      // 2 stages
   static constexpr int OFF_CS = 6 * TILE_BYTES;     // 2 stages of 8 table rows (e^{i p0 theta_j} per page)
   static constexpr int OFF_BAR = OFF_CS + 2 * CS_STAGE_BYTES;
-  static constexpr int NUM_BARS = 26;
+  static constexpr int NUM_BARS = 28;
   static constexpr int OFF_TMEM = OFF_BAR + NUM_BARS * 8;
   static constexpr int OFF_SIGN = OFF_TMEM + 16;    // ring of 4 tiles x 8 pages: sign of the page's relative offset
                                                     // (LAZY_K_STORED_POS) or its logical start (ALiBi)
-  static constexpr int SMEM_BYTES = OFF_SIGN + 4 * kPagesPerTile * 4 + 1024;   // + alignment slack
+  static constexpr int OFF_SC = OFF_SIGN + 4 * kPagesPerTile * 4;   // FP8 pages: [stage][K, V][page][16] row scales
+  static constexpr int SMEM_BYTES = OFF_SC + 2 * 2 * kPagesPerTile * 64 + 1024;   // + alignment slack
 };
 
 // barrier indices
@@ -59,9 +62,28 @@ enum : int {
   B_OFULL = 20,   // +t   MMA commit -> softmax WG t (epilogue)
   B_PHALF = 22,   // +t   softmax WG t (4 warps) -> MMA: first half of P (keys 0..63) is in TMEM
   B_PVH = 24,     // +t   MMA commit -> softmax WG t: PV over the first half of P has completed (slow path only)
+  B_VREADY = 26,  // +s   FP8 pages: rotate WG (4 warps) -> MMA: the V tile has been dequantised to bf16
 };
 
-template <int D, int KM>
+// FP8 pages: 8 E4M3 codes (two words) -> 8 fp32 values, exact
+__device__ __forceinline__ void e4m3x8_to_f32(uint2 v, float2 (&x)[4]) {
+  const uint32_t h[4] = {ptx::e4m3x2_lo_to_f16x2(v.x), ptx::e4m3x2_hi_to_f16x2(v.x), ptx::e4m3x2_lo_to_f16x2(v.y),
+                         ptx::e4m3x2_hi_to_f16x2(v.y)};
+#pragma unroll
+  for (int w = 0; w < 4; ++w) x[w] = __half22float2(*reinterpret_cast<const __half2*>(&h[w]));
+}
+__device__ __forceinline__ uint2 lds64(uint32_t addr) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+  return v;
+}
+
+// F8: LAZY_KV_FP8_E4M3 pages.  A page's E4M3 codes land (TMA, un-swizzled rows of D bytes) at the
+// start of the page's own 2 KB region of the bf16 tile; the rotate warpgroup reads ALL codes of the page into
+// registers, and then writes the bf16 tile over them: K dequantised (code x the token's scale) and rotated in one
+// pass, V dequantised -- and the rows past the end of the sequence cleared, which is the tail fixer's job on bf16
+// pages.  The tensor cores see exactly the bf16 tiles they see on bf16 pages.
+template <int D, int KM, bool F8>
 __global__ void __launch_bounds__(kPrefillThreads, 1)
 prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
                     const __grid_constant__ CUtensorMap tmap_v, const PrefillArgs a) {
@@ -108,6 +130,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 
   if (tid == 0) {
     for (int x = 0; x < 2; ++x) {
+      ptx::mbar_init(bar(B_VREADY + x), 4);
       ptx::mbar_init(bar(B_QFULL + x), 1);  ptx::mbar_init(bar(B_QREADY + x), 4);
       ptx::mbar_init(bar(B_KFULL + x), 1);  ptx::mbar_init(bar(B_KREADY + x), 4);
       ptx::mbar_init(bar(B_KEMPTY + x), 1); ptx::mbar_init(bar(B_VFULL + x), 1);
@@ -174,21 +197,33 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         if (KM == LAZY_K_STORED_POS && lane < kPagesPerTile) s_sign[(j & 3) * kPagesPerTile + pg] = p0_sign;
         if (KM == kKmAlibi && lane < kPagesPerTile) s_sign[(j & 3) * kPagesPerTile + pg] = p0;
         __syncwarp();
+        const uint32_t sSC = smem_base + C::OFF_SC + s * (2 * kPagesPerTile * 64) + pg * 64;
         if (lane == 0)
-          ptx::mbar_arrive_expect_tx(bar(B_KFULL + s), npv * (C::NH * kPageSize * 128 +
+          ptx::mbar_arrive_expect_tx(bar(B_KFULL + s), npv * ((F8 ? kPageSize * D + 64 : C::NH * kPageSize * 128) +
                                                               (kNoRotate ? 0 : C::CS_ROW_BYTES)));
         __syncwarp();
         if (kvsel == 0 && lane_on && pg < npv) {
-          ptx::tma_load_2d(sK + dst, &tmap_k, bar(B_KFULL + s), half * 64, row0);
+          if (!F8) ptx::tma_load_2d(sK + dst, &tmap_k, bar(B_KFULL + s), half * 64, row0);
+          if (F8 && half == 0) {
+            ptx::tma_load_2d(sK + dst, &tmap_k, bar(B_KFULL + s), 0, row0);
+            ptx::bulk_load_1d(sSC, a.k_scale + row0, 64, bar(B_KFULL + s));
+          }
           if (half == 0 && !kNoRotate)
             ptx::bulk_load_1d(sCS + s * C::CS_STAGE_BYTES + pg * C::CS_ROW_BYTES, a.cs + (size_t)p0 * (D / 2),
                               C::CS_ROW_BYTES, bar(B_KFULL + s));
         }
         ptx::mbar_wait_sleep(bar(B_VEMPTY + s), ph ^ 1);
-        if (lane == 0) ptx::mbar_arrive_expect_tx(bar(B_VFULL + s), npv * C::NH * kPageSize * 128);
+        if (lane == 0)
+          ptx::mbar_arrive_expect_tx(bar(B_VFULL + s), npv * (F8 ? kPageSize * D + 64 : C::NH * kPageSize * 128));
         __syncwarp();
-        if (kvsel == 1 && lane_on && pg < npv) ptx::tma_load_2d(sV + dst, &tmap_v, bar(B_VFULL + s), half * 64, row0);
-        if (j == n_kv - 1) {
+        if (kvsel == 1 && lane_on && pg < npv) {
+          if (!F8) ptx::tma_load_2d(sV + dst, &tmap_v, bar(B_VFULL + s), half * 64, row0);
+          if (F8 && half == 0) {
+            ptx::tma_load_2d(sV + dst, &tmap_v, bar(B_VFULL + s), 0, row0);
+            ptx::bulk_load_1d(sSC + kPagesPerTile * 64, a.v_scale + row0, 64, bar(B_VFULL + s));
+          }
+        }
+        if (!F8 && j == n_kv - 1) {
           __syncwarp();
           if (lane == 0) ptx::mbar_arrive(bar(B_VLAST));
         }
@@ -235,8 +270,8 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       commit(B_KEMPTY + 0);
       for (int j = 0; j < nkv; ++j) {
         const int s = j & 1;
-        ptx::mbar_wait(bar(B_VFULL + s), (j >> 1) & 1);
-        if (j == nkv - 1) ptx::mbar_wait(bar(B_VFIXED), 0);
+        ptx::mbar_wait(bar((F8 ? B_VREADY : B_VFULL) + s), (j >> 1) & 1);
+        if (!F8 && j == nkv - 1) ptx::mbar_wait(bar(B_VFIXED), 0);
 #pragma unroll
         for (int t = 0; t < 2; ++t) {
           // PV starts on the first 64 keys while the softmax warpgroup is still exponentiating the other 64
@@ -262,7 +297,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
         }
       }
       __syncwarp();
-    } else if (warp == 14) {
+    } else if (warp == 14 && !F8) {
       // ================================ V tail fixer ========================================================
       // The fixer is not part of the V ring's full/empty hand-shake, so it must not walk the ring's phases (a lagging
       // observer would alias parities).  It sleeps on a one-shot barrier until the producer has ISSUED the last tile's
@@ -312,6 +347,104 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
       const uint32_t kb = sK + s * C::TILE_BYTES;
       const uint32_t cb = sCS + s * C::CS_STAGE_BYTES;
       ptx::mbar_wait(bar(B_KFULL + s), (j >> 1) & 1);
+      if (F8) {
+        // ---- FP8 pages: dequantise + rotate K, then dequantise V, each over its own landing area ----------------
+        const uint32_t sc = smem_base + C::OFF_SC + s * (2 * kPagesPerTile * 64) + i * 64 + t0 * 4;
+        const uint32_t land = i * (kPageSize * 128) + t0 * D + 8 * c;   // codes of (page i, token t0, dims 8c..)
+        uint2 ra[TOK], rb[TOK];
+        float scl[TOK];
+        float2 zc[4], zs[4];
+        if (i < npv) {
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const uint4 v = ptx::lds128(cb + i * C::CS_ROW_BYTES + 16 * cs_f4_index<D>(c, x));
+            const float2 wc = make_float2(f32(v.x), f32(v.y)), ws = make_float2(f32(v.z), f32(v.w));
+            zc[x] = __ffma2_rn(neg2(ws), u0s[x], __fmul2_rn(wc, u0c[x]));     // z = w * u0: the group's first token
+            zs[x] = __ffma2_rn(wc, u0s[x], __fmul2_rn(ws, u0c[x]));
+          }
+#pragma unroll
+          for (int tt = 0; tt < TOK; ++tt) {
+            ra[tt] = lds64(kb + land + tt * D);
+            rb[tt] = lds64(kb + land + tt * D + D / 2);
+            scl[tt] = __int_as_float(ptx::lds32(sc + tt * 4));
+          }
+        }
+        __syncwarp();                               // the 16 threads of a page have read its codes: overwrite them
+        if (i < npv) {
+#pragma unroll
+          for (int tt = 0; tt < TOK; ++tt) {
+            float2 x1[4], x2[4];
+            e4m3x8_to_f32(ra[tt], x1);
+            e4m3x8_to_f32(rb[tt], x2);
+            const float2 sk2 = make_float2(scl[tt], scl[tt]);
+            uint4 va, vb;
+            uint32_t* aw = reinterpret_cast<uint32_t*>(&va);
+            uint32_t* bw = reinterpret_cast<uint32_t*>(&vb);
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+              const float2 cc = __fmul2_rn(zc[w], sk2), ss = __fmul2_rn(zs[w], sk2);   // the token's scale rides on z
+              const float2 y1 = __ffma2_rn(neg2(x2[w]), ss, __fmul2_rn(x1[w], cc));
+              const float2 y2 = __ffma2_rn(x2[w], cc, __fmul2_rn(x1[w], ss));
+              aw[w] = ptx::pack_bf16(y1.x, y1.y);
+              bw[w] = ptx::pack_bf16(y2.x, y2.y);
+            }
+            const int row = i * kPageSize + t0 + tt;
+            ptx::sts128(kb + chunk_off(row, c), va);
+            ptx::sts128(kb + chunk_off(row, c + C::CPR), vb);
+            if (tt + 1 < TOK) {                     // next token: z <- z * e^{i theta_j}
+#pragma unroll
+              for (int x = 0; x < 4; ++x) {
+                const float2 wc = zc[x], ws = zs[x];
+                zc[x] = __ffma2_rn(neg2(ws), u1s[x], __fmul2_rn(wc, u1c[x]));
+                zs[x] = __ffma2_rn(wc, u1s[x], __fmul2_rn(ws, u1c[x]));
+              }
+            }
+          }
+        }
+        ptx::fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(B_KREADY + s));
+        // ---- V: code x the token's scale -> bf16; rows at or past seq_len become zeros (never multiplied)
+        const uint32_t vb_ = sV + s * C::TILE_BYTES;
+        ptx::mbar_wait(bar(B_VFULL + s), (j >> 1) & 1);
+        const int rows_valid = L - j * kTileRows;   // >= 128 on interior tiles
+        if (i < npv) {
+#pragma unroll
+          for (int tt = 0; tt < TOK; ++tt) {
+            ra[tt] = lds64(vb_ + land + tt * D);
+            rb[tt] = lds64(vb_ + land + tt * D + D / 2);
+            scl[tt] = __int_as_float(ptx::lds32(sc + kPagesPerTile * 64 + tt * 4));
+          }
+        }
+        __syncwarp();
+#pragma unroll
+        for (int tt = 0; tt < TOK; ++tt) {
+          const int row = i * kPageSize + t0 + tt;
+          uint4 va = make_uint4(0, 0, 0, 0), vb = make_uint4(0, 0, 0, 0);
+          if (i < npv && row < rows_valid) {
+            float2 x1[4], x2[4];
+            e4m3x8_to_f32(ra[tt], x1);
+            e4m3x8_to_f32(rb[tt], x2);
+            const float2 sv2 = make_float2(scl[tt], scl[tt]);
+            uint32_t* aw = reinterpret_cast<uint32_t*>(&va);
+            uint32_t* bw = reinterpret_cast<uint32_t*>(&vb);
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+              const float2 y1 = __fmul2_rn(x1[w], sv2), y2 = __fmul2_rn(x2[w], sv2);
+              aw[w] = ptx::pack_bf16(y1.x, y1.y);
+              bw[w] = ptx::pack_bf16(y2.x, y2.y);
+            }
+          }
+          if (i < npv || j == n_kv - 1) {           // pages that do not exist are cleared on the last tile only
+            ptx::sts128(vb_ + chunk_off(row, c), va);
+            ptx::sts128(vb_ + chunk_off(row, c + C::CPR), vb);
+          }
+        }
+        ptx::fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(B_VREADY + s));
+        continue;
+      }
       if (!kNoRotate && i < npv) {
         float2 zc[4], zs[4];                        // e^{i (p0+t) theta_j}, or e^{i Delta theta_j} of the page
 #pragma unroll
@@ -642,10 +775,10 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
 
 }  // namespace
 
-template <int D, int KM>
+template <int D, int KM, bool F8 = false>
 static int launch_prefill_t(const lazy_handle* h, const PrefillArgs& args, int grid, cudaStream_t stream) {
   using C = PrefillCfg<D>;
-  auto kern = prefill_umma_kernel<D, KM>;
+  auto kern = prefill_umma_kernel<D, KM, F8>;
   // per launch: the attribute is per device, and a process may hold handles on several devices
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
     return LAZY_ERR_CUDA;
@@ -664,12 +797,17 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   const int group = c.num_q_heads / c.num_kv_heads;
   const int tpt = kTileRows / group;                 // query tokens per 128-row tile
   const long long rows = (long long)c.num_pages * c.num_kv_heads * kPageSize;
+  const bool fp8 = c.dtype == LAZY_KV_FP8_E4M3;
   if (h->tmap_pk_ptr != k_cache) {
-    if (!encode_pool_tmap(h->tmap_pk, k_cache, rows, c.head_dim, kPageSize)) return LAZY_ERR_CUDA;
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_pk, k_cache, rows, c.head_dim, kPageSize, false)
+              : encode_pool_tmap(h->tmap_pk, k_cache, rows, c.head_dim, kPageSize)))
+      return LAZY_ERR_CUDA;
     h->tmap_pk_ptr = k_cache;
   }
   if (h->tmap_pv_ptr != v_cache) {
-    if (!encode_pool_tmap(h->tmap_pv, v_cache, rows, c.head_dim, kPageSize)) return LAZY_ERR_CUDA;
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_pv, v_cache, rows, c.head_dim, kPageSize, false)
+              : encode_pool_tmap(h->tmap_pv, v_cache, rows, c.head_dim, kPageSize)))
+      return LAZY_ERR_CUDA;
     h->tmap_pv_ptr = v_cache;
   }
   if (h->tmap_pq_ptr != q || h->tmap_pq_rows != total_q) {
@@ -691,6 +829,15 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   a.mblocks = (max_q_len + 2 * tpt - 1) / (2 * tpt);
   a.tokens_per_tile = tpt;
   a.sh = h->shape;
+  a.k_scale = h->k_scale;
+  a.v_scale = h->v_scale;
+  if (fp8) {
+    // FP8 pages run on the one-CTA kernel at either head_dim (its rotate warpgroup dequantises both tiles)
+    const long long grid = (long long)a.mblocks * c.num_kv_heads * num_reqs;
+    if (grid <= 0 || grid > INT_MAX) return LAZY_ERR_INVALID;
+    return c.head_dim == 128 ? launch_prefill_t<128, LAZY_K_UNROTATED, true>(h, a, (int)grid, stream)
+                             : launch_prefill_t<64, LAZY_K_UNROTATED, true>(h, a, (int)grid, stream);
+  }
   if (c.head_dim == 128 && !(c.flags & LAZY_FLAG_PREFILL_ONE_CTA)) {
     // CTA pairs (prefill_umma2.cu): a pair covers 4 * tpt query tokens
     a.mblocks = (max_q_len + 4 * tpt - 1) / (4 * tpt);
