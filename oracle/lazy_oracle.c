@@ -58,17 +58,26 @@ double lazy_oracle_e4m3_to_double(uint8_t c) {
 }
 
 /* Nearest E4M3 code of x: round to nearest, ties to the code with an even mantissa bit, magnitudes beyond 448
- * saturate to +-448 (never NaN, never infinity); NaN gives the NaN code.  Written as a search over the 127
- * non-negative finite values (codes 0x00..0x7e are increasing in value), not as bit manipulation. */
+ * saturate to +-448 (never NaN, never infinity); NaN gives the NaN code.  Written as a search (bisection) over the
+ * 127 non-negative finite values (codes 0x00..0x7e are increasing in value), not as bit manipulation. */
 uint8_t lazy_oracle_e4m3_from_float(float x) {
+    static double val[0x7f];                     /* values of codes 0x00..0x7e (every thread writes the same numbers) */
+    static volatile int ready = 0;
+    if (!ready) {
+        for (int c = 0; c < 0x7f; ++c) val[c] = lazy_oracle_e4m3_to_double((uint8_t)c);
+        ready = 1;
+    }
     if (x != x) return 0x7f;
     uint8_t sign = (x < 0.0f || (x == 0.0f && 1.0f / x < 0.0f)) ? 0x80 : 0x00;
     double a = fabs((double)x);
     if (a >= 448.0) return sign | 0x7e;
-    int c = 0;                                   /* largest code whose value is <= a */
-    while (c < 0x7e && lazy_oracle_e4m3_to_double((uint8_t)(c + 1)) <= a) ++c;
-    double lo = lazy_oracle_e4m3_to_double((uint8_t)c), hi = lazy_oracle_e4m3_to_double((uint8_t)(c + 1));
-    double dl = a - lo, dh = hi - a;             /* exact: fp32 and E4M3 values are dyadic, differences fit in fp64 */
+    int lo_c = 0, hi_c = 0x7e;                   /* bisection: largest code c with val[c] <= a (val[0] = 0 <= a < val[0x7e]) */
+    while (hi_c - lo_c > 1) {
+        int mid = (lo_c + hi_c) / 2;
+        if (val[mid] <= a) lo_c = mid; else hi_c = mid;
+    }
+    int c = lo_c;
+    double dl = a - val[c], dh = val[c + 1] - a; /* exact: fp32 and E4M3 values are dyadic, differences fit in fp64 */
     if (dh < dl || (dh == dl && (c & 1))) ++c;
     return sign | (uint8_t)c;
 }

@@ -98,3 +98,57 @@ def test_fp8_needs_scales_and_rejects_unsupported_modes():
         B.lazy_set_kv_scales(hb, torch.zeros(64, device=dev), torch.zeros(64, device=dev))
     assert e.value.status == B.LAZY_ERR_UNSUPPORTED
     hb.close()
+
+
+@pytest.mark.parametrize("cfg,rows", [(2, 0), (3, 96), (4, 0), (5, 64)])
+def test_fp8_configs_full_size_sampled(cfg, rows):
+    """BASELINE.json sizes on FP8 pages, the launch configurations bench.py's fp8 legs time; the oracle on sampled
+    query rows (decode configs are compared in full).  Same margins as the bf16 full-size test: the kernels' own
+    error (f16 / bf16 rounding of the rotated operands and of P) is what is measured, not the quantisation."""
+    stats = _run(W.CONFIGS[cfg](), sample_rows=rows, seed=cfg)
+    max_b, mean_b = {2: (2e-3, 2e-4), 3: (2e-3, 2e-4), 4: (1e-3, 1e-4), 5: (1.5e-2, 5e-4)}[cfg]
+    assert all(s["max_abs"] < max_b and s["mean_abs"] < mean_b for s in stats), stats
+
+
+def test_fp8_v_scale_outlier_tokens():
+    """V rows whose magnitudes differ by 2^+-20 inside one request (and inside one page): the decode kernel's running
+    reference V scale must re-reference O in both directions; the prefill kernel folds the scale into the bf16 tile."""
+    b = W.config2(scale=0.1)
+    g = torch.Generator().manual_seed(5)
+    v = b.v_pool.float()
+    fin = torch.isfinite(v).all(dim=-1, keepdim=True)
+    e = torch.randint(-20, 21, v.shape[:-1] + (1,), generator=g).float()
+    sparse = torch.rand(v.shape[:-1] + (1,), generator=g) < 0.05
+    b.v_pool = torch.where(fin & sparse, v * torch.exp2(e), v).to(torch.bfloat16)
+    _run(b, scale_abs_by_output=True, gates=dict(rel_rms=2e-2))
+
+
+def test_fp8_mixed_call_matches_oracle():
+    """lazy_attn_mixed on FP8 pages (two kernels on forked streams: the one-launch step is bf16-only)."""
+    from oracle import oracle as O
+    from paper_2606_04302_b200.runner import DeviceBatch
+    from gpu_util import compare
+    batch = W.config5(scale=0.2)
+    pre, dec = batch.steps[0], batch.steps[1]
+    dev = DeviceBatch(batch, dtype=B.LAZY_KV_FP8_E4M3)
+    d = dev.device
+    pools = O.quantize_pool_fp8(batch.k_pool, batch.v_pool)
+    try:
+        dev.write(pre); dev.write(dec)
+        ref_p = O.run_step_fp8(batch, pre, pools)
+        ref_d = O.run_step_fp8(batch, dec, pools)
+        bt_p, pp_p = dev.tables_for(pre)
+        bt_d, pp_d = dev.tables_for(dec)
+        out_p = torch.zeros_like(pre.q, device=d)
+        out_d = torch.zeros_like(dec.q, device=d)
+        max_q = int((pre.cu_q_lens[1:] - pre.cu_q_lens[:-1]).max())
+        B.lazy_attn_mixed(dev.handle, dev.k_pool, dev.v_pool, q_prefill=pre.q.to(d), block_table_prefill=bt_p,
+                          page_logical_pos_prefill=pp_p, seq_lens_prefill=pre.seq_lens.to(d),
+                          cu_q_lens=pre.cu_q_lens.to(d), max_q_len=max_q, out_prefill=out_p, q_decode=dec.q.to(d),
+                          block_table_decode=bt_d, page_logical_pos_decode=pp_d, seq_lens_decode=dec.seq_lens.to(d),
+                          out_decode=out_d)
+        torch.cuda.synchronize()
+        compare(out_p, ref_p, "fp8 mixed prefill")
+        compare(out_d, ref_d, "fp8 mixed decode")
+    finally:
+        dev.close()
