@@ -118,6 +118,9 @@ typedef struct lazy_config {
 #define LAZY_FLAG_PREFILL_ONE_CTA 2  /* head_dim 128: run prefill on single CTAs (prefill_umma.cu) instead of CTA
                                       pairs (prefill_umma2.cu); the A/B arm of DESIGN.md 6.2 */
 
+#define LAZY_FLAG_FP8_DECODE_8_WARPS 4  /* LAZY_KV_FP8_E4M3 decode with the bf16 kernel's 8 consumer warps instead of 12
+                                        (the A/B arm of DESIGN.md 6.7) */
+
 #define LAZY_OK               0
 #define LAZY_ERR_INVALID     -1  /* null / misaligned pointer, negative count, num_reqs > max_reqs ...     */
 #define LAZY_ERR_UNSUPPORTED -2  /* head_dim, page_size, head grouping, dtype or rope_style not supported  */

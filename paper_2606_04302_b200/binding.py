@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "liblazyattn.so")
 LAZY_OK, LAZY_ERR_INVALID, LAZY_ERR_UNSUPPORTED, LAZY_ERR_WORKSPACE, LAZY_ERR_CUDA = 0, -1, -2, -3, -4
 LAZY_FLAG_ROWWISE_KERNELS = 1
 LAZY_FLAG_PREFILL_ONE_CTA = 2
+LAZY_FLAG_FP8_DECODE_8_WARPS = 4
 LAZY_K_UNROTATED, LAZY_K_STORED_POS, LAZY_K_ABSOLUTE = 0, 1, 2
 LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
 LAZY_KV_BF16, LAZY_KV_FP8_E4M3 = 0, 1

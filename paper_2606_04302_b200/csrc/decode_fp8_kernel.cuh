@@ -24,10 +24,15 @@
 namespace lazy {
 namespace {
 
-template <int HKV_CTA>
+// NCW consumer warps: 8 (the bf16 kernel's cut: 224 registers per consumer thread) or 12 (160 registers, which this
+// kernel fits: three dependent-chain warps per scheduler instead of two).  A CTA then holds NCW * 32 + 128 threads.
+template <int HKV_CTA, int NCW>
 struct DecodeFp8Cfg {
   static constexpr int D = 128;
-  static constexpr int PPS = kConsumerWarps / HKV_CTA;  // pages per pipeline stage
+  static constexpr int THREADS = NCW * 32 + 128;
+  static constexpr int REGS_CONSUMER = NCW == 8 ? kRegsConsumer : 160;   // 384 * 160 + 128 * 32 = 65536
+  static constexpr int REGS_PRODUCER = NCW == 8 ? kRegsProducer : 32;
+  static constexpr int PPS = NCW / HKV_CTA;             // pages per pipeline stage
   static constexpr int BOX_ROWS = 16 * HKV_CTA;
   static constexpr int PAGE_BYTES = BOX_ROWS * 128;     // K (or V) codes of one page, HKV_CTA heads: rows of 128 B
   static constexpr int CS_ROW_BYTES = D / 2 * 8;
@@ -38,13 +43,16 @@ struct DecodeFp8Cfg {
   static constexpr int OFF_SV = OFF_SK + PPS * SC_BYTES;
   static constexpr int OFF_META = OFF_SV + PPS * SC_BYTES;
   static constexpr int STAGE_BYTES = (OFF_META + PPS * 4 + 1023) / 1024 * 1024;
-  static constexpr int NSTAGES = 5;
+  // 37 KB stages x 5 (8 warps) / 52-56 KB stages x 3 (12 warps); a 4th stage was measured: no gain (84.1 -> 85.4 us)
+  static constexpr int NSTAGES = NCW == 8 ? 5 : 3;
+  static constexpr int MAX_REQS = kMaxReqsSmem;         // requests per launch (smem prefix sums)
   static constexpr int NL = 8;                          // words of 2 rotation pairs per thread per half
   static constexpr int NC = D / 16;
   static constexpr int OFF_CUM = NSTAGES * STAGE_BYTES;
-  static constexpr int OFF_LEN = OFF_CUM + (kMaxReqsSmem + 4) * 4;
-  static constexpr int OFF_BAR = OFF_LEN + kMaxReqsSmem * 4;
+  static constexpr int OFF_LEN = OFF_CUM + (MAX_REQS + 4) * 4;
+  static constexpr int OFF_BAR = OFF_LEN + MAX_REQS * 4;
   static constexpr int SMEM_BYTES = OFF_BAR + 2 * NSTAGES * 8 + 16 + 1024;
+  static_assert(SMEM_BYTES <= 232448, "decode_fp8: shared memory");
 };
 
 struct DecodeFp8Args {
@@ -69,11 +77,11 @@ __device__ __forceinline__ uint32_t h2mulsub(uint32_t a, uint32_t b, uint32_t c,
   return *reinterpret_cast<const uint32_t*>(&r);
 }
 
-template <int HKV_CTA>
+template <int HKV_CTA, int NCW>
 __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const CUtensorMap& tmap_v,
                                                const DecodeFp8Args& fa, const int bid, const int G_in, const int hg,
                                                const int HG, unsigned char* smem_raw) {
-  using C = DecodeFp8Cfg<HKV_CTA>;
+  using C = DecodeFp8Cfg<HKV_CTA, NCW>;
   constexpr int D = C::D;
   const DecodeArgs& a = fa.d;
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -95,12 +103,12 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
   if (tid == 0) {
     for (int s = 0; s < C::NSTAGES; ++s) {
       ptx::mbar_init(bar_full + 8 * s, 1);
-      ptx::mbar_init(bar_empty + 8 * s, kConsumerWarps);
+      ptx::mbar_init(bar_empty + 8 * s, NCW);
     }
     ptx::mbar_init(bar_empty + C::NSTAGES * 8 + 8, 1);
     ptx::fence_mbar_init();
   }
-  if (warp == kConsumerWarps && lane == 0) {
+  if (warp == NCW && lane == 0) {
     ptx::prefetch_tmap(&tmap_k);
     ptx::prefetch_tmap(&tmap_v);
   }
@@ -138,9 +146,9 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
     r0 = lo;
   }
 
-  if (warp >= kConsumerWarps) {
-    ptx::setmaxnreg_dec<kRegsProducer>();
-    if (warp > kConsumerWarps) return;
+  if (warp >= NCW) {
+    ptx::setmaxnreg_dec<C::REGS_PRODUCER>();
+    if (warp > NCW) return;
     // ================================= producer warp =====================================================
     const int pl = lane;
     int r = r0, u = u_begin;
@@ -196,7 +204,7 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
   }
 
   // =================================== consumer warps ====================================================
-  ptx::setmaxnreg_inc<kRegsConsumer>();
+  ptx::setmaxnreg_inc<C::REGS_CONSUMER>();
   const int g = lane >> 2, tq = lane & 3;
   const int pl = warp / HKV_CTA;
   const int hl = warp % HKV_CTA;
@@ -411,7 +419,7 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
         if (g == 0) a.part_ml[(size_t)slot * sh.Hq + hq] = make_float2(m_run[e], l_run[e]);
       }
     }
-    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    ptx::named_bar_sync(1, NCW * 32);
     const long long c0 = s_cum[r], c1 = s_cum[r + 1];
     const int b_first = (int)(((c0 + 1) * G + U - 1) / U) - 1;
     const int b_last = (int)((c1 * G + U - 1) / U) - 1;
@@ -423,14 +431,14 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
       if (last) a.req_counter[r * HG + hg] = 0;
       *s_flag = last;
     }
-    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    ptx::named_bar_sync(1, NCW * 32);
     if (*s_flag) {
       __threadfence();
       // the ring is idle iff this segment ends the CTA's range (every issued stage has been consumed)
-      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane,
+      combine_request<D, NCW>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane,
                          s_cum[r] + seg_hi == u_end, smem_base, C::NSTAGES * C::STAGE_BYTES, bar_comb, comb_phase);
     }
-    ptx::named_bar_sync(1, kConsumerWarps * 32);
+    ptx::named_bar_sync(1, NCW * 32);
     u = s_cum[r] + seg_hi;
     ++r;
   }

@@ -70,7 +70,7 @@ struct DecodeArgs {
 // warps loaded four slots at a time from L2 / HBM, ~0.9 us per dependent batch: 16 us for the 20 slots x 28 heads of a
 // cfg-5 request, which held that decode under 70 % of the HBM roofline.)  Otherwise (the ring still holds pages of the
 // CTA's next request) the register path below runs.
-template <int D>
+template <int D, int NCW = kConsumerWarps>
 __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r, const int hg, const int heads_cta,
                                                 const int n_slots, const int slot0, const int warp, const int lane,
                                                 const bool ring_free, const uint32_t ring_u32, const int ring_bytes,
@@ -79,7 +79,7 @@ __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r
   const int slot_bytes = heads_cta * D * 4;
   if (ring_free && slot_bytes <= ring_bytes) {
     const int cap = min(32, ring_bytes / slot_bytes);
-    const int hpw = (heads_cta + kConsumerWarps - 1) / kConsumerWarps;      // heads per warp (<= 8)
+    const int hpw = (heads_cta + NCW - 1) / NCW;      // heads per warp (<= 8)
     float mstar[8], lsum[8], acc[8][D / 32];
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
@@ -103,7 +103,7 @@ __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r
       float2 ml[8];
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
-        const int hh = warp + k * kConsumerWarps;
+        const int hh = warp + k * NCW;
         ml[k] = make_float2(-INFINITY, 0.f);
         if (k < hpw && hh < heads_cta && lane < n)
           ml[k] = __ldcg(&a.part_ml[(size_t)(slot0 + base + lane) * sh.Hq + hg * heads_cta + hh]);
@@ -112,7 +112,7 @@ __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r
       cphase ^= 1;
 #pragma unroll
       for (int k = 0; k < 8; ++k) {
-        const int hh = warp + k * kConsumerWarps;
+        const int hh = warp + k * NCW;
         if (k < hpw && hh < heads_cta) {
           float mx = ml[k].x;
 #pragma unroll
@@ -143,11 +143,11 @@ __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r
           }
         }
       }
-      if (base + cap < n_slots) ptx::named_bar_sync(1, kConsumerWarps * 32);   // the next round overwrites the ring
+      if (base + cap < n_slots) ptx::named_bar_sync(1, NCW * 32);   // the next round overwrites the ring
     }
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
-      const int hh = warp + k * kConsumerWarps;
+      const int hh = warp + k * NCW;
       if (k < hpw && hh < heads_cta) {
         const float inv = lsum[k] > 0.f ? 1.f / lsum[k] : 0.f;
         __nv_bfloat16* op = a.out + ((size_t)r * sh.Hq + hg * heads_cta + hh) * D + lane * (D / 32);
@@ -158,7 +158,7 @@ __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r
     }
     return;
   }
-  for (int hh = warp; hh < heads_cta; hh += kConsumerWarps) {
+  for (int hh = warp; hh < heads_cta; hh += NCW) {
     const int hq = hg * heads_cta + hh;
     // single pass with a running max; the loads of four partials are issued together so that their L2
     // latencies overlap (the partials were written by other SMs)

@@ -38,12 +38,12 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
 }
 
 // LAZY_KV_FP8_E4M3 pages (decode_fp8_kernel.cuh), head_dim 128
-template <int HKV_CTA>
-__global__ void __launch_bounds__(kDecodeThreads, 1)
+template <int HKV_CTA, int NCW>
+__global__ void __launch_bounds__(NCW * 32 + 128, 1)
 decode_fp8_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
                   const DecodeFp8Args a) {
   extern __shared__ unsigned char smem_raw[];
-  decode_fp8_cta<HKV_CTA>(tmap_k, tmap_v, a, (int)blockIdx.x, (int)gridDim.x, (int)blockIdx.y, (int)gridDim.y, smem_raw);
+  decode_fp8_cta<HKV_CTA, NCW>(tmap_k, tmap_v, a, (int)blockIdx.x, (int)gridDim.x, (int)blockIdx.y, (int)gridDim.y, smem_raw);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -133,15 +133,15 @@ static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, i
   }
 }
 
-template <int HKV_CTA>
+template <int HKV_CTA, int NCW>
 static int launch_decode_fp8_t(lazy_handle* h, const DecodeFp8Args& args, int grid_x, int grid_y, cudaStream_t stream) {
-  using C = DecodeFp8Cfg<HKV_CTA>;
-  auto kern = decode_fp8_kernel<HKV_CTA>;
+  using C = DecodeFp8Cfg<HKV_CTA, NCW>;
+  auto kern = decode_fp8_kernel<HKV_CTA, NCW>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
     return LAZY_ERR_CUDA;
   const CUtensorMap* mk = reinterpret_cast<const CUtensorMap*>(h->tmap_k);
   const CUtensorMap* mv = reinterpret_cast<const CUtensorMap*>(h->tmap_v);
-  kern<<<dim3(grid_x, grid_y), kDecodeThreads, C::SMEM_BYTES, stream>>>(*mk, *mv, args);
+  kern<<<dim3(grid_x, grid_y), C::THREADS, C::SMEM_BYTES, stream>>>(*mk, *mv, args);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
 
@@ -149,10 +149,13 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
                   const int32_t* block_table, const int32_t* page_logical_pos, const int32_t* seq_lens,
                   int num_reqs, void* out, cudaStream_t stream) {
   const lazy_config& c = h->cfg;
-  const int hkv_cta = c.num_kv_heads >= 8 ? 8 : c.num_kv_heads;
+  const bool fp8 = c.dtype == LAZY_KV_FP8_E4M3;
+  // FP8 pages: 12 consumer warps = 4 kv heads x 3 pages (or fewer heads x more pages) per stage, unless the A/B flag
+  // asks for the bf16 kernel's 8-warp cut
+  const bool w12 = fp8 && !(c.flags & LAZY_FLAG_FP8_DECODE_8_WARPS);
+  const int hkv_cta = w12 ? (c.num_kv_heads >= 4 ? 4 : c.num_kv_heads) : (c.num_kv_heads >= 8 ? 8 : c.num_kv_heads);
   const int HG = c.num_kv_heads / hkv_cta;
   const long long rows = (long long)c.num_pages * c.num_kv_heads * kPageSize;
-  const bool fp8 = c.dtype == LAZY_KV_FP8_E4M3;
   if (fp8 && c.head_dim != 128) return LAZY_ERR_UNSUPPORTED;   // the caller routes head_dim 64 to the row-wise kernel
   if (h->tmap_k_ptr != k_cache) {
     if (!(fp8 ? encode_pool_tmap_u8(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta, true)
@@ -167,8 +170,9 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
     h->tmap_v_ptr = v_cache;
   }
   int launches = 0;
-  for (int r0 = 0; r0 < num_reqs; r0 += kMaxReqsSmem) {
-    const int n = (num_reqs - r0 < kMaxReqsSmem) ? num_reqs - r0 : kMaxReqsSmem;
+  const int max_reqs = kMaxReqsSmem;                                // requests per launch (smem prefix sums)
+  for (int r0 = 0; r0 < num_reqs; r0 += max_reqs) {
+    const int n = (num_reqs - r0 < max_reqs) ? num_reqs - r0 : max_reqs;
     DecodeArgs a;
     a.q = static_cast<const __nv_bfloat16*>(q) + (size_t)r0 * c.num_q_heads * c.head_dim;
     a.out = static_cast<__nv_bfloat16*>(out) + (size_t)r0 * c.num_q_heads * c.head_dim;
@@ -193,10 +197,14 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
       fa.d = a;
       fa.k_scale = h->k_scale;
       fa.v_scale = h->v_scale;
-      if (hkv_cta == 8) rc = launch_decode_fp8_t<8>(h, fa, gx, HG, stream);
-      else if (hkv_cta == 4) rc = launch_decode_fp8_t<4>(h, fa, gx, HG, stream);
-      else if (hkv_cta == 2) rc = launch_decode_fp8_t<2>(h, fa, gx, HG, stream);
-      else rc = launch_decode_fp8_t<1>(h, fa, gx, HG, stream);
+      if (w12) {
+        if (hkv_cta == 4) rc = launch_decode_fp8_t<4, 12>(h, fa, gx, HG, stream);
+        else if (hkv_cta == 2) rc = launch_decode_fp8_t<2, 12>(h, fa, gx, HG, stream);
+        else rc = launch_decode_fp8_t<1, 12>(h, fa, gx, HG, stream);
+      } else if (hkv_cta == 8) rc = launch_decode_fp8_t<8, 8>(h, fa, gx, HG, stream);
+      else if (hkv_cta == 4) rc = launch_decode_fp8_t<4, 8>(h, fa, gx, HG, stream);
+      else if (hkv_cta == 2) rc = launch_decode_fp8_t<2, 8>(h, fa, gx, HG, stream);
+      else rc = launch_decode_fp8_t<1, 8>(h, fa, gx, HG, stream);
     } else if (c.head_dim == 128) {
       if (hkv_cta == 8) rc = launch_decode_t<128, 8>(h, a, gx, HG, stream);
       else if (hkv_cta == 4) rc = launch_decode_t<128, 4>(h, a, gx, HG, stream);

@@ -44,8 +44,14 @@ Layout workspace_layout(const lazy_config* c) {
   size_t off = 0;
   // decode partials: one slot per (request, CTA) intersection and page lane (8 / kv-heads-per-CTA lanes)
   int hkv_cta = c->num_kv_heads >= 8 ? 8 : c->num_kv_heads;
-  size_t parts = ((size_t)c->max_reqs + lazy::kMaxDecodeCtas) * (8 / hkv_cta);
+  size_t lanes = 8 / hkv_cta;
   size_t head_groups = (size_t)c->num_kv_heads / hkv_cta;
+  if (c->dtype == LAZY_KV_FP8_E4M3) {               // 12 consumer warps: at most 4 kv heads per CTA
+    int h12 = c->num_kv_heads >= 4 ? 4 : c->num_kv_heads;
+    if ((size_t)(12 / h12) > lanes) lanes = 12 / h12;
+    if ((size_t)c->num_kv_heads / h12 > head_groups) head_groups = (size_t)c->num_kv_heads / h12;
+  }
+  size_t parts = ((size_t)c->max_reqs + lazy::kMaxDecodeCtas) * lanes;
   l.cs = off;          off = align_up(off + (size_t)c->max_position * (c->head_dim / 2) * sizeof(float2), 256);
   l.part_o = off;      off = align_up(off + parts * c->num_q_heads * c->head_dim * sizeof(float), 256);
   l.part_ml = off;     off = align_up(off + parts * c->num_q_heads * sizeof(float2), 256);

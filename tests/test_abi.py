@@ -56,7 +56,7 @@ def test_workspace_bytes(lib):
     assert B.lazy_workspace_bytes(_cfg(num_q_heads=32, num_kv_heads=2)) == 0   # group 16 > 8
     assert B.lazy_workspace_bytes(_cfg(num_pages=0)) == 0
     assert B.lazy_workspace_bytes(_cfg(dtype=2)) == 0
-    assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3)) == n          # FP8 pages: same workspace
+    assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3)) >= n          # FP8 pages: more split-KV partial slots
     assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3, k_storage=1)) == 0
     assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3, rope_style=2)) == 0
 
