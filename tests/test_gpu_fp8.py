@@ -152,3 +152,55 @@ def test_fp8_mixed_call_matches_oracle():
         compare(out_d, ref_d, "fp8 mixed decode")
     finally:
         dev.close()
+
+
+# ---- edge cases on FP8 pages: ragged lengths, partial (poisoned) last pages, repeated pages, position gaps, keys
+# positioned above the query, every head grouping of the 12-warp and 8-warp decode cuts, empty requests
+from test_gpu_edges import _custom, SH128, SH64, SH7   # noqa: E402
+
+SH2 = W.LazyShape(8, 2, 128, 1.0e4)      # 2 kv heads: 6 pages per stage in the 12-warp cut
+SH1 = W.LazyShape(8, 1, 128, 1.0e4)      # 1 kv head: 12 pages per stage
+SH16 = W.LazyShape(32, 16, 128, 5.0e5)   # 16 kv heads: 4 head groups (grid.y = 4)
+DFLAGS = [pytest.param(0, id="w12"), pytest.param(B.LAZY_FLAG_FP8_DECODE_8_WARPS, id="w8")]
+
+
+@pytest.mark.parametrize("flags", DFLAGS)
+@pytest.mark.parametrize("shape", [SH128, SH7, SH2, SH1, SH16, SH64], ids=["g4", "g7", "hkv2", "hkv1", "hkv16", "d64"])
+def test_fp8_ragged_decode(shape, flags):
+    seq = [1, 2, 15, 16, 17, 31, 33, 100, 257, 640, 1000, 3]
+    _run(_custom(shape, seq, [1] * len(seq), seed=21, kind="decode"), flags=flags)
+
+
+@pytest.mark.parametrize("shape", [SH128, SH64, SH7, SH2], ids=["g4d128", "g4d64", "g7d128", "hkv2"])
+def test_fp8_ragged_prefill(shape):
+    seq = [5, 16, 200, 129, 300, 47, 1]
+    qls = [5, 3, 200, 1, 130, 47, 1]
+    _run(_custom(shape, seq, qls, seed=22))
+
+
+def test_fp8_zero_length_repeated_pages_gaps():
+    _run(_custom(SH128, [0, 40, 0], [1, 1, 1], seed=23, kind="decode"))
+    _run(_custom(SH128, [33, 0, 20], [4, 0, 20], seed=24))
+    _run(_custom(SH128, [200, 333], [1, 1], seed=25, repeat_pages=True, kind="decode"))
+    _run(_custom(SH128, [200, 333], [8, 70], seed=26, repeat_pages=True, pos_gap=1000))
+    _run(_custom(SH128, [77, 160], [1, 1], seed=27, pos_gap=4096, unaligned_pos=True, kind="decode"))
+
+
+def test_fp8_key_positions_above_the_query():
+    """Pages positioned AFTER the query token (negative page offset: the sign path of the q re-rotation)."""
+    b = _custom(SH128, [100, 260], [1, 1], seed=28, kind="decode")
+    pp = b.page_logical_pos.clone()
+    pp[:, 0:3] += 5000                               # the first pages sit far above the query's position
+    b.page_logical_pos = pp
+    _run(b)
+    b2 = _custom(SH128, [100, 260], [10, 40], seed=29)
+    pp = b2.page_logical_pos.clone()
+    pp[:, 1:3] += 7000
+    b2.page_logical_pos = pp
+    _run(b2)
+
+
+def test_fp8_many_requests_split_over_launches():
+    """More requests than one decode launch holds in shared memory (2048)."""
+    n = 2100
+    _run(_custom(W.LazyShape(8, 4, 128, 1.0e4), [3 + (i % 40) for i in range(n)], [1] * n, seed=30, kind="decode"))
