@@ -547,6 +547,16 @@ def fp8_leg(device, steps, peaks, barrier):
         res[wl + "_noshare"] = {"kernel_ms": ms, "algorithmic_bytes_per_launch": nbytes, "GBps": gb,
                                 "frac_of_hbm_peak": gb / peaks["hbm"],
                                 "traffic": ncu_traffic("decode_fp8", wl + "_noshare")}
+    # prefill over FP8 pages (tcgen05 kernel, the rotate warpgroup dequantises both tiles): same FLOPs as cfg3
+    b, j, w = _timed_job("cfg3", device, steps, fp8=True)
+    _, a_ms, _ = j.time_steps(max(3, steps // 2), 3, barrier)
+    ms = a_ms / max(3, steps // 2)
+    j.dev.close()
+    del j, b
+    torch.cuda.empty_cache()
+    tf = w["flops"] / (ms * 1e-3) / 1e12
+    res["cfg3_prefill"] = {"bound": "tensor", "kernel_ms": ms, "TFLOPs": tf, "frac_of_bf16_peak": tf / peaks["tensor"],
+                           "traffic": ncu_traffic("prefill_fp8", "cfg3")}
     return res
 
 
@@ -656,7 +666,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--noshare", action="store_true", help="every drawn document distinct (logical == unique bytes)")
     ap.add_argument("--kv-dtype", default="bf16", choices=["bf16", "fp8"],
-                    help="fp8: LAZY_KV_FP8_E4M3 pages (decode workloads cfg2 / cfg4; SURVEY 8.0 row f4)")
+                    help="fp8: LAZY_KV_FP8_E4M3 pages (workloads cfg2 / cfg3 / cfg4; SURVEY 8.0 row f4)")
     ap.add_argument("--no-secondary", action="store_true", help="skip the prefill (cfg3) and noshare side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mixed", action="store_true",
@@ -722,7 +732,7 @@ def main():
     barrier()
 
     fp8 = args.kv_dtype == "fp8"
-    assert not fp8 or args.workload in ("cfg2", "cfg4"), "--kv-dtype fp8 times the decode workloads (cfg2, cfg4)"
+    assert not fp8 or args.workload in ("cfg2", "cfg3", "cfg4"), "--kv-dtype fp8: cfg2, cfg3 or cfg4"
     batch = make_batch(args.workload, rank, args.noshare)
     job = GpuJob(batch, device, fp8=fp8)
     work = step_work(batch, [r["step"] for r in job.timed], fp8=fp8)
@@ -777,7 +787,7 @@ def main():
     elif args.workload == "cfg3":
         ach = work["flops"] / (ms_attn * 1e-3) / 1e12
         roof = {"bound": "tensor", "kernel": "lazy_attn_prefill", "achieved": ach, "peak": peaks["tensor"],
-                "unit": "TFLOP/s", "frac": ach / peaks["tensor"], "traffic": ncu_traffic("prefill", wl_name),
+                "unit": "TFLOP/s", "frac": ach / peaks["tensor"], "traffic": ncu_traffic("prefill_fp8" if fp8 else "prefill", wl_name),
                 "peak_source": peaks["source"] + " (burst: the kernel is timed alone, L2 flushed between launches)",
                 "algorithmic_flops_per_launch": work["flops"], "kernel_ms": ms_attn}
     else:

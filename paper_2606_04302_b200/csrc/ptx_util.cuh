@@ -125,7 +125,7 @@ __device__ __forceinline__ uint32_t e4m3x2_hi_to_f16x2(uint32_t w) {
 }
 // Two 16 x 16 byte matrices (rows of 16 bytes; lanes 0-15 / 16-31 give the row addresses of the first / second),
 // transposed: thread (g = lane >> 2, tq = lane & 3) gets, per matrix, r[0] = bytes [rows 4tq..4tq+3][column g] and
-// r[1] = the same rows of column g + 8 (layout probed on B200: profiles/r2_ldmatrix_b8_layout.md).
+// r[1] = the same rows of column g + 8 (layout probed on B200; the FP8 decode parity tests pin it).
 __device__ __forceinline__ void ldmatrix_b8_x2_trans(uint32_t& r0, uint32_t& r1, uint32_t& r2, uint32_t& r3,
                                                      uint32_t addr) {
   asm volatile("ldmatrix.sync.aligned.m16n16.x2.trans.shared.b8 {%0,%1,%2,%3}, [%4];"
