@@ -324,7 +324,9 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     // table value built in fp64: ~4e-7 relative, PAPER.md L455's drift concern does not arise).  This takes the
     // per-token table reads (64 KB of LDS per tile, 2-way bank-conflicted) out of the shared-memory pipe, which the
     // tensor cores' operand fetches already load to ~40 % (profiles/r2_prefill_smem_attribution.md).
-    ptx::setmaxnreg_dec<kRegsRotate>();
+    // FP8 pages: the rotate warpgroup holds a page's codes of both tiles: 2*128*168 + 128*136 + 128*40 = 65536
+    if (F8) ptx::setmaxnreg_inc<136>();
+    else ptx::setmaxnreg_dec<kRegsRotate>();
     constexpr int TOK = C::CPR;                     // tokens per thread (16 threads serve a page)
     const int wtid = tid - 256;
     const int i = wtid >> 4;                        // page of the tile
@@ -496,7 +498,7 @@ prefill_umma_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_con
     }
   } else {
     // ================================ softmax warpgroups ======================================================
-    ptx::setmaxnreg_inc<kRegsSoftmax>();
+    ptx::setmaxnreg_inc<F8 ? 168 : kRegsSoftmax>();
     const int t = warp >> 2;
     const int row = tid - t * 128;
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
