@@ -81,12 +81,13 @@ bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, in
 
 // FP8 code pool: rows of D bytes; box = [box_rows][D bytes] (swizzled for the decode kernel -- D = 128: one 128-byte
 // swizzle span per row -- plain rows for the prefill kernel, which re-writes the tile as bf16)
-bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D, int box_rows, bool swizzle) {
+bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D, int box_rows, bool swizzle,
+                         int box_cols) {
   EncodeTiledFn fn = get_encode_fn();
   if (!fn) return false;
   cuuint64_t gdim[2] = {(cuuint64_t)D, (cuuint64_t)rows};
   cuuint64_t gstride[1] = {(cuuint64_t)D};
-  cuuint32_t box[2] = {(cuuint32_t)D, (cuuint32_t)box_rows};
+  cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
   cuuint32_t estr[2] = {1u, 1u};
   CUresult rc = fn(reinterpret_cast<CUtensorMap*>(out_map), CU_TENSOR_MAP_DATA_TYPE_UINT8, 2,
                    const_cast<void*>(pool), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
@@ -158,13 +159,13 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
   const long long rows = (long long)c.num_pages * c.num_kv_heads * kPageSize;
   if (fp8 && c.head_dim != 128) return LAZY_ERR_UNSUPPORTED;   // the caller routes head_dim 64 to the row-wise kernel
   if (h->tmap_k_ptr != k_cache) {
-    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta, true)
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta, true, c.head_dim)
               : encode_pool_tmap(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta)))
       return LAZY_ERR_CUDA;
     h->tmap_k_ptr = k_cache;
   }
   if (h->tmap_v_ptr != v_cache) {
-    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta, true)
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta, true, c.head_dim)
               : encode_pool_tmap(h->tmap_v, v_cache, rows, c.head_dim, 16 * hkv_cta)))
       return LAZY_ERR_CUDA;
     h->tmap_v_ptr = v_cache;

@@ -67,7 +67,8 @@ namespace lazy {
 //   q    : 4-D view (D, group, Hkv, total_q) of q [total_q][Hq][D], box = (64, group, 1, tokens_per_tile):
 //          lands as rows token*group + head-in-group of one kv head's GQA group.
 bool encode_pool_tmap(void* out_map, const void* pool, long long rows, int D, int box_rows);
-bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D, int box_rows, bool swizzle);
+bool encode_pool_tmap_u8(void* out_map, const void* pool, long long rows, int D, int box_rows, bool swizzle,
+                         int box_cols);
 bool encode_q_tmap(void* out_map, const void* q, int total_q, int Hq, int Hkv, int D, int tokens_per_tile);
 
 // Each launcher enqueues on `stream` and returns the number of kernels launched (<0: LAZY_ERR_*).

@@ -1,6 +1,8 @@
 // prefill_pair_kernel.cuh -- one CTA of a prefill CTA pair (head_dim 128, tcgen05 cta_group::2) as a device function,
 // shared by prefill_umma2.cu (its own kernel) and mixed_fused.cu.  See prefill_umma2.cu for the design notes.
 #pragma once
+#include <cuda_fp16.h>
+
 #include "prefill_common.cuh"
 
 namespace lazy {
@@ -22,10 +24,12 @@ struct PairCfg {                        // head_dim 128
   static constexpr int OFF_V = OFF_K + kStages * K_STAGE;
   static constexpr int OFF_CS = OFF_V + kStages * V_STAGE;
   static constexpr int OFF_BAR = OFF_CS + kStages * CS_STAGE;
-  static constexpr int NUM_BARS = 40;
+  static constexpr int NUM_BARS = 48;
   static constexpr int OFF_TMEM = OFF_BAR + NUM_BARS * 8;
   static constexpr int OFF_SIGN = OFF_TMEM + 16;                // ring of 8 tiles x 8 pages (sign / page start)
-  static constexpr int SMEM_BYTES = OFF_SIGN + 8 * kPagesPerTile * 4 + 1024;   // + alignment slack
+  static constexpr int OFF_SC = OFF_SIGN + 8 * kPagesPerTile * 4;   // FP8 pages: [stage][4 K pages | 8 V pages][16] row scales
+  static constexpr int SC_STAGE = (kHalfPages + kPagesPerTile) * 64;
+  static constexpr int SMEM_BYTES = OFF_SC + kStages * SC_STAGE + 1024;   // + alignment slack
 };
 
 // barrier indices.  (L): only the leader CTA's copy is used, threads of both CTAs arrive on it.
@@ -44,7 +48,22 @@ enum : int {
   P_PREADY = 30,    // +2t+h  softmax WG t of both CTAs -> MMA: P half h is in TMEM (L)
   P_PVDONE = 34,    // +2t+h  MMA commit (multicast) -> softmax WG t: O_t += P_h V has completed (slow path only)
   P_OFULL = 38,     // +t     MMA commit (multicast) -> softmax WG t (epilogue)
+  P_VLOCAL = 40,    // +s     FP8 pages: this CTA's V boxes (codes + scales) -> its rotate WG (local)
+  P_VREADY = 44,    // +s     FP8 pages: rotate WGs of both CTAs (8 warps) -> MMA: V tile dequantised     (L)
 };
+
+// FP8 pages: 8 E4M3 codes (two words) -> 8 fp32 values, exact
+__device__ __forceinline__ void pair_e4m3x8_to_f32(uint2 v, float2 (&x)[4]) {
+  const uint32_t h[4] = {ptx::e4m3x2_lo_to_f16x2(v.x), ptx::e4m3x2_hi_to_f16x2(v.x), ptx::e4m3x2_lo_to_f16x2(v.y),
+                         ptx::e4m3x2_hi_to_f16x2(v.y)};
+#pragma unroll
+  for (int w = 0; w < 4; ++w) x[w] = __half22float2(*reinterpret_cast<const __half2*>(&h[w]));
+}
+__device__ __forceinline__ uint2 pair_lds64(uint32_t addr) {
+  uint2 v;
+  asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+  return v;
+}
 
 // byte offset of 16-byte chunk `ci` of row `row` (0..63) inside a K half-stage (two 64-row slabs, 128B swizzle)
 __device__ __forceinline__ uint32_t kchunk_off(int row, int ci) {
@@ -53,7 +72,11 @@ __device__ __forceinline__ uint32_t kchunk_off(int row, int ci) {
 
 // The body of one CTA of a pair; `pair` is the pair's work-item index.  prefill_pair_kernel maps it to blockIdx.x / 2;
 // the fused mixed-step kernel (mixed_fused.cu) runs the same body on the CTAs behind its decode CTAs.
-template <int KM>
+// F8: LAZY_KV_FP8_E4M3 pages.  As in prefill_umma.cu, a page's codes land (plain rows) at the start of the page's own
+// region of the bf16 stage and the rotate warpgroup writes the bf16 tile over them: this CTA's 4 pages of K dequantised
+// and rotated, its 64-column slab of all 8 pages of V dequantised (rows past the sequence cleared -- there is no tail
+// fixer).  V boxes report to a LOCAL barrier; the leader's MMA warp waits for VREADY (8 rotate warps) instead of VFULL.
+template <int KM, bool F8 = false>
 __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, const CUtensorMap& tmap_k,
                                                  const CUtensorMap& tmap_v, const PrefillArgs& a, const int pair,
                                                  unsigned char* smem_raw) {
@@ -117,6 +140,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
     }
     ptx::mbar_init(bar(P_VLASTFULL), 1);
     ptx::mbar_init(bar(P_VFIXED), 2);
+    for (int x = 0; x < kStages; ++x) { ptx::mbar_init(bar(P_VLOCAL + x), 1); ptx::mbar_init(bar(P_VREADY + x), 8); }
     ptx::fence_mbar_init();
   }
   if (warp == 13) {
@@ -172,19 +196,33 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
         if (KM == LAZY_K_STORED_POS && is_v) s_sign[(j & 7) * kPagesPerTile + pg] = p0_sign;
         if (KM == kKmAlibi && is_v) s_sign[(j & 7) * kPagesPerTile + pg] = p0;
         __syncwarp();
+        const uint32_t sSC = smem_base + C::OFF_SC + s * C::SC_STAGE;
         if (lane == 0)
-          ptx::mbar_arrive_expect_tx(bar(P_KFULL + s), npk * (2 * kPageSize * 128 + (kNoRotate ? 0 : C::CS_ROW_BYTES)));
+          ptx::mbar_arrive_expect_tx(bar(P_KFULL + s), npk * ((F8 ? kPageSize * 128 + 64 : 2 * kPageSize * 128) +
+                                                              (kNoRotate ? 0 : C::CS_ROW_BYTES)));
         __syncwarp();
         if (is_k && pgl < npk) {
-          ptx::tma_load_2d(sK + s * C::K_STAGE + half * C::K_SLAB + pgl * (kPageSize * 128), &tmap_k, bar(P_KFULL + s),
-                           half * 64, row0);
+          if (!F8) ptx::tma_load_2d(sK + s * C::K_STAGE + half * C::K_SLAB + pgl * (kPageSize * 128), &tmap_k,
+                                    bar(P_KFULL + s), half * 64, row0);
+          if (F8 && half == 0) {                    // one box of 16 rows x 128 code bytes, and the rows' scales
+            ptx::tma_load_2d(sK + s * C::K_STAGE + pgl * (kPageSize * 128), &tmap_k, bar(P_KFULL + s), 0, row0);
+            ptx::bulk_load_1d(sSC + pgl * 64, a.k_scale + row0, 64, bar(P_KFULL + s));
+          }
           if (half == 0 && !kNoRotate)
             ptx::bulk_load_1d(sCS + s * C::CS_STAGE + pgl * C::CS_ROW_BYTES, a.cs + (size_t)p0 * (D / 2),
                               C::CS_ROW_BYTES, bar(P_KFULL + s));
         }
         ptx::mbar_wait_sleep(bar(P_VEMPTY + s), ph ^ 1);
         const uint32_t vdst = sV + s * C::V_STAGE + (lane & 7) * (kPageSize * 128);
-        if (j < n_kv - 1) {
+        if (F8) {
+          // this CTA's 64 code bytes of each row of every page of the tile + the rows' scales, to the local barrier
+          if (lane == 0) ptx::mbar_arrive_expect_tx(bar(P_VLOCAL + s), npv * (kPageSize * 64 + 64));
+          __syncwarp();
+          if (is_v && (lane & 7) < npv) {
+            ptx::tma_load_2d(vdst, &tmap_v, bar(P_VLOCAL + s), rank * 64, row0);
+            ptx::bulk_load_1d(sSC + (kHalfPages + (lane & 7)) * 64, a.v_scale + row0, 64, bar(P_VLOCAL + s));
+          }
+        } else if (j < n_kv - 1) {
           // bytes of both CTAs are counted on the leader's barrier; the leader announces them (a peer box that lands
           // first only drives the pending-byte count negative for a moment)
           if (lane == 0 && rank == 0) ptx::mbar_arrive_expect_tx(bar(P_VFULL + s), 2 * npv * kPageSize * 128);
@@ -251,7 +289,8 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
         // ahead of the other; the kernel then alternated between bursts of one tile and refill latencies: 668 TFLOP/s.)
         for (int j = 0; j < nkv; ++j) {
           const int s = j & (kStages - 1), sn = (j + 1) & (kStages - 1);
-          if (j == nkv - 1) ptx::mbar_wait(bar(P_VFIXED), 0);
+          if (F8) ptx::mbar_wait(bar(P_VREADY + s), (j / kStages) & 1);
+          else if (j == nkv - 1) ptx::mbar_wait(bar(P_VFIXED), 0);
           else ptx::mbar_wait(bar(P_VFULL + s), (j / kStages) & 1);
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
@@ -278,7 +317,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
         }
         __syncwarp();
       }
-    } else if (warp == 14) {
+    } else if (warp == 14 && !F8) {
       // ================================ V tail fixer ========================================================
       // zeroes the rows >= seq_len of this CTA's slab of the last V tile, so that poisoned bytes never reach PV
       const int jl = n_kv - 1;
@@ -301,7 +340,9 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
     // a 16-byte access) hold the four c of one parity x two ADJACENT tokens: their table chunks are 4 distinct
     // 16-byte words (broadcast across the two tokens; chunk pairs c and c+1 would collide, they sit 256 B apart), and
     // their K chunks, swizzled by (row & 7), fall into disjoint bank groups because adjacent rows differ in parity.
-    ptx::setmaxnreg_dec<kRegsRotate>();
+    // (FP8 pages: the warpgroup holds a page's codes of both tiles: 2*128*168 + 128*136 + 128*40 = 65536)
+    if (F8) ptx::setmaxnreg_inc<136>();
+    else ptx::setmaxnreg_dec<kRegsRotate>();
     constexpr int TOK = 4;
     const int wtid = tid - 256;
     const int i = wtid >> 5;                        // page of this CTA's half tile
@@ -326,6 +367,104 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
       const uint32_t kb = sK + s * C::K_STAGE;
       const uint32_t cb = sCS + s * C::CS_STAGE;
       ptx::mbar_wait(bar(P_KFULL + s), (j / kStages) & 1);
+      if (F8) {
+        // ---- K: this CTA's 4 pages; thread = (page i, tokens tg + 4tt, pairs 8c..8c+7); a warp serves one page
+        const uint32_t sc = smem_base + C::OFF_SC + s * C::SC_STAGE;
+        const uint32_t land = kb + i * (kPageSize * 128) + tg * 128 + 8 * c;     // codes of (page i, token tg, dims 8c..)
+        uint2 ra[TOK], rb[TOK];
+        float scl[TOK];
+        float2 zc[4], zs[4];
+        if (i < npk) {
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            const uint4 v = ptx::lds128(cb + i * C::CS_ROW_BYTES + 16 * cs_f4_index<D>(c, x));
+            const float2 wc = make_float2(f32(v.x), f32(v.y)), ws = make_float2(f32(v.z), f32(v.w));
+            zc[x] = __ffma2_rn(neg2(ws), u0s[x], __fmul2_rn(wc, u0c[x]));
+            zs[x] = __ffma2_rn(wc, u0s[x], __fmul2_rn(ws, u0c[x]));
+          }
+#pragma unroll
+          for (int tt = 0; tt < TOK; ++tt) {
+            ra[tt] = pair_lds64(land + 4 * tt * 128);
+            rb[tt] = pair_lds64(land + 4 * tt * 128 + 64);
+            scl[tt] = __int_as_float(ptx::lds32(sc + i * 64 + (tg + 4 * tt) * 4));
+          }
+        }
+        __syncwarp();                               // the page's codes are in registers: overwrite them
+        if (i < npk) {
+          const int row0 = i * kPageSize + tg;
+#pragma unroll
+          for (int tt = 0; tt < TOK; ++tt) {
+            float2 x1[4], x2[4];
+            pair_e4m3x8_to_f32(ra[tt], x1);
+            pair_e4m3x8_to_f32(rb[tt], x2);
+            const float2 sk2 = make_float2(scl[tt], scl[tt]);
+            uint4 va, vb;
+            uint32_t* aw = reinterpret_cast<uint32_t*>(&va);
+            uint32_t* bw = reinterpret_cast<uint32_t*>(&vb);
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+              const float2 cc = __fmul2_rn(zc[w], sk2), ss = __fmul2_rn(zs[w], sk2);
+              const float2 y1 = __ffma2_rn(neg2(x2[w]), ss, __fmul2_rn(x1[w], cc));
+              const float2 y2 = __ffma2_rn(x2[w], cc, __fmul2_rn(x1[w], ss));
+              aw[w] = ptx::pack_bf16(y1.x, y1.y);
+              bw[w] = ptx::pack_bf16(y2.x, y2.y);
+            }
+            ptx::sts128(kb + kchunk_off(row0 + 4 * tt, c), va);
+            ptx::sts128(kb + kchunk_off(row0 + 4 * tt, c + 8), vb);
+            if (tt + 1 < TOK) {
+#pragma unroll
+              for (int x = 0; x < 4; ++x) {
+                const float2 wc = zc[x], ws = zs[x];
+                zc[x] = __ffma2_rn(neg2(ws), u1s[x], __fmul2_rn(wc, u1c[x]));
+                zs[x] = __ffma2_rn(wc, u1s[x], __fmul2_rn(ws, u1c[x]));
+              }
+            }
+          }
+        }
+        ptx::fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_KREADY + s));
+        // ---- V: this CTA's 64-column slab of all 8 pages; thread = (page vp, token vt): 64 codes -> one 128-byte row
+        const int vp = wtid >> 4, vt = wtid & 15;
+        const int vrow = vp * kPageSize + vt;
+        const uint32_t vs_ = sV + s * C::V_STAGE;
+        ptx::mbar_wait(bar(P_VLOCAL + s), (j / kStages) & 1);
+        const bool live = vp < npv && j * kTileRows + vrow < L;
+        uint4 cv[4];
+        float sv = 0.f;
+        if (live) {
+#pragma unroll
+          for (int x = 0; x < 4; ++x) cv[x] = ptx::lds128(vs_ + vp * (kPageSize * 128) + vt * 64 + 16 * x);
+          sv = __int_as_float(ptx::lds32(sc + (kHalfPages + vp) * 64 + vt * 4));
+        }
+        __syncwarp();
+        if (vp < npv || j == n_kv - 1) {            // pages that do not exist are cleared on the last tile only
+          const float2 sv2 = make_float2(sv, sv);
+#pragma unroll
+          for (int x = 0; x < 4; ++x) {
+            uint4 o0 = make_uint4(0, 0, 0, 0), o1 = make_uint4(0, 0, 0, 0);
+            if (live) {
+              float2 f0[4], f1[4];
+              pair_e4m3x8_to_f32(make_uint2(cv[x].x, cv[x].y), f0);
+              pair_e4m3x8_to_f32(make_uint2(cv[x].z, cv[x].w), f1);
+              uint32_t* w0 = reinterpret_cast<uint32_t*>(&o0);
+              uint32_t* w1 = reinterpret_cast<uint32_t*>(&o1);
+#pragma unroll
+              for (int w = 0; w < 4; ++w) {
+                const float2 y0 = __fmul2_rn(f0[w], sv2), y1 = __fmul2_rn(f1[w], sv2);
+                w0[w] = ptx::pack_bf16(y0.x, y0.y);
+                w1[w] = ptx::pack_bf16(y1.x, y1.y);
+              }
+            }
+            ptx::sts128(vs_ + vrow * 128 + (((2 * x) ^ (vrow & 7)) << 4), o0);
+            ptx::sts128(vs_ + vrow * 128 + (((2 * x + 1) ^ (vrow & 7)) << 4), o1);
+          }
+        }
+        ptx::fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_VREADY + s));
+        continue;
+      }
       if (!kNoRotate && i < npk) {
         float2 zc[4], zs[4];                        // e^{i (p0+t) theta_j}, or e^{i Delta theta_j} of the page
 #pragma unroll
@@ -374,7 +513,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
     }
   } else {
     // ================================ softmax warpgroups ======================================================
-    ptx::setmaxnreg_inc<kRegsSoftmax>();
+    ptx::setmaxnreg_inc<F8 ? 168 : kRegsSoftmax>();
     const int t = warp >> 2;
     const int row = tid - t * 128;
     const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;

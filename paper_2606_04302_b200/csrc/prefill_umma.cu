@@ -800,14 +800,16 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   const int tpt = kTileRows / group;                 // query tokens per 128-row tile
   const long long rows = (long long)c.num_pages * c.num_kv_heads * kPageSize;
   const bool fp8 = c.dtype == LAZY_KV_FP8_E4M3;
+  const bool fp8_pair = fp8 && c.head_dim == 128 && !(c.flags & LAZY_FLAG_PREFILL_ONE_CTA);
   if (h->tmap_pk_ptr != k_cache) {
-    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_pk, k_cache, rows, c.head_dim, kPageSize, false)
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_pk, k_cache, rows, c.head_dim, kPageSize, false, c.head_dim)
               : encode_pool_tmap(h->tmap_pk, k_cache, rows, c.head_dim, kPageSize)))
       return LAZY_ERR_CUDA;
     h->tmap_pk_ptr = k_cache;
   }
   if (h->tmap_pv_ptr != v_cache) {
-    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_pv, v_cache, rows, c.head_dim, kPageSize, false)
+    // (FP8 pages on CTA pairs: a CTA takes its own 64 code bytes of every V row)
+    if (!(fp8 ? encode_pool_tmap_u8(h->tmap_pv, v_cache, rows, c.head_dim, kPageSize, false, fp8_pair ? 64 : c.head_dim)
               : encode_pool_tmap(h->tmap_pv, v_cache, rows, c.head_dim, kPageSize)))
       return LAZY_ERR_CUDA;
     h->tmap_pv_ptr = v_cache;
@@ -833,8 +835,8 @@ int launch_prefill(lazy_handle* h, const void* q, const void* k_cache, const voi
   a.sh = h->shape;
   a.k_scale = h->k_scale;
   a.v_scale = h->v_scale;
-  if (fp8) {
-    // FP8 pages run on the one-CTA kernel at either head_dim (its rotate warpgroup dequantises both tiles)
+  if (fp8 && !fp8_pair) {
+    // FP8 pages at head_dim 64 (and the A/B arm at 128) run on the one-CTA kernel
     const long long grid = (long long)a.mblocks * c.num_kv_heads * num_reqs;
     if (grid <= 0 || grid > INT_MAX) return LAZY_ERR_INVALID;
     return c.head_dim == 128 ? launch_prefill_t<128, LAZY_K_UNROTATED, true>(h, a, (int)grid, stream)

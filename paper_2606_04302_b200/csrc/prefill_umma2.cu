@@ -24,17 +24,17 @@
 namespace lazy {
 namespace {
 
-template <int KM>
+template <int KM, bool F8>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kPrefillThreads, 1)
 prefill_pair_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
                     const __grid_constant__ CUtensorMap tmap_v, const PrefillArgs a) {
   extern __shared__ unsigned char smem_raw[];
-  prefill_pair_cta<KM>(tmap_q, tmap_k, tmap_v, a, (int)(blockIdx.x >> 1), smem_raw);
+  prefill_pair_cta<KM, F8>(tmap_q, tmap_k, tmap_v, a, (int)(blockIdx.x >> 1), smem_raw);
 }
 
-template <int KM>
+template <int KM, bool F8 = false>
 int launch_pair_t(const lazy_handle* h, const PrefillArgs& args, int grid, cudaStream_t stream) {
-  auto kern = prefill_pair_kernel<KM>;
+  auto kern = prefill_pair_kernel<KM, F8>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, PairCfg::SMEM_BYTES) != cudaSuccess)
     return LAZY_ERR_CUDA;
   const CUtensorMap* mq = reinterpret_cast<const CUtensorMap*>(h->tmap_pq);
@@ -48,6 +48,7 @@ int launch_pair_t(const lazy_handle* h, const PrefillArgs& args, int grid, cudaS
 
 // head_dim 128 only; `a.mblocks` counts CTA PAIRS per (request, kv head); the grid is 2 CTAs per pair.
 int launch_prefill_pair(const lazy_handle* h, const PrefillArgs& a, int km, int grid, cudaStream_t stream) {
+  if (h->cfg.dtype == LAZY_KV_FP8_E4M3) return launch_pair_t<LAZY_K_UNROTATED, true>(h, a, grid, stream);
   switch (km) {
     case LAZY_K_STORED_POS: return launch_pair_t<LAZY_K_STORED_POS>(h, a, grid, stream);
     case LAZY_K_ABSOLUTE:   return launch_pair_t<LAZY_K_ABSOLUTE>(h, a, grid, stream);

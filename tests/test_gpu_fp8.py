@@ -11,7 +11,8 @@ from paper_2606_04302_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
-FLAGS = [pytest.param(0, id="prod"), pytest.param(B.LAZY_FLAG_ROWWISE_KERNELS, id="rowwise")]
+FLAGS = [pytest.param(0, id="prod"), pytest.param(B.LAZY_FLAG_ROWWISE_KERNELS, id="rowwise"),
+         pytest.param(B.LAZY_FLAG_PREFILL_ONE_CTA, id="one_cta")]   # head_dim 128 prefill on single CTAs (A/B arm)
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -171,11 +172,12 @@ def test_fp8_ragged_decode(shape, flags):
     _run(_custom(shape, seq, [1] * len(seq), seed=21, kind="decode"), flags=flags)
 
 
+@pytest.mark.parametrize("flags", [pytest.param(0, id="pairs"), pytest.param(B.LAZY_FLAG_PREFILL_ONE_CTA, id="one_cta")])
 @pytest.mark.parametrize("shape", [SH128, SH64, SH7, SH2], ids=["g4d128", "g4d64", "g7d128", "hkv2"])
-def test_fp8_ragged_prefill(shape):
+def test_fp8_ragged_prefill(shape, flags):
     seq = [5, 16, 200, 129, 300, 47, 1]
     qls = [5, 3, 200, 1, 130, 47, 1]
-    _run(_custom(shape, seq, qls, seed=22))
+    _run(_custom(shape, seq, qls, seed=22), flags=flags)
 
 
 def test_fp8_zero_length_repeated_pages_gaps():
