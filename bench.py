@@ -557,6 +557,13 @@ def fp8_leg(device, steps, peaks, barrier):
     tf = w["flops"] / (ms * 1e-3) / 1e12
     res["cfg3_prefill"] = {"bound": "tensor", "kernel_ms": ms, "TFLOPs": tf, "frac_of_bf16_peak": tf / peaks["tensor"],
                            "traffic": ncu_traffic("prefill_fp8", "cfg3")}
+    # the mixed step (configs[4]) on FP8 pages: one launch (mixed_step_fp8_kernel)
+    b, j, w = _timed_job("cfg5", device, steps, fp8=True)
+    t_ms, a_ms, _ = j.time_steps(steps, 3, barrier)
+    j.dev.close()
+    del j, b
+    torch.cuda.empty_cache()
+    res["cfg5_mixed_step"] = {"ms_per_step": t_ms / steps, "attention_ms": a_ms / steps}
     return res
 
 
@@ -615,23 +622,23 @@ def prefill_leg(workload, device, steps, peaks, barrier, sustained_s=2.0):
     return res
 
 
-def cfg5_leg(device, steps, peaks, job=None):
+def cfg5_leg(device, steps, peaks, job=None, fp8=False):
     """configs[4], kernel by kernel (separate calls, L2 flushed before each): the block-local prefill of the 4 miss
     documents (tensor roofline; 464 one-CTA work items = 232 CTA pairs on 74 SM pairs, causal: 1..8 KV tiles per pair)
     and the decode of the 16 running requests (HBM roofline, on the noshare variant), plus the mixed-step time."""
     own = job is None
     if own:
-        b, job, _ = _timed_job("cfg5", device, steps)
+        b, job, _ = _timed_job("cfg5", device, steps, fp8=fp8)
     per = job.time_calls(steps, 3)
-    works = {r["step"].kind: step_work(job.batch, [r["step"]]) for r in job.timed}
+    works = {r["step"].kind: step_work(job.batch, [r["step"]], fp8=fp8) for r in job.timed}
     t_ms, a_ms, _ = job.time_steps(steps, 3, lambda: None)
     if own:
         job.dev.close()
         del job
         torch.cuda.empty_cache()
-    bn, jn, _ = _timed_job("cfg5", device, steps, noshare=True)
+    bn, jn, _ = _timed_job("cfg5", device, steps, noshare=True, fp8=fp8)
     per_ns = jn.time_calls(steps, 3)
-    wn = {r["step"].kind: step_work(bn, [r["step"]]) for r in jn.timed}
+    wn = {r["step"].kind: step_work(bn, [r["step"]], fp8=fp8) for r in jn.timed}
     jn.dev.close()
     tf = works["prefill"]["flops"] / (per["prefill"] * 1e-3) / 1e12
     sh = bn.shape
@@ -666,7 +673,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--noshare", action="store_true", help="every drawn document distinct (logical == unique bytes)")
     ap.add_argument("--kv-dtype", default="bf16", choices=["bf16", "fp8"],
-                    help="fp8: LAZY_KV_FP8_E4M3 pages (workloads cfg2 / cfg3 / cfg4; SURVEY 8.0 row f4)")
+                    help="fp8: LAZY_KV_FP8_E4M3 pages (SURVEY 8.0 row f4)")
     ap.add_argument("--no-secondary", action="store_true", help="skip the prefill (cfg3) and noshare side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mixed", action="store_true",
@@ -732,7 +739,6 @@ def main():
     barrier()
 
     fp8 = args.kv_dtype == "fp8"
-    assert not fp8 or args.workload in ("cfg2", "cfg3", "cfg4"), "--kv-dtype fp8: cfg2, cfg3 or cfg4"
     batch = make_batch(args.workload, rank, args.noshare)
     job = GpuJob(batch, device, fp8=fp8)
     work = step_work(batch, [r["step"] for r in job.timed], fp8=fp8)
@@ -792,11 +798,11 @@ def main():
                 "algorithmic_flops_per_launch": work["flops"], "kernel_ms": ms_attn}
     else:
         # mixed step: the dominant kernel by bytes is the decode kernel; both kernels are reported per call
-        leg = cfg5_leg(device, max(5, args.steps // 2), peaks, job=job)
+        leg = cfg5_leg(device, max(5, args.steps // 2), peaks, job=job, fp8=fp8)
         d = leg["decode_noshare"]
         roof = {"bound": "hbm", "kernel": "lazy_attn_decode (split-KV + combine) of the mixed step",
                 "achieved": d["GBps"], "peak": peaks["hbm"], "unit": "GB/s", "frac": d["frac_of_hbm_peak"],
-                "traffic": ncu_traffic("decode", "cfg5_noshare"), "peak_source": peaks["source"],
+                "traffic": ncu_traffic("decode_fp8" if fp8 else "decode", "cfg5_noshare"), "peak_source": peaks["source"],
                 "workload": "cfg5 decode requests, noshare variant", "kernel_ms": d["kernel_ms"],
                 "algorithmic_bytes_per_launch": d["bytes"], "step": leg}
 

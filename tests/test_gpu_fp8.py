@@ -206,3 +206,46 @@ def test_fp8_many_requests_split_over_launches():
     """More requests than one decode launch holds in shared memory (2048)."""
     n = 2100
     _run(_custom(W.LazyShape(8, 4, 128, 1.0e4), [3 + (i % 40) for i in range(n)], [1] * n, seed=30, kind="decode"))
+
+
+@pytest.mark.parametrize("decode_sms", [0, 8, 148])
+def test_fp8_mixed_one_launch_8_kv_heads(decode_sms):
+    """The one-launch FP8 mixed step with 8 kv heads (two head groups alternate over the decode CTAs): a prefill chunk
+    of the last 8 tokens of every request and the decode of the same requests, in one call, against the oracle."""
+    from oracle import oracle as O
+    from paper_2606_04302_b200.runner import DeviceBatch
+    from gpu_util import compare
+    batch = W.config2(scale=0.1)
+    assert batch.shape.num_kv_heads == 8
+    dec = [s for s in batch.steps if s.kind == "decode"][0]
+    dev = DeviceBatch(batch, dtype=B.LAZY_KV_FP8_E4M3)
+    d = dev.device
+    pools = O.quantize_pool_fp8(batch.k_pool, batch.v_pool)
+    try:
+        for st in batch.steps:                       # every cache write of the batch (question tokens, decode token)
+            dev.write(st)
+            if st.k_new is not None:
+                O.cache_write_fp8(st.k_new, st.v_new, st.slot_mapping.numpy(), pools)
+        R = dec.seq_lens.shape[0]
+        nq = 8
+        g = torch.Generator().manual_seed(77)
+        qp = torch.randn(R * nq, batch.shape.num_q_heads, batch.shape.head_dim, generator=g).to(torch.bfloat16)
+        pre = W.Step(kind="prefill", q=qp, seq_lens=dec.seq_lens.clone(),
+                     cu_q_lens=(nq * torch.arange(R + 1)).to(torch.int32), req_ids=dec.req_ids)
+        ref_p = O.run_step_fp8(batch, pre, pools)
+        ref_d = O.run_step_fp8(batch, W.dataclasses.replace(dec, k_new=None, v_new=None, slot_mapping=None), pools)
+        bt, pp = dev.tables_for(dec)
+        out_p = torch.zeros_like(qp, device=d)
+        out_d = torch.zeros_like(dec.q, device=d)
+        for _ in range(2):
+            B.lazy_attn_mixed(dev.handle, dev.k_pool, dev.v_pool, q_prefill=qp.to(d), block_table_prefill=bt,
+                              page_logical_pos_prefill=pp, seq_lens_prefill=pre.seq_lens.to(d),
+                              cu_q_lens=pre.cu_q_lens.to(d), max_q_len=nq, out_prefill=out_p, q_decode=dec.q.to(d),
+                              block_table_decode=bt, page_logical_pos_decode=pp, seq_lens_decode=dec.seq_lens.to(d),
+                              out_decode=out_d, decode_sms=decode_sms)
+        torch.cuda.synchronize()
+        compare(out_p, ref_p, "fp8 mixed prefill, 8 kv heads")
+        compare(out_d, ref_d, "fp8 mixed decode, 8 kv heads")
+        assert np.array_equal(dev.k_pool.cpu().numpy(), pools.k_codes)       # read path is read-only
+    finally:
+        dev.close()
