@@ -109,7 +109,10 @@ typedef struct lazy_config {
  *                     quantises: scale = max|row| / 448 in fp32 (1 for an all-zero row), code = nearest E4M3 (ties
  *                     to even, saturating) of the fp32 quotient row[d] / scale.  The attention calls compute what the
  *                     bf16 calls would compute on the exactly dequantised pages (code value x scale).  Supported
- *                     with LAZY_ROPE_HALF_SPLIT and LAZY_K_UNROTATED; lazy_materialize_pages is bf16-only. */
+ *                     with LAZY_ROPE_HALF_SPLIT and LAZY_K_UNROTATED; lazy_materialize_pages is bf16-only.  head_dim 128
+ *                     runs on the product kernels (split-KV decode, tcgen05 prefill on CTA pairs, one-launch mixed
+ *                     step); head_dim 64 prefill on the one-CTA tcgen05 kernel, head_dim 64 decode on the row-wise
+ *                     CUDA kernel. */
 #define LAZY_KV_BF16      0
 #define LAZY_KV_FP8_E4M3  1
 
@@ -300,7 +303,8 @@ int lazy_host_step_packed(lazy_handle* h, const lazy_host_step_packed_args* a, v
  * For the product configuration (head_dim 128, un-rotated K, RoPE, 4 or 8 kv heads) the step is ONE launch: the first
  * `decode_sms` CTAs of the grid run the decode body, CTA pairs behind them the prefill work items (mixed_fused.cu);
  * decode_sms = 0 picks 7/16 of the SMs (64 of 148).  Bit 0 of `reserved0` forces the two-stream path described above
- * (the A/B arm); other configurations always take it. */
+ * (the A/B arm); other configurations always take it.  LAZY_KV_FP8_E4M3 pages have their own one-launch kernel under the
+ * same conditions (head_dim 128, 4 or 8 kv heads, no LAZY_FLAG_*). */
 typedef struct lazy_mixed_args {
   const void* q_prefill;  const int32_t* block_table_prefill;  const int32_t* page_logical_pos_prefill;
   const int32_t* seq_lens_prefill;  const int32_t* cu_q_lens;
