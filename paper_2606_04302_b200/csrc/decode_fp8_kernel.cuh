@@ -1,4 +1,4 @@
-// decode_fp8_kernel.cuh -- the split-KV decode CTA over LAZY_KV_FP8_E4M3 pages (head_dim 128, un-rotated K).
+// decode_fp8_kernel.cuh -- the split-KV decode CTA over LAZY_KV_FP8_E4M3 pages (head_dim 128 or 64, un-rotated K).
 //
 // Same decomposition, pipeline, rotation identity and in-kernel combine as decode_kernel.cuh (see decode_splitkv.cu);
 // what changes is the arithmetic type of a tile, chosen so that a tile of HALF the bytes does not cost MORE
@@ -26,15 +26,15 @@ namespace {
 
 // NCW consumer warps: 8 (the bf16 kernel's cut: 224 registers per consumer thread) or 12 (160 registers, which this
 // kernel fits: three dependent-chain warps per scheduler instead of two).  A CTA then holds NCW * 32 + 128 threads.
-template <int HKV_CTA, int NCW>
+template <int HKV_CTA, int NCW, int D_ = 128>
 struct DecodeFp8Cfg {
-  static constexpr int D = 128;
+  static constexpr int D = D_;                          // a row of codes is D bytes: 128-byte (D = 128) or 64-byte swizzle
   static constexpr int THREADS = NCW * 32 + 128;
   static constexpr int REGS_CONSUMER = NCW == 8 ? kRegsConsumer : 160;   // 384 * 160 + 128 * 32 = 65536
   static constexpr int REGS_PRODUCER = NCW == 8 ? kRegsProducer : 32;
   static constexpr int PPS = NCW / HKV_CTA;             // pages per pipeline stage
   static constexpr int BOX_ROWS = 16 * HKV_CTA;
-  static constexpr int PAGE_BYTES = BOX_ROWS * 128;     // K (or V) codes of one page, HKV_CTA heads: rows of 128 B
+  static constexpr int PAGE_BYTES = BOX_ROWS * D;       // K (or V) codes of one page, HKV_CTA heads: rows of D bytes
   static constexpr int CS_ROW_BYTES = D / 2 * 8;
   static constexpr int SC_BYTES = HKV_CTA * 64;         // K (or V) scales of one page, HKV_CTA heads
   static constexpr int OFF_V = PPS * PAGE_BYTES;
@@ -46,7 +46,7 @@ struct DecodeFp8Cfg {
   // 37 KB stages x 5 (8 warps) / 52-56 KB stages x 3 (12 warps); a 4th stage was measured: no gain (84.1 -> 85.4 us)
   static constexpr int NSTAGES = NCW == 8 ? 5 : 3;
   static constexpr int MAX_REQS = kMaxReqsSmem;         // requests per launch (smem prefix sums)
-  static constexpr int NL = 8;                          // words of 2 rotation pairs per thread per half
+  static constexpr int NL = D / 16;                     // words of 2 rotation pairs per thread per half
   static constexpr int NC = D / 16;
   static constexpr int OFF_CUM = NSTAGES * STAGE_BYTES;
   static constexpr int OFF_LEN = OFF_CUM + (MAX_REQS + 4) * 4;
@@ -77,11 +77,11 @@ __device__ __forceinline__ uint32_t h2mulsub(uint32_t a, uint32_t b, uint32_t c,
   return *reinterpret_cast<const uint32_t*>(&r);
 }
 
-template <int HKV_CTA, int NCW>
+template <int HKV_CTA, int NCW, int D_ = 128>
 __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const CUtensorMap& tmap_v,
                                                const DecodeFp8Args& fa, const int bid, const int G_in, const int hg,
                                                const int HG, unsigned char* smem_raw) {
-  using C = DecodeFp8Cfg<HKV_CTA, NCW>;
+  using C = DecodeFp8Cfg<HKV_CTA, NCW, D_>;
   constexpr int D = C::D;
   const DecodeArgs& a = fa.d;
   unsigned char* smem = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -250,8 +250,8 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
 #pragma unroll
       for (int h = 0; h < 2; ++h)
 #pragma unroll
-        for (int x = 0; x < 2; ++x) {
-          const uint4 v = qp[(h * (D / 2) + 16 * tq) / 8 + x];
+        for (int x = 0; x < D / 64; ++x) {
+          const uint4 v = qp[(h * (D / 2) + (D / 8) * tq) / 8 + x];
           const uint32_t ww[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
           for (int y = 0; y < 4; ++y) {
@@ -279,14 +279,22 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
       if (nv > 0) {
         const uint32_t st = smem_base + stage * C::STAGE_BYTES;
         const int delta = ptx::lds32(st + C::OFF_META + pl * 4);
-        // ---- K codes -> registers: 16 bytes per (half, token row): dims 64h + 16tq .. +15
-        uint4 kc[2][2];
+        // ---- K codes -> registers: D/8 bytes per (half, token row): dims (D/2)h + (D/8)tq .. (one 16-byte chunk of
+        // the 128B-swizzled row at D = 128, half a chunk of the 64B-swizzled row at D = 64)
+        uint32_t kc[2][2][C::NL / 2];
 #pragma unroll
         for (int h = 0; h < 2; ++h)
 #pragma unroll
           for (int rw = 0; rw < 2; ++rw) {
             const int Rr = hl * 16 + t0 + 2 * rw;
-            kc[h][rw] = ptx::lds128(st + pl * C::PAGE_BYTES + Rr * 128 + (((4 * h + tq) ^ (Rr & 7)) * 16));
+            if (D == 128) {
+              const uint4 v = ptx::lds128(st + pl * C::PAGE_BYTES + Rr * 128 + (((4 * h + tq) ^ (Rr & 7)) * 16));
+              kc[h][rw][0] = v.x; kc[h][rw][1] = v.y; kc[h][rw][C::NL / 2 - 2] = v.z; kc[h][rw][C::NL / 2 - 1] = v.w;
+            } else {
+              const int off = h * 32 + 8 * tq;
+              const uint2 v = ptx::lds64(st + pl * C::PAGE_BYTES + Rr * 64 + (((off >> 4) ^ ((Rr >> 1) & 3)) * 16) + (off & 15));
+              kc[h][rw][0] = v.x; kc[h][rw][1] = v.y;
+            }
           }
         // scales of this thread's two tokens: K (times log2(e)/sqrt(D)) and V
         const uint32_t sc_off = pl * C::SC_BYTES + (hl * 16 + t0) * 4;
@@ -314,8 +322,8 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
         uint32_t kreg[2][2][C::NL];
 #pragma unroll
         for (int rw = 0; rw < 2; ++rw) {
-          const uint32_t a1[4] = {kc[0][rw].x, kc[0][rw].y, kc[0][rw].z, kc[0][rw].w};
-          const uint32_t a2[4] = {kc[1][rw].x, kc[1][rw].y, kc[1][rw].z, kc[1][rw].w};
+          const uint32_t* a1 = kc[0][rw];
+          const uint32_t* a2 = kc[1][rw];
 #pragma unroll
           for (int w = 0; w < C::NL; ++w) {
             const uint32_t x1 = (w & 1) ? ptx::e4m3x2_hi_to_f16x2(a1[w >> 1]) : ptx::e4m3x2_lo_to_f16x2(a1[w >> 1]);
@@ -380,11 +388,11 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
           vmask = (vt < nv ? 0xffu : 0u) | (vt + 4 < nv ? 0xff00u : 0u) | (vt + 2 < nv ? 0xff0000u : 0u) |
                   (vt + 6 < nv ? 0xff000000u : 0u);
         }
-        const uint32_t vbase = st + C::OFF_V + pl * C::PAGE_BYTES + vrow * 128;
+        const uint32_t vbase = st + C::OFF_V + pl * C::PAGE_BYTES + vrow * D;
 #pragma unroll
         for (int i = 0; i < C::NC; i += 2) {
           uint32_t r0, r1, r2, r3;
-          ptx::ldmatrix_b8_x2_trans(r0, r1, r2, r3, vbase + ((((i + vmat)) ^ (vrow & 7)) * 16));
+          ptx::ldmatrix_b8_x2_trans(r0, r1, r2, r3, vbase + (((i + vmat) ^ (D == 128 ? (vrow & 7) : ((vrow >> 1) & 3))) * 16));
           if (nv < kPageSize) { r0 &= vmask; r1 &= vmask; r2 &= vmask; r3 &= vmask; }
           ptx::mma_f16_16816(oacc[i], ptx::e4m3x2_lo_to_f16x2(r0), ptx::e4m3x2_lo_to_f16x2(r1),
                              ptx::e4m3x2_hi_to_f16x2(r0), ptx::e4m3x2_hi_to_f16x2(r1), pb0, pb1);

@@ -38,12 +38,12 @@ decode_splitkv_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_c
 }
 
 // LAZY_KV_FP8_E4M3 pages (decode_fp8_kernel.cuh), head_dim 128
-template <int HKV_CTA, int NCW>
+template <int HKV_CTA, int NCW, int D>
 __global__ void __launch_bounds__(NCW * 32 + 128, 1)
 decode_fp8_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
                   const DecodeFp8Args a) {
   extern __shared__ unsigned char smem_raw[];
-  decode_fp8_cta<HKV_CTA, NCW>(tmap_k, tmap_v, a, (int)blockIdx.x, (int)gridDim.x, (int)blockIdx.y, (int)gridDim.y, smem_raw);
+  decode_fp8_cta<HKV_CTA, NCW, D>(tmap_k, tmap_v, a, (int)blockIdx.x, (int)gridDim.x, (int)blockIdx.y, (int)gridDim.y, smem_raw);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -134,16 +134,22 @@ static int launch_decode_t(lazy_handle* h, const DecodeArgs& args, int grid_x, i
   }
 }
 
-template <int HKV_CTA, int NCW>
-static int launch_decode_fp8_t(lazy_handle* h, const DecodeFp8Args& args, int grid_x, int grid_y, cudaStream_t stream) {
-  using C = DecodeFp8Cfg<HKV_CTA, NCW>;
-  auto kern = decode_fp8_kernel<HKV_CTA, NCW>;
+template <int HKV_CTA, int NCW, int D>
+static int launch_decode_fp8_d(lazy_handle* h, const DecodeFp8Args& args, int grid_x, int grid_y, cudaStream_t stream) {
+  using C = DecodeFp8Cfg<HKV_CTA, NCW, D>;
+  auto kern = decode_fp8_kernel<HKV_CTA, NCW, D>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
     return LAZY_ERR_CUDA;
   const CUtensorMap* mk = reinterpret_cast<const CUtensorMap*>(h->tmap_k);
   const CUtensorMap* mv = reinterpret_cast<const CUtensorMap*>(h->tmap_v);
   kern<<<dim3(grid_x, grid_y), C::THREADS, C::SMEM_BYTES, stream>>>(*mk, *mv, args);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
+}
+
+template <int HKV_CTA, int NCW>
+static int launch_decode_fp8_t(lazy_handle* h, const DecodeFp8Args& args, int grid_x, int grid_y, cudaStream_t stream) {
+  return h->cfg.head_dim == 128 ? launch_decode_fp8_d<HKV_CTA, NCW, 128>(h, args, grid_x, grid_y, stream)
+                                : launch_decode_fp8_d<HKV_CTA, NCW, 64>(h, args, grid_x, grid_y, stream);
 }
 
 int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
@@ -157,7 +163,6 @@ int launch_decode(lazy_handle* h, const void* q, const void* k_cache, const void
   const int hkv_cta = w12 ? (c.num_kv_heads >= 4 ? 4 : c.num_kv_heads) : (c.num_kv_heads >= 8 ? 8 : c.num_kv_heads);
   const int HG = c.num_kv_heads / hkv_cta;
   const long long rows = (long long)c.num_pages * c.num_kv_heads * kPageSize;
-  if (fp8 && c.head_dim != 128) return LAZY_ERR_UNSUPPORTED;   // the caller routes head_dim 64 to the row-wise kernel
   if (h->tmap_k_ptr != k_cache) {
     if (!(fp8 ? encode_pool_tmap_u8(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta, true, c.head_dim)
               : encode_pool_tmap(h->tmap_k, k_cache, rows, c.head_dim, 16 * hkv_cta)))

@@ -254,8 +254,7 @@ int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const v
   if (num_reqs == 0) return LAZY_OK;
   cudaStream_t s = static_cast<cudaStream_t>(stream);
   int n;
-  // FP8 pages at head_dim 64 have no split-KV kernel: they run on the row-wise CUDA kernel
-  if ((h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS) || (h->cfg.dtype == LAZY_KV_FP8_E4M3 && h->cfg.head_dim != 128))
+  if (h->cfg.flags & LAZY_FLAG_ROWWISE_KERNELS)
     n = lazy::launch_rowwise(h, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, nullptr,
                              num_reqs, num_reqs, 1, out, s);
   else

@@ -162,11 +162,13 @@ from test_gpu_edges import _custom, SH128, SH64, SH7   # noqa: E402
 SH2 = W.LazyShape(8, 2, 128, 1.0e4)      # 2 kv heads: 6 pages per stage in the 12-warp cut
 SH1 = W.LazyShape(8, 1, 128, 1.0e4)      # 1 kv head: 12 pages per stage
 SH16 = W.LazyShape(32, 16, 128, 5.0e5)   # 16 kv heads: 4 head groups (grid.y = 4)
+SH64B = W.LazyShape(32, 8, 64, 1.0e4)    # head_dim 64 with 8 kv heads (64-byte swizzled rows, two head groups)
 DFLAGS = [pytest.param(0, id="w12"), pytest.param(B.LAZY_FLAG_FP8_DECODE_8_WARPS, id="w8")]
 
 
 @pytest.mark.parametrize("flags", DFLAGS)
-@pytest.mark.parametrize("shape", [SH128, SH7, SH2, SH1, SH16, SH64], ids=["g4", "g7", "hkv2", "hkv1", "hkv16", "d64"])
+@pytest.mark.parametrize("shape", [SH128, SH7, SH2, SH1, SH16, SH64, SH64B],
+                         ids=["g4", "g7", "hkv2", "hkv1", "hkv16", "d64", "d64hkv8"])
 def test_fp8_ragged_decode(shape, flags):
     seq = [1, 2, 15, 16, 17, 31, 33, 100, 257, 640, 1000, 3]
     _run(_custom(shape, seq, [1] * len(seq), seed=21, kind="decode"), flags=flags)
