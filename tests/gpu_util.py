@@ -69,7 +69,7 @@ def run_and_compare(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, 
 
 
 def run_and_compare_fp8(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, scale_abs_by_output: bool = False,
-                        gates=None, dev_kw=None):
+                        gates=None, dev_kw=None, oracle_kw=None):
     """FP8 KV pages (LAZY_KV_FP8_E4M3): the library quantises (lazy_cache_write), the oracle quantises its own copy;
     codes and scales must agree BIT FOR BIT after every step (integer decisions taken in fp32 on both sides), and the
     attention outputs must match the oracle's exact-dequantisation result under the same gates as the bf16 path."""
@@ -99,7 +99,7 @@ def run_and_compare_fp8(batch, flags: int = 0, sample_rows: int = 0, seed: int =
                 rows = np.sort(rng.choice(step.q.shape[0], size=sample_rows, replace=False))
                 sel = np.zeros(step.q.shape[0], dtype=np.uint8)
                 sel[rows] = 1
-            ref = O.run_step_fp8(batch, step, pools, row_select=sel)
+            ref = O.run_step_fp8(batch, step, pools, row_select=sel, **(oracle_kw or {}))
             check_pools(si)
             if got is not None:
                 sc = max(1.0, float(np.abs(ref).max())) if scale_abs_by_output else 1.0

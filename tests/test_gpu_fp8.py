@@ -251,3 +251,16 @@ def test_fp8_mixed_one_launch_8_kv_heads(decode_sms):
         assert np.array_equal(dev.k_pool.cpu().numpy(), pools.k_codes)       # read path is read-only
     finally:
         dev.close()
+
+
+@pytest.mark.parametrize("cfg,scale", [(1, None), (2, 0.1), (3, 0.05), (5, 0.2)])
+def test_fp8_scaled_frequencies_and_temperature(cfg, scale):
+    """Frequency-scaled RoPE (Llama-3.1 style per-pair frequencies, lazy_set_rope_frequencies) and a softmax temperature on
+    FP8 pages: every FP8 kernel reads its angles through the rebuilt table and its scale from the handle."""
+    import math
+    from test_gpu_posvariants import _llama31_style
+    batch = W.CONFIGS[cfg]() if scale is None else W.CONFIGS[cfg](scale=scale)
+    sh = batch.shape
+    f = _llama31_style(sh.rope_theta, sh.head_dim)
+    temp = 1.1 / math.sqrt(sh.head_dim)
+    _run(batch, dev_kw=dict(inv_freq=f, softmax_scale=temp), oracle_kw=dict(inv_freq=f, scale=temp))
