@@ -109,7 +109,7 @@ typedef struct lazy_config {
  *                     quantises: scale = max|row| / 448 in fp32 (1 for an all-zero row), code = nearest E4M3 (ties
  *                     to even, saturating) of the fp32 quotient row[d] / scale.  The attention calls compute what the
  *                     bf16 calls would compute on the exactly dequantised pages (code value x scale).  Supported
- *                     with LAZY_ROPE_HALF_SPLIT and LAZY_K_UNROTATED; lazy_materialize_pages is bf16-only.  Every call
+ *                     with both RoPE pairings (not ALiBi) and LAZY_K_UNROTATED; lazy_materialize_pages is bf16-only.  Every call
  *                     runs on the product kernels at either head_dim (split-KV decode; tcgen05 prefill, on CTA pairs
  *                     at head_dim 128; the one-launch mixed step at head_dim 128). */
 #define LAZY_KV_BF16      0

@@ -247,18 +247,34 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
       for (int w = 0; w < C::NL; ++w) { qf[h][w][0] = 0.f; qf[h][w][1] = 0.f; }
     if (g < group) {
       const uint4* qp = reinterpret_cast<const uint4*>(a.q + ((size_t)r * sh.Hq + hk * group + g) * D);
+      if (!a.q_interleaved) {
 #pragma unroll
-      for (int h = 0; h < 2; ++h)
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+          for (int x = 0; x < D / 64; ++x) {
+            const uint4 v = qp[(h * (D / 2) + (D / 8) * tq) / 8 + x];
+            const uint32_t ww[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int y = 0; y < 4; ++y) {
+              qf[h][4 * x + y][0] = ptx::bf16_lo(ww[y]);
+              qf[h][4 * x + y][1] = ptx::bf16_hi(ww[y]);
+            }
+          }
+      } else {
+        // LAZY_ROPE_INTERLEAVED: model order (x1_j, x2_j) per word -> this thread's x1 and x2 values of pairs
+        // j = (D/8) tq + 8x .. + 7 (two 16-byte loads hold 8 pairs)
 #pragma unroll
         for (int x = 0; x < D / 64; ++x) {
-          const uint4 v = qp[(h * (D / 2) + (D / 8) * tq) / 8 + x];
-          const uint32_t ww[4] = {v.x, v.y, v.z, v.w};
+          const int j0 = (D / 8) * tq + 8 * x;
+          const uint4 s0 = qp[j0 / 4], s1 = qp[j0 / 4 + 1];
+          const uint32_t sw[8] = {s0.x, s0.y, s0.z, s0.w, s1.x, s1.y, s1.z, s1.w};
 #pragma unroll
-          for (int y = 0; y < 4; ++y) {
-            qf[h][4 * x + y][0] = ptx::bf16_lo(ww[y]);
-            qf[h][4 * x + y][1] = ptx::bf16_hi(ww[y]);
+          for (int wi = 0; wi < 4; ++wi) {
+            qf[0][4 * x + wi][0] = ptx::bf16_lo(sw[2 * wi]);     qf[1][4 * x + wi][0] = ptx::bf16_hi(sw[2 * wi]);
+            qf[0][4 * x + wi][1] = ptx::bf16_lo(sw[2 * wi + 1]); qf[1][4 * x + wi][1] = ptx::bf16_hi(sw[2 * wi + 1]);
           }
         }
+      }
     }
     uint32_t qhat[2][C::NL];
 

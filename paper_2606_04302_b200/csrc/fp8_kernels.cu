@@ -26,7 +26,7 @@ __device__ __forceinline__ float e4m3_to_float(uint8_t c) {
 template <int D>
 __global__ void __launch_bounds__(256)
 cache_write_fp8_kernel(const __nv_bfloat16* __restrict__ k_new, const __nv_bfloat16* __restrict__ v_new,
-                       const long long* __restrict__ slot_mapping, long long num_rows, int Hkv,
+                       const long long* __restrict__ slot_mapping, long long num_rows, int Hkv, int deinterleave,
                        uint8_t* __restrict__ k_codes, uint8_t* __restrict__ v_codes, float* __restrict__ k_scale,
                        float* __restrict__ v_scale) {
   constexpr int PER = D / 32;                       // elements per lane: 4 (D = 128) or 2 (D = 64)
@@ -43,7 +43,16 @@ cache_write_fp8_kernel(const __nv_bfloat16* __restrict__ k_new, const __nv_bfloa
   const int off = (int)(slot % kPageSize);
   const __nv_bfloat16* src = (which ? v_new : k_new) + (tok * Hkv + head) * D + lane * PER;
   float x[PER];
-  if (PER == 4) {
+  if (deinterleave && which == 0) {
+    // LAZY_ROPE_INTERLEAVED: stored dim d' < D/2 is model dim 2d', stored dim D/2 + d' is model dim 2d' + 1 (the row's
+    // values, hence its scale, are the same set: still position-free)
+    const __nv_bfloat16* rowp = k_new + (tok * Hkv + head) * D;
+#pragma unroll
+    for (int i = 0; i < PER; ++i) {
+      const int d = lane * PER + i;
+      x[i] = __bfloat162float(rowp[d < D / 2 ? 2 * d : 2 * (d - D / 2) + 1]);
+    }
+  } else if (PER == 4) {
     const uint2 v = *reinterpret_cast<const uint2*>(src);
     x[0] = ptx::bf16_lo(v.x); x[1] = ptx::bf16_hi(v.x); x[PER - 2] = ptx::bf16_lo(v.y); x[PER - 1] = ptx::bf16_hi(v.y);
   } else {
@@ -78,7 +87,7 @@ rowwise_attn_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __re
                         const float* __restrict__ v_scale, const int* __restrict__ block_table,
                         const int* __restrict__ page_pos, const int* __restrict__ seq_lens,
                         const int* __restrict__ cu_q_lens, int num_reqs, Shape sh, const float2* __restrict__ cs,
-                        __nv_bfloat16* __restrict__ out) {
+                        int q_interleaved, __nv_bfloat16* __restrict__ out) {
   constexpr int HALF = D / 2;
   constexpr int PER = D / 64;
   const int row = blockIdx.x;
@@ -109,7 +118,8 @@ rowwise_attn_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __re
 #pragma unroll
     for (int e = 0; e < PER; ++e) {
       int j = lane * PER + e;
-      float a = __bfloat162float(qp[j]), b = __bfloat162float(qp[j + HALF]);
+      float a = __bfloat162float(qp[q_interleaved ? 2 * j : j]);
+      float b = __bfloat162float(qp[q_interleaved ? 2 * j + 1 : j + HALF]);
       float2 t = cs_load(cs + (size_t)pos_q * HALF, j, D);
       q1[e] = (a * t.x - b * t.y) * sh.scale_log2;
       q2[e] = (a * t.y + b * t.x) * sh.scale_log2;
@@ -174,11 +184,12 @@ int launch_cache_write_fp8(lazy_handle* h, const void* k_new, const void* v_new,
   auto sm = reinterpret_cast<const long long*>(slot_mapping);
   auto kc = static_cast<uint8_t*>(k_cache);
   auto vc = static_cast<uint8_t*>(v_cache);
+  const int deint = h->cfg.rope_style == LAZY_ROPE_INTERLEAVED;
   if (h->cfg.head_dim == 128)
-    cache_write_fp8_kernel<128><<<(unsigned)blocks, threads, 0, stream>>>(kn, vn, sm, rows, h->cfg.num_kv_heads, kc, vc,
+    cache_write_fp8_kernel<128><<<(unsigned)blocks, threads, 0, stream>>>(kn, vn, sm, rows, h->cfg.num_kv_heads, deint, kc, vc,
                                                                           h->k_scale, h->v_scale);
   else
-    cache_write_fp8_kernel<64><<<(unsigned)blocks, threads, 0, stream>>>(kn, vn, sm, rows, h->cfg.num_kv_heads, kc, vc,
+    cache_write_fp8_kernel<64><<<(unsigned)blocks, threads, 0, stream>>>(kn, vn, sm, rows, h->cfg.num_kv_heads, deint, kc, vc,
                                                                          h->k_scale, h->v_scale);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
@@ -194,11 +205,11 @@ int launch_rowwise_fp8(lazy_handle* h, const void* q, const void* k_cache, const
   if (h->cfg.head_dim == 128)
     rowwise_attn_fp8_kernel<128><<<grid, 128, 0, stream>>>(qp, kp, vp, h->k_scale, h->v_scale, block_table,
                                                            page_logical_pos, seq_lens, cu_q_lens, num_reqs, h->shape,
-                                                           h->ws.cs, op);
+                                                           h->ws.cs, h->cfg.rope_style == LAZY_ROPE_INTERLEAVED, op);
   else
     rowwise_attn_fp8_kernel<64><<<grid, 128, 0, stream>>>(qp, kp, vp, h->k_scale, h->v_scale, block_table,
                                                           page_logical_pos, seq_lens, cu_q_lens, num_reqs, h->shape,
-                                                          h->ws.cs, op);
+                                                          h->ws.cs, h->cfg.rope_style == LAZY_ROPE_INTERLEAVED, op);
   return cudaGetLastError() == cudaSuccess ? 1 : LAZY_ERR_CUDA;
 }
 

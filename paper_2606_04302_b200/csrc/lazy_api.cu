@@ -21,7 +21,7 @@ bool config_supported(const lazy_config* c) {
   int hkv = c->num_kv_heads;
   if (!(hkv == 1 || hkv == 2 || hkv == 4 || hkv % 8 == 0)) return false;
   if (c->dtype != LAZY_KV_BF16 && c->dtype != LAZY_KV_FP8_E4M3) return false;
-  if (c->dtype == LAZY_KV_FP8_E4M3 && (c->rope_style != LAZY_ROPE_HALF_SPLIT || c->k_storage != LAZY_K_UNROTATED))
+  if (c->dtype == LAZY_KV_FP8_E4M3 && (c->rope_style == LAZY_POS_ALIBI || c->k_storage != LAZY_K_UNROTATED))
     return false;
   if (c->rope_style < LAZY_ROPE_HALF_SPLIT || c->rope_style > LAZY_POS_ALIBI) return false;
   if (c->rope_style == LAZY_POS_ALIBI && (c->k_storage != LAZY_K_UNROTATED || c->num_q_heads > lazy::kMaxAlibiHeads))

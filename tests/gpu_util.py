@@ -69,7 +69,7 @@ def run_and_compare(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, 
 
 
 def run_and_compare_fp8(batch, flags: int = 0, sample_rows: int = 0, seed: int = 0, scale_abs_by_output: bool = False,
-                        gates=None, dev_kw=None, oracle_kw=None):
+                        gates=None, dev_kw=None, oracle_kw=None, k_perm=None):
     """FP8 KV pages (LAZY_KV_FP8_E4M3): the library quantises (lazy_cache_write), the oracle quantises its own copy;
     codes and scales must agree BIT FOR BIT after every step (integer decisions taken in fp32 on both sides), and the
     attention outputs must match the oracle's exact-dequantisation result under the same gates as the bf16 path."""
@@ -86,7 +86,8 @@ def run_and_compare_fp8(batch, flags: int = 0, sample_rows: int = 0, seed: int =
         assert np.array_equal(np.isnan(dev.k_scale.cpu().numpy()), ~valid), f"step {si}: which rows are written"
         assert np.array_equal(ks[valid], pools.k_scale.view(np.uint32)[valid]), f"step {si}: K scales"
         assert np.array_equal(vs[valid], pools.v_scale.view(np.uint32)[valid]), f"step {si}: V scales"
-        assert np.array_equal(kc, pools.k_codes), f"step {si}: K codes"
+        # k_perm: order in which the library stores K's last axis (LAZY_ROPE_INTERLEAVED de-interleaves on write)
+        assert np.array_equal(kc, pools.k_codes if k_perm is None else pools.k_codes[..., k_perm]), f"step {si}: K codes"
         assert np.array_equal(vc, pools.v_codes), f"step {si}: V codes"
 
     try:

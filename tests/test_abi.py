@@ -58,7 +58,8 @@ def test_workspace_bytes(lib):
     assert B.lazy_workspace_bytes(_cfg(dtype=2)) == 0
     assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3)) >= n          # FP8 pages: more split-KV partial slots
     assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3, k_storage=1)) == 0
-    assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3, rope_style=2)) == 0
+    assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3, rope_style=2)) == 0          # no ALiBi on FP8 pages
+    assert B.lazy_workspace_bytes(_cfg(dtype=B.LAZY_KV_FP8_E4M3, rope_style=1)) > 0
 
 
 def test_create_rejects_without_touching_the_gpu(lib):

@@ -264,3 +264,14 @@ def test_fp8_scaled_frequencies_and_temperature(cfg, scale):
     f = _llama31_style(sh.rope_theta, sh.head_dim)
     temp = 1.1 / math.sqrt(sh.head_dim)
     _run(batch, dev_kw=dict(inv_freq=f, softmax_scale=temp), oracle_kw=dict(inv_freq=f, scale=temp))
+
+
+@pytest.mark.parametrize("flags", [pytest.param(0, id="prod"), pytest.param(B.LAZY_FLAG_ROWWISE_KERNELS, id="rowwise")])
+@pytest.mark.parametrize("cfg,scale", [(1, None), (2, 0.1), (3, 0.05), (5, 0.2)])
+def test_fp8_interleaved_pairing(cfg, scale, flags):
+    """LAZY_ROPE_INTERLEAVED on FP8 pages: lazy_cache_write de-interleaves the K row before quantising it (same values,
+    same scale, codes in the stored order), the kernels de-interleave q on load."""
+    batch = W.CONFIGS[cfg]() if scale is None else W.CONFIGS[cfg](scale=scale)
+    D = batch.shape.head_dim
+    perm = np.concatenate([np.arange(0, D, 2), np.arange(1, D, 2)])
+    _run(batch, flags=flags, dev_kw=dict(rope_style=B.LAZY_ROPE_INTERLEAVED), oracle_kw=dict(rope_style=1), k_perm=perm)
