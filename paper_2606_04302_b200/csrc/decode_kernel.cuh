@@ -91,7 +91,7 @@ __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r
       const int n = min(cap, n_slots - base);
       if (warp == 0) {
         if (lane == 0) {
-          ptx::fence_proxy_async();                 // the partials were written through the generic proxy
+          ptx::fence_proxy_async_all();             // the partials were written through the generic proxy
           ptx::mbar_arrive_expect_tx(cbar, (uint32_t)(n * slot_bytes));
         }
         __syncwarp();
