@@ -232,6 +232,29 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
   const int vtok = 8 * ((lane >> 3) & 1) + 4 * (lane & 1) + 2 * ((lane >> 1) & 1) + ((lane >> 2) & 1);
   const int vrow = hl * 16 + vtok;
   const int vmat = lane >> 4;                       // which of the two 16-dim tiles of an x2 load this lane addresses
+  // Per-thread byte offsets inside a stage, fixed for the whole kernel.  They are laundered through an empty asm so
+  // that the compiler keeps them in registers: at 160 registers per thread it otherwise re-derives them from the lane
+  // id for every tile (~60 integer instructions of the ~390 a tile costs).
+  uint32_t kofs[2][2], vofs[C::NC / 2], scofs;
+#pragma unroll
+  for (int h = 0; h < 2; ++h)
+#pragma unroll
+    for (int rw = 0; rw < 2; ++rw) {
+      const int Rr = hl * 16 + t0 + 2 * rw;
+      if (D == 128) kofs[h][rw] = pl * C::PAGE_BYTES + Rr * 128 + (((4 * h + tq) ^ (Rr & 7)) * 16);
+      else {
+        const int off = h * 32 + 8 * tq;
+        kofs[h][rw] = pl * C::PAGE_BYTES + Rr * 64 + (((off >> 4) ^ ((Rr >> 1) & 3)) * 16) + (off & 15);
+      }
+      asm volatile("" : "+r"(kofs[h][rw]));
+    }
+#pragma unroll
+  for (int i = 0; i < C::NC; i += 2) {
+    vofs[i / 2] = C::OFF_V + pl * C::PAGE_BYTES + vrow * D + (((i + vmat) ^ (D == 128 ? (vrow & 7) : ((vrow >> 1) & 3))) * 16);
+    asm volatile("" : "+r"(vofs[i / 2]));
+  }
+  scofs = pl * C::SC_BYTES + (hl * 16 + t0) * 4;
+  asm volatile("" : "+r"(scofs));
 
   int r = r0, u = u_begin, it = 0;
   while (u < u_end) {
@@ -302,18 +325,16 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
         for (int h = 0; h < 2; ++h)
 #pragma unroll
           for (int rw = 0; rw < 2; ++rw) {
-            const int Rr = hl * 16 + t0 + 2 * rw;
             if (D == 128) {
-              const uint4 v = ptx::lds128(st + pl * C::PAGE_BYTES + Rr * 128 + (((4 * h + tq) ^ (Rr & 7)) * 16));
+              const uint4 v = ptx::lds128(st + kofs[h][rw]);
               kc[h][rw][0] = v.x; kc[h][rw][1] = v.y; kc[h][rw][C::NL / 2 - 2] = v.z; kc[h][rw][C::NL / 2 - 1] = v.w;
             } else {
-              const int off = h * 32 + 8 * tq;
-              const uint2 v = ptx::lds64(st + pl * C::PAGE_BYTES + Rr * 64 + (((off >> 4) ^ ((Rr >> 1) & 3)) * 16) + (off & 15));
+              const uint2 v = ptx::lds64(st + kofs[h][rw]);
               kc[h][rw][0] = v.x; kc[h][rw][1] = v.y;
             }
           }
         // scales of this thread's two tokens: K (times log2(e)/sqrt(D)) and V
-        const uint32_t sc_off = pl * C::SC_BYTES + (hl * 16 + t0) * 4;
+        const uint32_t sc_off = scofs;
         const float sk0 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off)) * sh.scale_log2;
         const float sk1 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off + 8)) * sh.scale_log2;
         float sv0 = __int_as_float(ptx::lds32(st + C::OFF_SV + sc_off));
@@ -399,16 +420,15 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
         // ---- O^T += V^T P'  (a7): 8-bit transposing ldmatrix, two 16-dim tiles per load; byte b of a register is
         // token tau(4tq + b) = vt + 4(b&1) + 2(b>>1) -- bytes past the tail are cleared (their codes may be NaN)
         uint32_t vmask = 0xffffffffu;
-        if (nv < kPageSize) {
+        if (nv < kPageSize) {                       // the last page of a request only
           const int vt = 8 * (tq >> 1) + (tq & 1);
           vmask = (vt < nv ? 0xffu : 0u) | (vt + 4 < nv ? 0xff00u : 0u) | (vt + 2 < nv ? 0xff0000u : 0u) |
                   (vt + 6 < nv ? 0xff000000u : 0u);
         }
-        const uint32_t vbase = st + C::OFF_V + pl * C::PAGE_BYTES + vrow * D;
 #pragma unroll
         for (int i = 0; i < C::NC; i += 2) {
           uint32_t r0, r1, r2, r3;
-          ptx::ldmatrix_b8_x2_trans(r0, r1, r2, r3, vbase + (((i + vmat) ^ (D == 128 ? (vrow & 7) : ((vrow >> 1) & 3))) * 16));
+          ptx::ldmatrix_b8_x2_trans(r0, r1, r2, r3, st + vofs[i / 2]);
           if (nv < kPageSize) { r0 &= vmask; r1 &= vmask; r2 &= vmask; r3 &= vmask; }
           ptx::mma_f16_16816(oacc[i], ptx::e4m3x2_lo_to_f16x2(r0), ptx::e4m3x2_lo_to_f16x2(r1),
                              ptx::e4m3x2_hi_to_f16x2(r0), ptx::e4m3x2_hi_to_f16x2(r1), pb0, pb1);
