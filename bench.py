@@ -622,6 +622,13 @@ def prefill_leg(workload, device, steps, peaks, barrier, sustained_s=2.0):
     return res
 
 
+def _cache_write_entry(_batch, tokens, sh, fp8, ms):
+    rd = tokens * sh.num_kv_heads * sh.head_dim * 2 * 2                      # bf16 K and V rows in
+    wr = tokens * sh.num_kv_heads * (2 * (sh.head_dim + 4) if fp8 else sh.head_dim * 2 * 2)   # pages (+ scales) out
+    return {"bound": "hbm", "tokens": tokens, "bytes": rd + wr, "ms": ms, "GBps": (rd + wr) / (ms * 1e-3) / 1e9,
+            "note": "two launches (prefill tokens, decode tokens): launch-latency-bound at this size"}
+
+
 def cfg5_leg(device, steps, peaks, job=None, fp8=False):
     """configs[4], kernel by kernel (separate calls, L2 flushed before each): the block-local prefill of the 4 miss
     documents (tensor roofline; 464 one-CTA work items = 232 CTA pairs on 74 SM pairs, causal: 1..8 KV tiles per pair)
@@ -630,6 +637,7 @@ def cfg5_leg(device, steps, peaks, job=None, fp8=False):
     if own:
         b, job, _ = _timed_job("cfg5", device, steps, fp8=fp8)
     per = job.time_calls(steps, 3)
+    job_timed_tokens = int(sum(r["k_new"].shape[0] for r in job.timed))
     works = {r["step"].kind: step_work(job.batch, [r["step"]], fp8=fp8) for r in job.timed}
     t_ms, a_ms, _ = job.time_steps(steps, 3, lambda: None)
     if own:
@@ -661,7 +669,11 @@ def cfg5_leg(device, steps, peaks, job=None, fp8=False):
             "decode_shared": {"kernel_ms": per["decode"], "logical_GBps": gb_sh,
                               "logical_over_hbm_peak": gb_sh / peaks["hbm"]},
             "mixed_step_ms": t_ms / steps, "mixed_attention_ms": a_ms / steps,
-            "separate_kernels_sum_ms": per["prefill"] + per["decode"]}
+            "separate_kernels_sum_ms": per["prefill"] + per["decode"],
+            # row a0 (HBM-bound, 2*Hkv*D*2 B read + the same written per token): the step's two
+            # lazy_cache_write launches = step time - attention time; a few MB, i.e. launch-latency-bound
+            "cache_write": _cache_write_entry(job.batch if not own else None, job_timed_tokens, sh, fp8,
+                                              (t_ms - a_ms) / steps)}
 
 
 def main():
