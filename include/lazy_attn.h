@@ -128,6 +128,7 @@ typedef struct lazy_config {
 #define LAZY_ERR_UNSUPPORTED -2  /* head_dim, page_size, head grouping, dtype or rope_style not supported  */
 #define LAZY_ERR_WORKSPACE   -3  /* workspace too small or misaligned                                      */
 #define LAZY_ERR_CUDA        -4  /* CUDA error at launch (cudaGetLastError)                                */
+#define LAZY_ERR_STATIC_LIMIT -5 /* lazy_attn_decode_static: cfg needs more scratch than LAZY_STATIC_SCRATCH_BYTES */
 
 /* Bytes of device workspace lazy_create needs for `cfg` (RoPE cos/sin table built from fp64 angles --
  * PAPER.md L138/L173 "loaded from a table", L455 stateless absolute-index rotation -- plus split-KV
@@ -173,6 +174,30 @@ int lazy_attn_prefill(lazy_handle* h, const void* q, const void* k_cache, const 
 int lazy_attn_decode(lazy_handle* h, const void* q, const void* k_cache, const void* v_cache,
                      const int32_t* block_table, const int32_t* page_logical_pos,
                      const int32_t* seq_lens, int32_t num_reqs, void* out, void* stream);
+
+/* Decode WITHOUT a caller-provided workspace, for callers that cannot allocate device memory: code that runs inside
+ * a host framework which owns all device memory and forbids raw cudaMalloc, serving loops where cudaMalloc is banned
+ * because it synchronises the device, components that only ever see the input and output buffers of one call.  Same
+ * computation, same kernel and same results as lazy_create + lazy_attn_decode with `cfg`; the scratch that call keeps
+ * in the workspace (cos/sin table, split-KV partials, arrival counters) lives in a device array that is part of the
+ * library image: LAZY_STATIC_SCRATCH_BYTES per GPU that loads it, held until the process exits.  The call and
+ * everything under it use no cudaMalloc / cudaFree / allocating library routine.
+ *   cfg   : HOST pointer.  bf16 pages, LAZY_K_UNROTATED, a RoPE pairing (not ALiBi), flags == 0, otherwise
+ *           LAZY_ERR_UNSUPPORTED.  lazy_workspace_bytes(cfg) must be <= LAZY_STATIC_SCRATCH_BYTES, otherwise
+ *           LAZY_ERR_STATIC_LIMIT and nothing is enqueued (at Hq 32 / Hkv 8 / D 128 / 64 requests the limit is reached
+ *           near max_position = 60000; lower max_position or max_reqs to fit).
+ *   other arguments: as lazy_attn_decode.  num_reqs <= cfg->max_reqs.
+ * Set-up: the FIRST call on a device, and any call whose cfg differs from the previous call's on that device, also
+ * looks up the array's device address, clears the counters and enqueues the table build (one extra launch) on
+ * `stream` ahead of the decode kernel; later calls with the same cfg enqueue one small memset and the kernel.  Make
+ * that first call during start-up, before any stream capture is begun.
+ * Sharing: there is ONE array per GPU and every call on that GPU uses it.  Two calls whose GPU work may overlap
+ * (different streams without an event between them, or different host threads racing to enqueue) corrupt each other's
+ * partials -- keep all calls on one stream or order them yourself.  Host-side the call is thread-safe. */
+#define LAZY_STATIC_SCRATCH_BYTES (48u << 20)
+int lazy_attn_decode_static(const lazy_config* cfg, const void* q, const void* k_cache, const void* v_cache,
+                            const int32_t* block_table, const int32_t* page_logical_pos,
+                            const int32_t* seq_lens, int32_t num_reqs, void* out, void* stream);
 
 /* f3. Frequency-scaled RoPE families (Llama-3.1 / NTK / YaRN scaling only change "variant-specific
  * scaling metadata").  Replaces the rotation frequency of pair j, theta_j = rope_theta^(-2j/D), by inv_freq[j]

@@ -14,6 +14,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "liblazyattn.so")
 
 LAZY_OK, LAZY_ERR_INVALID, LAZY_ERR_UNSUPPORTED, LAZY_ERR_WORKSPACE, LAZY_ERR_CUDA = 0, -1, -2, -3, -4
+LAZY_ERR_STATIC_LIMIT = -5
+LAZY_STATIC_SCRATCH_BYTES = 48 << 20
 LAZY_FLAG_ROWWISE_KERNELS = 1
 LAZY_FLAG_PREFILL_ONE_CTA = 2
 LAZY_FLAG_FP8_DECODE_8_WARPS = 4
@@ -22,7 +24,7 @@ LAZY_ROPE_HALF_SPLIT, LAZY_ROPE_INTERLEAVED, LAZY_POS_ALIBI = 0, 1, 2
 LAZY_KV_BF16, LAZY_KV_FP8_E4M3 = 0, 1
 
 EXPORTS = ["lazy_workspace_bytes", "lazy_create", "lazy_destroy", "lazy_cache_write", "lazy_attn_prefill",
-           "lazy_attn_decode", "lazy_set_rope_frequencies", "lazy_set_alibi_slopes", "lazy_set_page_stored_pos",
+           "lazy_attn_decode", "lazy_attn_decode_static", "lazy_set_rope_frequencies", "lazy_set_alibi_slopes", "lazy_set_page_stored_pos",
            "lazy_set_kv_scales",
            "lazy_materialize_pages", "lazy_status_string", "lazy_launch_count", "lazy_host_step_staging_bytes", "lazy_host_step", "lazy_host_step_layout", "lazy_host_step_packed",
            "lazy_attn_mixed", "lazy_debug_validate",
@@ -63,6 +65,8 @@ def lib() -> ctypes.CDLL:
         L.lazy_attn_prefill.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp, vp]
         L.lazy_attn_decode.restype = ctypes.c_int
         L.lazy_attn_decode.argtypes = [vp, vp, vp, vp, vp, vp, vp, i32, vp, vp]
+        L.lazy_attn_decode_static.restype = ctypes.c_int
+        L.lazy_attn_decode_static.argtypes = [ctypes.POINTER(LazyConfig), vp, vp, vp, vp, vp, vp, i32, vp, vp]
         L.lazy_set_rope_frequencies.restype = ctypes.c_int
         L.lazy_set_rope_frequencies.argtypes = [vp, vp, ctypes.c_double, vp]
         L.lazy_set_alibi_slopes.restype = ctypes.c_int
@@ -206,6 +210,17 @@ def lazy_attn_decode(h: LazyHandle, q, k_cache, v_cache, block_table, page_logic
                                 _ptr(page_logical_pos), _ptr(seq_lens), num_reqs, _ptr(out), _stream(stream))
     if rc != 0:
         raise LazyError("lazy_attn_decode", rc)
+
+
+def lazy_attn_decode_static(cfg: LazyConfig, q, k_cache, v_cache, block_table, page_logical_pos, seq_lens, out,
+                            stream=None) -> None:
+    """Decode for callers that cannot allocate device memory (no handle, no workspace tensor): the library's built-in
+    LAZY_STATIC_SCRATCH_BYTES array is the scratch.  One call at a time per GPU; see include/lazy_attn.h."""
+    num_reqs = int(seq_lens.shape[0])
+    rc = lib().lazy_attn_decode_static(ctypes.byref(cfg), _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_table),
+                                       _ptr(page_logical_pos), _ptr(seq_lens), num_reqs, _ptr(out), _stream(stream))
+    if rc != 0:
+        raise LazyError("lazy_attn_decode_static", rc)
 
 
 def lazy_set_rope_frequencies(h: LazyHandle, inv_freq=None, softmax_scale: float = 0.0, stream=None) -> None:

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(CSRC, "liblazyattn.so")
-SOURCES = ["lazy_api.cu", "basic_kernels.cu", "decode_splitkv.cu", "prefill_umma.cu", "prefill_umma2.cu", "mixed_fused.cu", "fp8_kernels.cu", "page_pool.cpp"]
+SOURCES = ["lazy_api.cu", "basic_kernels.cu", "decode_splitkv.cu", "decode_static.cu", "prefill_umma.cu", "prefill_umma2.cu", "mixed_fused.cu", "fp8_kernels.cu", "page_pool.cpp"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
          "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC] + os.environ.get("LAZY_NVCC_EXTRA", "").split()

@@ -357,6 +357,7 @@ const char* lazy_status_string(int status) {
     case LAZY_ERR_UNSUPPORTED: return "unsupported configuration";
     case LAZY_ERR_WORKSPACE: return "workspace too small or misaligned";
     case LAZY_ERR_CUDA: return "CUDA error at launch";
+    case LAZY_ERR_STATIC_LIMIT: return "configuration needs more scratch than LAZY_STATIC_SCRATCH_BYTES";
     default: return "unknown status";
   }
 }
