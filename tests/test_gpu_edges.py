@@ -191,6 +191,99 @@ def test_host_step_matches_device_calls():
     dev.close(); dev2.close()
 
 
+def _packed_step(dev, batch, step):
+    """One step through lazy_host_step_layout + lazy_host_step_packed (the call bench.py's e2e leg times): the caller
+    packs every input into one pinned block at the offsets the library states."""
+    bt = batch.block_table if step.req_ids is None else batch.block_table[step.req_ids]
+    pp = batch.page_logical_pos if step.req_ids is None else batch.page_logical_pos[step.req_ids]
+    R, tq = step.seq_lens.shape[0], step.q.shape[0]
+    nn = 0 if step.k_new is None else step.k_new.shape[0]
+    lay = B.lazy_host_step_layout(dev.handle, R, tq, nn)
+    assert lay.staging_bytes == B.lazy_host_step_staging_bytes(dev.handle, R, tq, nn)
+    assert lay.in_bytes == lay.out and lay.out < lay.staging_bytes
+    offs = [lay.q, lay.k_new, lay.v_new, lay.slot_mapping, lay.block_table, lay.page_logical_pos, lay.seq_lens,
+            lay.cu_q_lens, lay.out]
+    assert all(o % 256 == 0 for o in offs) and offs == sorted(offs)
+    packed = torch.full((int(lay.in_bytes),), 0xA5, dtype=torch.uint8).pin_memory()     # gaps hold junk
+
+    def put(off, t):
+        raw = t.contiguous().view(torch.uint8).reshape(-1)
+        packed[off:off + raw.numel()] = raw
+    put(lay.q, step.q)
+    if nn:
+        put(lay.k_new, step.k_new); put(lay.v_new, step.v_new); put(lay.slot_mapping, step.slot_mapping)
+    put(lay.block_table, bt.to(torch.int32)); put(lay.page_logical_pos, pp.to(torch.int32))
+    put(lay.seq_lens, step.seq_lens)
+    kind, max_q = 0, 1
+    if step.kind == "prefill":
+        kind = 1
+        put(lay.cu_q_lens, step.cu_q_lens)
+        max_q = int((step.cu_q_lens[1:] - step.cu_q_lens[:-1]).max())
+    hout = torch.full_like(step.q, float("nan")).pin_memory()
+    staging = torch.empty(int(lay.staging_bytes) + 256, dtype=torch.uint8, device="cuda")
+    base = (staging.data_ptr() + 255) // 256 * 256
+    args = B.HostStepPacked(kind, R, tq, max_q, nn, 0, packed.data_ptr(), hout.data_ptr(), dev.k_pool.data_ptr(),
+                            dev.v_pool.data_ptr(), base, int(lay.staging_bytes))
+    B.lazy_host_step_packed(dev.handle, args)
+    torch.cuda.synchronize()
+    return hout
+
+
+@pytest.mark.parametrize("cfg,scale", [(2, 0.1), (3, 0.05), (5, 0.2)])
+def test_host_step_packed_matches_oracle_and_device_calls(cfg, scale):
+    """lazy_host_step_layout + lazy_host_step_packed, decode and prefill kinds: every step of the batch (cache write
+    included) through the packed call on one handle, through the device-pointer calls on another and through the
+    oracle; pools bit-equal afterwards."""
+    from oracle import oracle as O
+    from gpu_util import compare
+    b = W.CONFIGS[cfg](scale=scale)
+    dev, dev2 = DeviceBatch(b), DeviceBatch(b)
+    k_ref, v_ref = b.k_pool.clone(), b.v_pool.clone()
+    kinds = set()
+    try:
+        for si, step in enumerate(b.steps):
+            want = dev.run_step(step)
+            ref = O.run_step(b, step, k_ref, v_ref)
+            if step.kind == "write_only":
+                dev2.write(step)
+                continue
+            got = _packed_step(dev2, b, step)
+            kinds.add(step.kind)
+            compare(got, ref, f"cfg{cfg} step {si} ({step.kind}) packed host step")
+            if step.kind == "prefill":                                     # same kernel, same grid: bit equal
+                assert torch.equal(got.view(torch.int16), want.cpu().view(torch.int16))
+            else:                                                          # split-KV summation order may differ
+                assert (got.float() - want.cpu().float()).abs().max().item() < 2e-3
+            assert torch.equal(dev2.k_pool.cpu().view(torch.int16), k_ref.view(torch.int16))
+            assert torch.equal(dev2.v_pool.cpu().view(torch.int16), v_ref.view(torch.int16))
+        assert kinds
+    finally:
+        dev.close(); dev2.close()
+
+
+def test_host_step_packed_rejects_bad_arguments():
+    b = W.config2(scale=0.05)
+    dev = DeviceBatch(b)
+    try:
+        lay = B.lazy_host_step_layout(dev.handle, 4, 4, 4)
+        a = B.HostStepPacked(0, 4, 4, 1, 4, 0, None, None, None, None, None, 0)
+        with pytest.raises(B.LazyError):
+            B.lazy_host_step_packed(dev.handle, a)
+        staging = torch.empty(int(lay.staging_bytes) + 256, dtype=torch.uint8, device="cuda")
+        base = (staging.data_ptr() + 255) // 256 * 256
+        host = torch.zeros(int(lay.in_bytes), dtype=torch.uint8).pin_memory()
+        hout = torch.zeros(4 * b.shape.num_q_heads * b.shape.head_dim, dtype=torch.bfloat16).pin_memory()
+        a = B.HostStepPacked(0, 4, 4, 1, 4, 0, host.data_ptr(), hout.data_ptr(), dev.k_pool.data_ptr(),
+                             dev.v_pool.data_ptr(), base, int(lay.staging_bytes) - 1)
+        with pytest.raises(B.LazyError) as e:
+            B.lazy_host_step_packed(dev.handle, a)
+        assert e.value.status == B.LAZY_ERR_WORKSPACE
+        with pytest.raises(B.LazyError):
+            B.lazy_host_step_layout(dev.handle, -1, 4, 4)
+    finally:
+        dev.close()
+
+
 def test_many_requests_cross_the_per_launch_limit():
     """Maximum sizes: more requests than one decode launch keeps in shared memory (2048) -> lazy_attn_decode splits
     the batch into several launches; many short prefill chunks -> one CTA per (request, kv head)."""
