@@ -90,10 +90,11 @@ __device__ __forceinline__ void combine_request(const DecodeArgs& a, const int r
     for (int base = 0; base < n_slots; base += cap) {
       const int n = min(cap, n_slots - base);
       if (warp == 0) {
-        if (lane == 0) {
-          ptx::fence_proxy_async_all();             // the partials were written through the generic proxy
-          ptx::mbar_arrive_expect_tx(cbar, (uint32_t)(n * slot_bytes));
-        }
+        // the partials were written through the generic proxy: EVERY lane that issues a bulk copy (an async-proxy
+        // read) fences first -- a proxy fence orders the executing thread's accesses only, and __syncwarp does not
+        // carry it to the other lanes
+        if (lane < n) ptx::fence_proxy_async_all();
+        if (lane == 0) ptx::mbar_arrive_expect_tx(cbar, (uint32_t)(n * slot_bytes));
         __syncwarp();
         if (lane < n)
           ptx::bulk_load_1d(ring_u32 + lane * slot_bytes,

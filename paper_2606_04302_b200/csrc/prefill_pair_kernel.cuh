@@ -267,9 +267,9 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
           }
         };
         auto commit = [&](int idx) { if (leader) ptx::umma_commit_pair(bar(idx)); };
-        ptx::mbar_wait(bar(P_KREADY + 0), 0);
+        ptx::mbar_wait_acquire_cluster(bar(P_KREADY + 0), 0);
         for (int t = 0; t < 2; ++t) {
-          ptx::mbar_wait(bar(P_QREADY + t), 0);
+          ptx::mbar_wait_acquire_cluster(bar(P_QREADY + t), 0);
           ptx::tc_fence_after();
           for (int h = 0; h < 2; ++h) { qk(t, 0, h); commit(P_SFULL + 2 * t + h); }
         }
@@ -280,21 +280,21 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
         // ahead of the other; the kernel then alternated between bursts of one tile and refill latencies: 668 TFLOP/s.)
         for (int j = 0; j < nkv; ++j) {
           const int s = j & (kStages - 1), sn = (j + 1) & (kStages - 1);
-          if (F8) ptx::mbar_wait(bar(P_VREADY + s), (j / kStages) & 1);
-          else if (j == nkv - 1) ptx::mbar_wait(bar(P_VFIXED), 0);
+          if (F8) ptx::mbar_wait_acquire_cluster(bar(P_VREADY + s), (j / kStages) & 1);
+          else if (j == nkv - 1) ptx::mbar_wait_acquire_cluster(bar(P_VFIXED), 0);
           else ptx::mbar_wait(bar(P_VFULL + s), (j / kStages) & 1);
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
-              ptx::mbar_wait(bar(P_PREADY + 2 * t + h), j & 1);
+              ptx::mbar_wait_tmem(bar(P_PREADY + 2 * t + h), j & 1);
               ptx::tc_fence_after();
               pv(t, s, h, (uint32_t)(j > 0 || h > 0));
               commit(P_PVDONE + 2 * t + h);
               if (h == 1 && t == 1) commit(P_VEMPTY + s);
               if (j + 1 < nkv) {
                 if (h == 0 && t == 0) {
-                  ptx::mbar_wait(bar(P_KREADY + sn), ((j + 1) / kStages) & 1);
+                  ptx::mbar_wait_acquire_cluster(bar(P_KREADY + sn), ((j + 1) / kStages) & 1);
                   ptx::tc_fence_after();
                 }
                 qk(t, sn, h);
@@ -320,7 +320,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
       }
       ptx::fence_proxy_async();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_VFIXED));
+      if (lane == 0) ptx::mbar_arrive_cluster_release(lbar(P_VFIXED));
     }
   } else if (warp >= 8) {
     // ================================ K-rotate warpgroup ======================================================
@@ -414,7 +414,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
         }
         ptx::fence_proxy_async();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_KREADY + s));
+        if (lane == 0) ptx::mbar_arrive_cluster_release(lbar(P_KREADY + s));
         // ---- V: this CTA's 64-column slab of all 8 pages; thread = (page vp, token vt): 64 codes -> one 128-byte row
         const int vp = wtid >> 4, vt = wtid & 15;
         const int vrow = vp * kPageSize + vt;
@@ -453,7 +453,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
         }
         ptx::fence_proxy_async();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_VREADY + s));
+        if (lane == 0) ptx::mbar_arrive_cluster_release(lbar(P_VREADY + s));
         continue;
       }
       if (!kNoRotate && i < npk) {
@@ -500,7 +500,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
       }
       ptx::fence_proxy_async();
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_KREADY + s));
+      if (lane == 0) ptx::mbar_arrive_cluster_release(lbar(P_KREADY + s));
     }
   } else {
     // ================================ softmax warpgroups ======================================================
@@ -574,7 +574,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
     }
     ptx::fence_proxy_async();
     __syncwarp();
-    if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_QREADY + t));
+    if (lane == 0) ptx::mbar_arrive_cluster_release(lbar(P_QREADY + t));
 
     float alibi_slope = 0.f;                                   // kKmAlibi: this row's slope (log2 units), position
     int alibi_pos_q = 0;
@@ -724,7 +724,7 @@ __device__ __forceinline__ void prefill_pair_cta(const CUtensorMap& tmap_q, cons
         ptx::tmem_wait_st();
         ptx::tc_fence_before();
         __syncwarp();
-        if (lane == 0) ptx::mbar_arrive_cluster(lbar(P_PREADY + 2 * t + hf));
+        if (lane == 0) ptx::mbar_arrive_cluster_tmem(lbar(P_PREADY + 2 * t + hf));
       }
     }
 

@@ -231,6 +231,62 @@ __device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
   asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
+// The same arrival with CLUSTER-scope release, for hand-offs that publish generic-proxy writes of THIS CTA's shared
+// memory to a thread of the OTHER CTA of the pair (the leader's MMA thread, whose cta_group::2 MMA reads both CTAs'
+// operand tiles): writer and observer sit in different CTAs, so the PTX memory model formally wants .cluster on both
+// sides (mbar_wait_acquire_cluster on the waiting side).  Build-time choice, -DLAZY_CLUSTER_SCOPE=
+//   0 (default)  CTA scope everywhere.  What makes this safe in practice: each SM's tensor core reads ITS OWN shared
+//                memory for its half of a cta_group::2 operand, the writer runs fence.proxy.async after its stores
+//                (they are visible to that SM's async proxy before the arrival is issued), and the arrival travels to
+//                the leader after it.  The formal gap is recorded in DESIGN.md 6.2 and watched by
+//                tests/test_gpu_determinism.py (1000 bit-identical runs per case under L2 / SM pressure).
+//   1            cluster scope on the shared-memory publishing hand-offs (K / V / Q ready, V fixed): + 3 MEMBAR.ALL.GPU
+//                and + 7 CCTL.IVALL in the pair kernel.  Measured on B200: cfg3 bf16 1.106 -> 1.122 ms, cfg5
+//                block-local prefill 76.4 -> 83.0 us, cfg5 mixed step 135.2 -> 142.7 us, cfg3 on FP8 pages (one V-ready
+//                hand-off per tile on top of K-ready) 1.142 -> 1.598 ms.
+//   2            also on the TMEM hand-off (P ready): cfg3 bf16 1.63 ms.
+#ifndef LAZY_CLUSTER_SCOPE
+#define LAZY_CLUSTER_SCOPE 0
+#endif
+__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t cluster_bar) {
+#if LAZY_CLUSTER_SCOPE >= 1
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+#else
+  mbar_arrive_cluster(cluster_bar);
+#endif
+}
+__device__ __forceinline__ void mbar_wait_acquire_cluster(uint32_t bar, uint32_t parity) {
+#if LAZY_CLUSTER_SCOPE >= 1
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+#else
+  mbar_wait(bar, parity);
+#endif
+}
+__device__ __forceinline__ void mbar_arrive_cluster_tmem(uint32_t cluster_bar) {
+#if LAZY_CLUSTER_SCOPE >= 2
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+#else
+  mbar_arrive_cluster(cluster_bar);
+#endif
+}
+__device__ __forceinline__ void mbar_wait_tmem(uint32_t bar, uint32_t parity) {
+#if LAZY_CLUSTER_SCOPE >= 2
+  mbar_wait_acquire_cluster(bar, parity);
+#else
+  mbar_wait(bar, parity);
+#endif
+}
 // TMA load whose completion bytes are counted on a barrier of the pair's LEADER CTA (cluster address)
 __device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const void* tmap, uint32_t leader_bar, int c0, int c1) {
   asm volatile(
