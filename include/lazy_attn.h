@@ -107,7 +107,12 @@ typedef struct lazy_config {
  *                     arrays [num_pages][num_kv_heads][page_size] fp32 registered with lazy_set_kv_scales (per token,
  *                     because lazy_cache_write appends single tokens to half-filled pages).  lazy_cache_write
  *                     quantises: scale = max|row| / 448 in fp32 (1 for an all-zero row), code = nearest E4M3 (ties
- *                     to even, saturating) of the fp32 quotient row[d] / scale.  The attention calls compute what the
+ *                     to even, saturating) of the fp32 quotient row[d] / scale.  k_new / v_new must be FINITE: a row
+ *                     with an Inf or NaN element is not rejected (there is no device-side error channel) but stored so
+ *                     that it reads back as NaN -- Inf makes the row's scale inf (code x inf = NaN for every element),
+ *                     a NaN element becomes the E4M3 NaN code -- and every query that sees the token returns NaN, as
+ *                     it would on bf16 pages.  q may have any finite bf16 magnitude (the FP8 decode kernel, which
+ *                     multiplies in f16, normalises q by a power of two first).  The attention calls compute what the
  *                     bf16 calls would compute on the exactly dequantised pages (code value x scale).  Supported
  *                     with both RoPE pairings (not ALiBi) and LAZY_K_UNROTATED; lazy_materialize_pages is bf16-only.  Every call
  *                     runs on the product kernels at either head_dim (split-KV decode; tcgen05 prefill, on CTA pairs
@@ -337,7 +342,8 @@ typedef struct lazy_mixed_args {
   const void* q_decode;  const int32_t* block_table_decode;  const int32_t* page_logical_pos_decode;
   const int32_t* seq_lens_decode;
   int32_t num_reqs_decode;
-  int32_t decode_sms;     /* SMs the decode kernel may occupy while both run; 0 = three quarters of the device     */
+  int32_t decode_sms;     /* SMs (= CTAs) given to the decode half; 0 = the default: 7/16 of the device on the one-launch
+                             path (64 of 148), three quarters on the two-stream path (reserved0 bit 0, other configurations) */
   void* out_decode;
 } lazy_mixed_args;
 int lazy_attn_mixed(lazy_handle* h, const lazy_mixed_args* a, const void* k_cache, const void* v_cache, void* stream);

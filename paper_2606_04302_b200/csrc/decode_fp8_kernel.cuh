@@ -299,6 +299,24 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
         }
       }
     }
+    // One power-of-two normaliser per (request, kv head): the largest |q| of the GQA group goes to [1, 2) before the
+    // f16 pack (|R q| <= sqrt(2) max|q| < 2.83), its inverse into the score scale.  Exact (powers of two), once per
+    // segment, nothing per page: f16's range (65504, 6e-5) puts no restriction on q.
+    float qmax = 0.f;
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int w = 0; w < C::NL; ++w) qmax = fmaxf(qmax, fmaxf(fabsf(qf[h][w][0]), fabsf(qf[h][w][1])));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) qmax = fmaxf(qmax, __shfl_xor_sync(0xffffffffu, qmax, o));
+    int qexp = 0;
+    if (qmax > 0.f && qmax < INFINITY) qexp = max(-126, min(126, ((__float_as_int(qmax) >> 23) & 0xff) - 127));
+    const float q_down = __int_as_float((127 - qexp) << 23);
+    const float scale_log2 = sh.scale_log2 * __int_as_float((127 + qexp) << 23);
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+      for (int w = 0; w < C::NL; ++w) { qf[h][w][0] *= q_down; qf[h][w][1] *= q_down; }
     uint32_t qhat[2][C::NL];
 
     float oacc[C::NC][4];
@@ -335,8 +353,8 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
           }
         // scales of this thread's two tokens: K (times log2(e)/sqrt(D)) and V
         const uint32_t sc_off = scofs;
-        const float sk0 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off)) * sh.scale_log2;
-        const float sk1 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off + 8)) * sh.scale_log2;
+        const float sk0 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off)) * scale_log2;
+        const float sk1 = __int_as_float(ptx::lds32(st + C::OFF_SK + sc_off + 8)) * scale_log2;
         float sv0 = __int_as_float(ptx::lds32(st + C::OFF_SV + sc_off));
         float sv1 = __int_as_float(ptx::lds32(st + C::OFF_SV + sc_off + 8));
         // ---- q re-rotated for this page: Qhat = R_{m - p0} q in fp32, rounded to f16 (a3/a4)

@@ -80,6 +80,35 @@ def test_fp8_cache_write_edge_rows():
     h.close()
 
 
+def test_fp8_cache_write_non_finite_rows_read_back_as_nan():
+    """include/lazy_attn.h (LAZY_KV_FP8_E4M3): inputs must be finite; a row with Inf or NaN is stored so that it reads
+    back as NaN instead of being silently flattened -- Inf: scale = inf and code x inf = NaN for every element; NaN:
+    finite scale from the other elements, the element itself gets the E4M3 NaN code.  Neighbouring rows are untouched."""
+    Hkv, D, P = 1, 128, 16
+    dev = torch.device("cuda")
+    h = B.lazy_create(4, Hkv, D, num_pages=2, max_position=256, max_reqs=1, max_pages_per_req=2, rope_theta=1e4,
+                      dtype=B.LAZY_KV_FP8_E4M3, device=dev)
+    kc = torch.zeros((2, Hkv, P, D), dtype=torch.uint8, device=dev)
+    vc = torch.zeros((2, Hkv, P, D), dtype=torch.uint8, device=dev)
+    ks = torch.ones((2, Hkv, P), dtype=torch.float32, device=dev)
+    vs = torch.ones((2, Hkv, P), dtype=torch.float32, device=dev)
+    B.lazy_set_kv_scales(h, ks, vs)
+    g = torch.Generator().manual_seed(9)
+    k = torch.randn(3, Hkv, D, generator=g).to(torch.bfloat16)
+    v = torch.randn(3, Hkv, D, generator=g).to(torch.bfloat16)
+    k[0, 0, 7] = float("inf")
+    v[1, 0, 100] = float("nan")
+    B.lazy_cache_write(h, k.to(dev), v.to(dev), torch.arange(3, dtype=torch.int64, device=dev), kc, vc)
+    torch.cuda.synchronize()
+    deq = lambda c, s: c.cpu().view(torch.float8_e4m3fn).float() * s.cpu()[..., None]
+    kd, vd = deq(kc, ks), deq(vc, vs)
+    assert torch.isinf(ks[0, 0, 0]) and torch.isnan(kd[0, 0, 0]).all()               # Inf row: every element NaN
+    assert torch.isfinite(vs[0, 0, 1]) and torch.isnan(vd[0, 0, 1, 100])             # NaN element stays NaN ...
+    assert torch.isfinite(vd[0, 0, 1]).sum() == D - 1                                #   ... the rest of its row is kept
+    assert torch.isfinite(kd[0, 0, 1:3]).all() and torch.isfinite(vd[0, 0, [0, 2]]).all()   # neighbours untouched
+    h.close()
+
+
 def test_fp8_needs_scales_and_rejects_unsupported_modes():
     dev = torch.device("cuda")
     with pytest.raises(B.LazyError):
@@ -125,7 +154,8 @@ def test_fp8_v_scale_outlier_tokens():
 
 
 def test_fp8_mixed_call_matches_oracle():
-    """lazy_attn_mixed on FP8 pages (two kernels on forked streams: the one-launch step is bf16-only)."""
+    """lazy_attn_mixed on FP8 pages at 4 kv heads: the one-launch FP8 step (mixed_step_fp8_kernel: 12-warp FP8 decode
+    body + FP8 pair prefill body in one grid)."""
     from oracle import oracle as O
     from paper_2606_04302_b200.runner import DeviceBatch
     from gpu_util import compare
@@ -275,3 +305,20 @@ def test_fp8_interleaved_pairing(cfg, scale, flags):
     D = batch.shape.head_dim
     perm = np.concatenate([np.arange(0, D, 2), np.arange(1, D, 2)])
     _run(batch, flags=flags, dev_kw=dict(rope_style=B.LAZY_ROPE_INTERLEAVED), oracle_kw=dict(rope_style=1), k_perm=perm)
+
+
+@pytest.mark.parametrize("log2_q", [16, -20])
+@pytest.mark.parametrize("cfg,scale", [(1, None), (2, 0.1), (5, 0.2)])
+def test_fp8_q_far_outside_the_f16_range(cfg, scale, log2_q):
+    """The FP8 decode kernel packs the rotated q to f16 for its MMAs.  q scaled by 2^16 puts the rotated values beyond
+    f16's largest finite number (65504 -> inf -> NaN after the softmax), q scaled by 2^-20 below its smallest normal
+    one (6e-5 -> precision lost, then flushed); the bf16-page kernels take both.  The kernel therefore normalises q by
+    a power of two per (request, kv head) and folds the inverse into the score scale.  Here the softmax temperature is
+    scaled the other way, so the scores -- and the oracle's answer -- are those of the unscaled batch and the usual
+    gates apply."""
+    import math
+    kw = dict(q_scale=2.0 ** log2_q)
+    batch = W.CONFIGS[cfg](**kw) if scale is None else W.CONFIGS[cfg](scale=scale, **kw)
+    temp = 2.0 ** (-log2_q) / math.sqrt(batch.shape.head_dim)
+    stats = _run(batch, dev_kw=dict(softmax_scale=temp), oracle_kw=dict(scale=temp))
+    assert stats
