@@ -179,6 +179,11 @@ class GpuJob:
                 rec["cu"] = st.cu_q_lens.to(d)
                 rec["max_q"] = int((st.cu_q_lens[1:] - st.cu_q_lens[:-1]).max())
             self.timed.append(rec)
+        # one lazy_cache_write per step: the ABI takes ONE slot mapping over all new tokens of the step (prefill chunk
+        # tokens and the decode tokens alike), which is how a serving engine hands them over
+        self.kv_cat = None
+        if len(self.timed) > 1:
+            self.kv_cat = tuple(torch.cat([r[k] for r in self.timed]).contiguous() for k in ("k_new", "v_new", "slots"))
         self.flush_buf = torch.empty(512 << 20, dtype=torch.uint8, device=d)
         self.sweep_buf = torch.zeros(64 << 20, dtype=torch.int32, device=d)      # 256 MB
 
@@ -191,8 +196,11 @@ class GpuJob:
     def run(self, ev_mid=None, call_evs=None):
         """call_evs: list that receives one (start, end) event pair per attention call (separate calls only)."""
         B, dev = self.B, self.dev
-        for rec in self.timed:
-            B.lazy_cache_write(dev.handle, rec["k_new"], rec["v_new"], rec["slots"], dev.k_pool, dev.v_pool)
+        if self.kv_cat is not None:
+            B.lazy_cache_write(dev.handle, self.kv_cat[0], self.kv_cat[1], self.kv_cat[2], dev.k_pool, dev.v_pool)
+        else:
+            for rec in self.timed:
+                B.lazy_cache_write(dev.handle, rec["k_new"], rec["v_new"], rec["slots"], dev.k_pool, dev.v_pool)
         if ev_mid is not None:
             ev_mid.record()
         kinds = [rec["step"].kind for rec in self.timed]
@@ -234,6 +242,7 @@ class GpuJob:
                     one = GpuJob.__new__(GpuJob)
                     one.__dict__.update(self.__dict__)
                     one.timed = [dict(rec, k_new=rec["k_new"][:0], v_new=rec["v_new"][:0], slots=rec["slots"][:0])]
+                    one.kv_cat = None
                     one.run(call_evs=evs)
                 torch.cuda.synchronize()
                 if i >= warmup:
@@ -293,22 +302,71 @@ class GpuJob:
             self.e2e.append(dict(args=args, packed=packed, out=out, staging=staging, h2d=int(lay.in_bytes),
                                  h2d_payload=h2d, d2h=out.numel() * 2))
 
+    def prepare_e2e_unpacked(self):
+        """The same steps through lazy_host_step: every input in its own pinned host tensor (what a caller with separate
+        tensors hands over), seven H2D copies per step instead of one packed block."""
+        B, dev = self.B, self.dev
+        self.e2e_unpacked = []
+        pin = lambda t: t.contiguous().pin_memory()
+        for rec in self.timed:
+            st = rec["step"]
+            bt = self.batch.block_table if st.req_ids is None else self.batch.block_table[st.req_ids]
+            pp = self.batch.page_logical_pos if st.req_ids is None else self.batch.page_logical_pos[st.req_ids]
+            R, tq, nn = st.seq_lens.shape[0], st.q.shape[0], st.k_new.shape[0]
+            host = dict(q=pin(st.q), k=pin(st.k_new), v=pin(st.v_new), s=pin(st.slot_mapping), bt=pin(bt.to(torch.int32)),
+                        pp=pin(pp.to(torch.int32)), sl=pin(st.seq_lens),
+                        cu=pin(st.cu_q_lens) if st.kind != "decode" else None)
+            out = torch.empty_like(st.q).pin_memory()
+            nbytes = B.lazy_host_step_staging_bytes(dev.handle, R, tq, nn)
+            staging = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev.device)
+            base = (staging.data_ptr() + 255) // 256 * 256
+            args = B.HostStep(0 if st.kind == "decode" else 1, R, tq, rec.get("max_q", 1), nn, 0, host["q"].data_ptr(),
+                              host["k"].data_ptr(), host["v"].data_ptr(), host["s"].data_ptr(), host["bt"].data_ptr(),
+                              host["pp"].data_ptr(), host["sl"].data_ptr(),
+                              None if host["cu"] is None else host["cu"].data_ptr(), out.data_ptr(),
+                              dev.k_pool.data_ptr(), dev.v_pool.data_ptr(), base, nbytes)
+            self.e2e_unpacked.append(dict(args=args, host=host, out=out, staging=staging))
+
     def run_e2e(self):
         for e in self.e2e:
             self.B.lazy_host_step_packed(self.dev.handle, e["args"])
 
-    def time_e2e(self, steps, warmup, barrier):
+    def run_e2e_unpacked(self):
+        for e in self.e2e_unpacked:
+            self.B.lazy_host_step(self.dev.handle, e["args"])
+
+    def time_e2e(self, steps, warmup, barrier, run=None):
+        run = run or self.run_e2e
         for _ in range(warmup):
-            self.flush_l2(); self.run_e2e()
+            self.flush_l2(); run()
         evs = [[torch.cuda.Event(enable_timing=True) for _ in range(2)] for _ in range(steps)]
         barrier(); torch.cuda.synchronize()
         for i in range(steps):
             self.flush_l2()
             evs[i][0].record()
-            self.run_e2e()
+            run()
             evs[i][1].record()
         torch.cuda.synchronize(); barrier()
         return sum(e[0].elapsed_time(e[1]) for e in evs)
+
+    def verify_e2e(self):
+        """Outside every timed region: what the timed host-buffer calls wrote to h_out against the `out` of the
+        device-pointer step on the same handle.  Prefill is the same kernel on the same grid (bit equal); decode may
+        differ in the split-KV combine order (which CTA arrives last), hence a bound instead of equality."""
+        self.run(); self.run_e2e()
+        if getattr(self, "e2e_unpacked", None):
+            self.run_e2e_unpacked()
+        torch.cuda.synchronize()
+        worst, bit_equal = 0.0, True
+        for i, rec in enumerate(self.timed):
+            want = rec["out"].float().cpu()
+            for e in [self.e2e[i]] + ([self.e2e_unpacked[i]] if getattr(self, "e2e_unpacked", None) else []):
+                got = e["out"].float()
+                assert torch.isfinite(got).all(), "e2e output is not finite"
+                worst = max(worst, float((got - want).abs().max()))
+                bit_equal = bit_equal and bool(torch.equal(e["out"].view(torch.int16), rec["out"].cpu().view(torch.int16)))
+        assert worst < 2e-3, f"e2e output differs from the device-pointer step by {worst}"
+        return {"max_abs_diff_vs_device_step": worst, "bit_equal": bit_equal}
 
 
 def run_ablation(job, steps, warmup):
@@ -444,6 +502,98 @@ def run_ablation(job, steps, warmup):
     res["materialize_bytes"] = 4 * n * page_bytes                 # K read + K write + V read + V write
     res["materialize_GBps"] = res["materialize_bytes"] / (mat_ms * 1e-3) / 1e9
     return res
+
+
+def _round(o):
+    """Floats to 5 significant digits (the whole line must fit the driver's 3 KB tail)."""
+    if isinstance(o, dict):
+        return {k: _round(v) for k, v in o.items()}
+    if isinstance(o, list):
+        return [_round(v) for v in o]
+    if isinstance(o, float):
+        return float(f"{o:.5g}")
+    return o
+
+
+def _get(o, *path):
+    for k in path:
+        if not isinstance(o, dict) or k not in o:
+            return None
+        o = o[k]
+    return o
+
+
+def compact_line(out):
+    """The one JSON line bench.py prints (the verbose record goes to stderr): the contract's keys, the side legs as
+    kernel times only, and LAST a flat `summary` -- so that it survives any tail cut -- with both halves of
+    BASELINE.json's metric (decode HBM fraction, prefill tensor fraction) and the f1 / f2 figures."""
+    line = {k: v for k, v in out.items() if k not in ("configs", "roofline", "e2e", "clocks", "ablation", "tokens_per_s",
+                                                      "cpu_baseline", "mixed", "graph")}
+    line["config"] = dict(out["config"], l2="flushed between timed steps", parallelism=f"replicas x{out['n_gpus']}")
+    r = out["roofline"]
+    line["roofline"] = {k: r[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "peak_source",
+                                          "workload", "kernel_ms", "note") if k in r}
+    if "shared" in r:
+        line["roofline"]["shared"] = {k: r["shared"][k] for k in ("kernel_ms", "logical_GBps", "unique_GBps", "traffic")}
+    e = out["e2e"]
+    line["e2e"] = {k: e[k] for k in ("value", "unit", "ms_per_step", "h2d_bytes_per_step", "d2h_bytes_per_step")}
+    line["e2e"]["api"] = "lazy_host_step_packed"
+    if "unpacked" in e:
+        line["e2e"]["lazy_host_step_ms"] = e["unpacked"]["ms_per_step"]
+        line["e2e"]["verified"] = e["verified"]
+    line["clocks"] = {k: v for k, v in out["clocks"].items() if k not in ("window", "samples")}
+    for k in ("mixed", "graph"):
+        if k in out:
+            line[k] = out[k]
+    c = out.get("configs") or {}
+    if c:
+        picks = {"cfg3_ms": ("cfg3", "kernel_ms"), "cfg3_sustained_ms": ("cfg3", "sustained", "kernel_ms"),
+                 "cfg3_sustained_reasons": ("cfg3", "sustained", "clocks", "reasons"),
+                 "cfg4_noshare_ms": ("cfg4", "noshare", "kernel_ms"), "cfg4_shared_ms": ("cfg4", "shared", "kernel_ms"),
+                 "cfg4_shared_logical_GBps": ("cfg4", "shared", "logical_GBps"),
+                 "cfg5_prefill_ms": ("cfg5", "prefill", "kernel_ms"),
+                 "cfg5_decode_noshare_ms": ("cfg5", "decode_noshare", "kernel_ms"),
+                 "cfg5_decode_shared_ms": ("cfg5", "decode_shared", "kernel_ms"),
+                 "cfg5_cache_write_ms": ("cfg5", "cache_write", "ms"),
+                 "fp8_cfg2_ms": ("fp8_pages", "cfg2_noshare", "kernel_ms"),
+                 "fp8_cfg4_ms": ("fp8_pages", "cfg4_noshare", "kernel_ms"),
+                 "fp8_cfg5_ms": ("fp8_pages", "cfg5_noshare", "kernel_ms"),
+                 "fp8_cfg3_prefill_ms": ("fp8_pages", "cfg3_prefill", "kernel_ms"),
+                 "fp8_cfg5_mixed_step_ms": ("fp8_pages", "cfg5_mixed_step", "ms_per_step")}
+        line["configs"] = {k: _get(c, *p) for k, p in picks.items() if _get(c, *p) is not None}
+        errs = {k: v["error"] for k, v in c.items() if isinstance(v, dict) and "error" in v}
+        if errs:
+            line["configs"]["errors"] = errs
+    ab = out.get("ablation") or {}
+    if ab:
+        line["ablation"] = {k: ab[k] for k in ("unrotated_ms", "stored_pos_ms", "absolute_ms", "materialize_GBps") if k in ab}
+    if "cpu_baseline" in out:
+        line["cpu_baseline"] = {k: v for k, v in out["cpu_baseline"].items() if k != "seconds"}
+    sm = {}
+
+    def put(name, *path, src=None):
+        v = _get(c if src is None else src, *path)
+        if v is not None:
+            sm[name] = v
+    wl = out["config"]["workload"].split()[0]
+    sm[f"{wl}_roofline_frac"] = r["frac"]
+    put("cfg2_shared_logical_GBps", "shared", "logical_GBps", src=r)
+    put("cfg3_TFLOPs", "cfg3", "TFLOPs"); put("cfg3_frac_burst", "cfg3", "frac_of_bf16_peak")
+    put("cfg3_sustained_TFLOPs", "cfg3", "sustained", "TFLOPs")
+    put("cfg3_frac_sustained", "cfg3", "sustained", "frac_of_bf16_sustained")
+    put("cfg3_sm_mhz", "cfg3", "sustained", "clocks", "sm_mhz")
+    put("cfg4_noshare_frac", "cfg4", "noshare", "frac_of_hbm_peak")
+    put("cfg5_decode_noshare_frac", "cfg5", "decode_noshare", "frac_of_hbm_peak")
+    put("cfg5_prefill_frac", "cfg5", "prefill", "frac_of_bf16_peak")
+    put("cfg5_mixed_attention_ms", "cfg5", "mixed_attention_ms"); put("cfg5_mixed_step_ms", "cfg5", "mixed_step_ms")
+    put("fp8_cfg2_frac", "fp8_pages", "cfg2_noshare", "frac_of_hbm_peak")
+    put("fp8_cfg4_frac", "fp8_pages", "cfg4_noshare", "frac_of_hbm_peak")
+    put("fp8_cfg5_frac", "fp8_pages", "cfg5_noshare", "frac_of_hbm_peak")
+    put("fp8_cfg3_frac_burst", "fp8_pages", "cfg3_prefill", "frac_of_bf16_peak")
+    for k in ("rotation_overhead_pct", "materialize_ms", "lazy_speedup_vs_materialising"):
+        put(k, k, src=ab)
+    line["summary"] = sm
+    return _round(line)
 
 
 def headline(workload, work, ms_step):
@@ -626,7 +776,7 @@ def _cache_write_entry(_batch, tokens, sh, fp8, ms):
     rd = tokens * sh.num_kv_heads * sh.head_dim * 2 * 2                      # bf16 K and V rows in
     wr = tokens * sh.num_kv_heads * (2 * (sh.head_dim + 4) if fp8 else sh.head_dim * 2 * 2)   # pages (+ scales) out
     return {"bound": "hbm", "tokens": tokens, "bytes": rd + wr, "ms": ms, "GBps": (rd + wr) / (ms * 1e-3) / 1e9,
-            "note": "two launches (prefill tokens, decode tokens): launch-latency-bound at this size"}
+            "note": "one launch over all new tokens of the step; launch-latency-bound at this size"}
 
 
 def cfg5_leg(device, steps, peaks, job=None, fp8=False):
@@ -670,8 +820,8 @@ def cfg5_leg(device, steps, peaks, job=None, fp8=False):
                               "logical_over_hbm_peak": gb_sh / peaks["hbm"]},
             "mixed_step_ms": t_ms / steps, "mixed_attention_ms": a_ms / steps,
             "separate_kernels_sum_ms": per["prefill"] + per["decode"],
-            # row a0 (HBM-bound, 2*Hkv*D*2 B read + the same written per token): the step's two
-            # lazy_cache_write launches = step time - attention time; a few MB, i.e. launch-latency-bound
+            # row a0 (HBM-bound, 2*Hkv*D*2 B read + the same written per token): the step's
+            # lazy_cache_write launch = step time - attention time; a few MB, i.e. launch-latency-bound
             "cache_write": _cache_write_entry(job.batch if not own else None, job_timed_tokens, sh, fp8,
                                               (t_ms - a_ms) / steps)}
 
@@ -772,6 +922,9 @@ def main():
     ms_step, ms_attn = total_ms / args.steps, attn_ms / args.steps
     job.prepare_e2e()
     e2e_ms = max_over_ranks(job.time_e2e(args.steps, args.warmup, barrier)) / args.steps
+    job.prepare_e2e_unpacked()
+    e2e_unpacked_ms = max_over_ranks(job.time_e2e(args.steps, args.warmup, barrier, run=job.run_e2e_unpacked)) / args.steps
+    e2e_check = job.verify_e2e()
 
     metric, value1, unit = headline(args.workload, work, ms_step)
     _, e2e1, _ = headline(args.workload, work, e2e_ms)
@@ -798,8 +951,10 @@ def main():
                 "peak": peaks["hbm"], "unit": "GB/s", "frac": ach / peaks["hbm"],
                 "traffic": ncu_traffic("decode_fp8" if fp8 else "decode", args.workload + "_noshare"),
                 "peak_source": peaks["source"],
-                "workload": args.workload + " noshare (every drawn document distinct: algorithmic == DRAM bytes)",
-                "algorithmic_bytes_per_launch": ns["bytes"], "kernel_ms": ns["kernel_ms"]}
+                "workload": args.workload + " noshare (every drawn document distinct)",
+                "algorithmic_bytes_per_launch": ns["bytes"], "kernel_ms": ns["kernel_ms"],
+                "note": "frac on the noshare variant; value is logical bytes on the Zipf-shared batch and may exceed the "
+                        "HBM peak"}
         if not args.noshare:
             roof["shared"] = shared
     elif args.workload == "cfg3":
@@ -834,7 +989,11 @@ def main():
         "e2e": {"value": e2e_value, "unit": unit, "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": int(sum(e["h2d"] for e in job.e2e)),
                 "d2h_bytes_per_step": int(sum(e["d2h"] for e in job.e2e)),
-                "api": "lazy_host_step_packed: one H2D copy of the packed inputs, the kernels, one D2H copy"},
+                "api": "lazy_host_step_packed: one H2D copy of the packed inputs, the kernels, one D2H copy "
+                       "(packing into the pinned block is the caller's and is not timed)",
+                "unpacked": {"api": "lazy_host_step: seven H2D copies from separate pinned tensors", "ms_per_step": e2e_unpacked_ms,
+                             "value": headline(args.workload, work, e2e_unpacked_ms)[1] * world},
+                "verified": e2e_check},
         "gpu_launches": int(launches), "clocks": clocks,
     }
     if args.mixed and rank == 0 and world == 1 and args.workload == "cfg5":
@@ -887,8 +1046,10 @@ def main():
         g_ms = float(np.mean([a.elapsed_time(b) for a, b in evs]))
         out["graph"] = {"ms_per_step": g_ms, "eager_ms_per_step": ms_step,
                         "launches_per_step": int(launches) // max(1, args.steps)}
-    if args.ablation and rank == 0 and world == 1 and args.workload != "cfg5":
-        abl = run_ablation(job, max(5, args.steps), 3)
+    default_abl = args.workload == "cfg2" and not args.no_secondary and not fp8 and not args.noshare
+    if (args.ablation or default_abl) and rank == 0 and world == 1 and args.workload != "cfg5":
+        # rows f1 / f2 (Fig. 5): in the default command a cut-down run on cfg2
+        abl = run_ablation(job, max(5, args.steps) if args.ablation else 10, 3)
         abl["lazy_shared_ms"] = ms_attn
         abl["materialise_then_attend_ms"] = abl["materialize_ms"] + abl["absolute_ms"]
         abl["lazy_speedup_vs_materialising"] = abl["materialise_then_attend_ms"] / ms_attn
@@ -918,7 +1079,8 @@ def main():
         out["cpu_baseline"] = {"value": v, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample,
                                "seconds": t}
     if rank == 0:
-        print(json.dumps(out))
+        sys.stderr.write("detail: " + json.dumps(out) + "\n")          # the verbose record (prose, byte counts)
+        print(json.dumps(compact_line(out)))
     if dist is not None:
         dist.destroy_process_group()
 
