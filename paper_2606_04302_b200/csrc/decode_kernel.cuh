@@ -569,20 +569,66 @@ __device__ __forceinline__ void decode_cta(const CUtensorMap& tmap_k, const CUte
         }
       }
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(bar_empty + 8 * stage);
+      // PPS > 1: the segment's LAST stage stays held -- its K / V tiles are the staging area of the page-lane merge below
+      if (lane == 0 && !(C::PPS > 1 && ul == seg_hi - 1)) ptx::mbar_arrive(bar_empty + 8 * stage);
     }
 
-    // ---- segment done: this warp's partial (o, m, l) for its kv head -> workspace (a8)
+    // ---- segment done.  PPS > 1 (fewer than 8 kv heads per CTA): the PPS page lanes of one kv head are merged inside
+    // the CTA first, so that a CTA writes ONE partial per (request, kv head) instead of PPS -- half (a quarter, an
+    // eighth) of the partial traffic and of the last arriver's combine work.  Both warps of a kv head hold the same
+    // (head column, dim) elements in the same lanes, so the hand-over is lane to lane: warp (pl > 0, hl) parks its
+    // accumulators in its OWN K tile of the held stage (NC float4 per lane, [i][lane] order: conflict-free) and
+    // (m, m, l, l) in its own V tile; warp (0, hl) folds them in with the usual running-max rescale.
+    if (C::PPS > 1) {
+      const uint32_t stl = smem_base + ((it - 1) % C::NSTAGES) * C::STAGE_BYTES;
+      if (pl > 0) {
+#pragma unroll
+        for (int i = 0; i < C::NC; ++i)
+          ptx::sts128(stl + pl * C::PAGE_BYTES + (i / 4) * C::BOX_BYTES + hl * 2048 + ((i % 4) * 32 + lane) * 16,
+                      make_uint4(__float_as_uint(oacc[i][0]), __float_as_uint(oacc[i][1]), __float_as_uint(oacc[i][2]),
+                                 __float_as_uint(oacc[i][3])));
+        ptx::sts128(stl + C::OFF_V + pl * C::PAGE_BYTES + hl * 2048 + lane * 16,
+                    make_uint4(__float_as_uint(m_run[0]), __float_as_uint(m_run[1]), __float_as_uint(l_run[0]),
+                               __float_as_uint(l_run[1])));
+        ptx::fence_proxy_async();                   // the next fill of this stage is a TMA (async-proxy) write
+      }
+      ptx::named_bar_sync(1, kConsumerWarps * 32);
+      if (pl == 0) {
+#pragma unroll 1
+        for (int q = 1; q < C::PPS; ++q) {
+          const float4 ml = ptx::lds128f(stl + C::OFF_V + q * C::PAGE_BYTES + hl * 2048 + lane * 16);
+          const float mn0 = fmaxf(m_run[0], ml.x), mn1 = fmaxf(m_run[1], ml.y);
+          const float fa0 = m_run[0] == -INFINITY ? 0.f : exp2f(m_run[0] - mn0);
+          const float fa1 = m_run[1] == -INFINITY ? 0.f : exp2f(m_run[1] - mn1);
+          const float fb0 = ml.x == -INFINITY ? 0.f : exp2f(ml.x - mn0);
+          const float fb1 = ml.y == -INFINITY ? 0.f : exp2f(ml.y - mn1);
+          m_run[0] = mn0; m_run[1] = mn1;
+          l_run[0] = l_run[0] * fa0 + ml.z * fb0;
+          l_run[1] = l_run[1] * fa1 + ml.w * fb1;
+#pragma unroll
+          for (int i = 0; i < C::NC; ++i) {
+            const float4 v = ptx::lds128f(stl + q * C::PAGE_BYTES + (i / 4) * C::BOX_BYTES + hl * 2048 +
+                                          ((i % 4) * 32 + lane) * 16);
+            oacc[i][0] = oacc[i][0] * fa0 + v.x * fb0; oacc[i][1] = oacc[i][1] * fa1 + v.y * fb1;
+            oacc[i][2] = oacc[i][2] * fa0 + v.z * fb0; oacc[i][3] = oacc[i][3] * fa1 + v.w * fb1;
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(bar_empty + 8 * ((it - 1) % C::NSTAGES));
+    }
+
+    // ---- this kv head's partial (o, m, l) -> workspace (a8); written by the page-lane-0 warp
 #pragma unroll
     for (int o = 4; o < 32; o <<= 1) {
       l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], o);
       l_run[1] += __shfl_xor_sync(0xffffffffu, l_run[1], o);
     }
-    const int slot = (r + bid) * C::PPS + pl;
+    const int slot = r + bid;
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const int n = 2 * tq + e;
-      if (n < group) {
+      if (n < group && pl == 0) {
         const int hq = hk * group + n;
         float* po = a.part_o + ((size_t)slot * sh.Hq + hq) * D;
 #pragma unroll
@@ -610,7 +656,7 @@ __device__ __forceinline__ void decode_cta(const CUtensorMap& tmap_k, const CUte
     if (*s_flag) {
       __threadfence();
       // the ring is idle iff this segment ends the CTA's range (every issued stage has been consumed)
-      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane,
+      combine_request<D>(a, r, hg, HKV_CTA * group, n_parts, r + b_first, warp, lane,
                          s_cum[r] + seg_hi == u_end, smem_base, C::NSTAGES * C::STAGE_BYTES, bar_comb, comb_phase);
     }
     ptx::named_bar_sync(1, kConsumerWarps * 32);    // s_flag is reused by the next segment
