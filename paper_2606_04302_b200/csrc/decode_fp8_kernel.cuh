@@ -455,10 +455,11 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
         }
       }
       __syncwarp();
-      if (lane == 0) ptx::mbar_arrive(bar_empty + 8 * stage);
+      // PPS > 1: the segment's LAST stage stays held -- its tiles are the staging area of the page-lane merge below
+      if (lane == 0 && !(C::PPS > 1 && ul == seg_hi - 1)) ptx::mbar_arrive(bar_empty + 8 * stage);
     }
 
-    // ---- segment done: O back to true units, then this warp's partial (o, m, l) -> workspace (a8)
+    // ---- segment done: O back to true units, softmax sums reduced over the token lanes
 #pragma unroll
     for (int i = 0; i < C::NC; ++i) { oacc[i][0] *= c_run; oacc[i][1] *= c_run; oacc[i][2] *= c_run; oacc[i][3] *= c_run; }
 #pragma unroll
@@ -466,11 +467,56 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
       l_run[0] += __shfl_xor_sync(0xffffffffu, l_run[0], o);
       l_run[1] += __shfl_xor_sync(0xffffffffu, l_run[1], o);
     }
-    const int slot = (r + bid) * C::PPS + pl;
+    // PPS > 1: the page lanes of one kv head are merged inside the CTA (as in decode_kernel.cuh): warp (pl > 0, hl)
+    // parks its accumulators lane to lane in its OWN K and V code tiles of the held stage (NC float4 per lane, half in
+    // each tile) and (m, m, l, l) of its four head-column pairs in its own K-scale slot (64 bytes); warp (0, hl) folds
+    // them in.  One partial per (request, kv head, CTA) instead of PPS.
+    if (C::PPS > 1) {
+      const uint32_t stl = smem_base + ((it - 1) % C::NSTAGES) * C::STAGE_BYTES;
+      const uint32_t tile = (uint32_t)(hl * 16 * D);
+      if (pl > 0) {
+#pragma unroll
+        for (int i = 0; i < C::NC; ++i)
+          ptx::sts128(stl + (i < C::NC / 2 ? 0 : C::OFF_V) + pl * C::PAGE_BYTES + tile + ((i % (C::NC / 2)) * 32 + lane) * 16,
+                      make_uint4(__float_as_uint(oacc[i][0]), __float_as_uint(oacc[i][1]), __float_as_uint(oacc[i][2]),
+                                 __float_as_uint(oacc[i][3])));
+        if (g == 0)
+          ptx::sts128(stl + C::OFF_SK + pl * C::SC_BYTES + hl * 64 + tq * 16,
+                      make_uint4(__float_as_uint(m_run[0]), __float_as_uint(m_run[1]), __float_as_uint(l_run[0]),
+                                 __float_as_uint(l_run[1])));
+        ptx::fence_proxy_async();                   // the next fill of this stage is an async-proxy write
+      }
+      ptx::named_bar_sync(1, NCW * 32);
+      if (pl == 0) {
+#pragma unroll 1
+        for (int q = 1; q < C::PPS; ++q) {
+          const float4 ml = ptx::lds128f(stl + C::OFF_SK + q * C::SC_BYTES + hl * 64 + tq * 16);
+          const float mn0 = fmaxf(m_run[0], ml.x), mn1 = fmaxf(m_run[1], ml.y);
+          const float fa0 = m_run[0] == -INFINITY ? 0.f : exp2f(m_run[0] - mn0);
+          const float fa1 = m_run[1] == -INFINITY ? 0.f : exp2f(m_run[1] - mn1);
+          const float fb0 = ml.x == -INFINITY ? 0.f : exp2f(ml.x - mn0);
+          const float fb1 = ml.y == -INFINITY ? 0.f : exp2f(ml.y - mn1);
+          m_run[0] = mn0; m_run[1] = mn1;
+          l_run[0] = l_run[0] * fa0 + ml.z * fb0;
+          l_run[1] = l_run[1] * fa1 + ml.w * fb1;
+#pragma unroll
+          for (int i = 0; i < C::NC; ++i) {
+            const float4 v = ptx::lds128f(stl + (i < C::NC / 2 ? 0 : C::OFF_V) + q * C::PAGE_BYTES + tile +
+                                          ((i % (C::NC / 2)) * 32 + lane) * 16);
+            oacc[i][0] = oacc[i][0] * fa0 + v.x * fb0; oacc[i][1] = oacc[i][1] * fa1 + v.y * fb1;
+            oacc[i][2] = oacc[i][2] * fa0 + v.z * fb0; oacc[i][3] = oacc[i][3] * fa1 + v.w * fb1;
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) ptx::mbar_arrive(bar_empty + 8 * ((it - 1) % C::NSTAGES));
+    }
+    // ---- this kv head's partial (o, m, l) -> workspace (a8); written by the page-lane-0 warp
+    const int slot = r + bid;
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const int n = 2 * tq + e;
-      if (n < group) {
+      if (n < group && pl == 0) {
         const int hq = hk * group + n;
         float* po = a.part_o + ((size_t)slot * sh.Hq + hq) * D;
 #pragma unroll
@@ -497,7 +543,7 @@ __device__ __forceinline__ void decode_fp8_cta(const CUtensorMap& tmap_k, const 
     if (*s_flag) {
       __threadfence();
       // the ring is idle iff this segment ends the CTA's range (every issued stage has been consumed)
-      combine_request<D, NCW>(a, r, hg, HKV_CTA * group, n_parts * C::PPS, (r + b_first) * C::PPS, warp, lane,
+      combine_request<D, NCW>(a, r, hg, HKV_CTA * group, n_parts, r + b_first, warp, lane,
                          s_cum[r] + seg_hi == u_end, smem_base, C::NSTAGES * C::STAGE_BYTES, bar_comb, comb_phase);
     }
     ptx::named_bar_sync(1, NCW * 32);
