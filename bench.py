@@ -528,7 +528,7 @@ def compact_line(out):
     kernel times only, and LAST a flat `summary` -- so that it survives any tail cut -- with both halves of
     BASELINE.json's metric (decode HBM fraction, prefill tensor fraction) and the f1 / f2 figures."""
     line = {k: v for k, v in out.items() if k not in ("configs", "roofline", "e2e", "clocks", "ablation", "tokens_per_s",
-                                                      "cpu_baseline", "mixed", "graph")}
+                                                      "cpu_baseline", "mixed", "graph", "e3")}
     line["config"] = dict(out["config"], l2="flushed between timed steps", parallelism=f"replicas x{out['n_gpus']}")
     r = out["roofline"]
     line["roofline"] = {k: r[k] for k in ("bound", "kernel", "achieved", "peak", "unit", "frac", "traffic", "peak_source",
@@ -542,7 +542,7 @@ def compact_line(out):
         line["e2e"]["lazy_host_step_ms"] = e["unpacked"]["ms_per_step"]
         line["e2e"]["verified"] = e["verified"]
     line["clocks"] = {k: v for k, v in out["clocks"].items() if k not in ("window", "samples")}
-    for k in ("mixed", "graph"):
+    for k in ("mixed", "graph", "e3"):
         if k in out:
             line[k] = out[k]
     c = out.get("configs") or {}
@@ -842,6 +842,9 @@ def main():
                     help="cfg5: also time the step with lazy_attn_mixed (prefill and decode concurrently, f4)")
     ap.add_argument("--graph", action="store_true",
                     help="also replay the step from a CUDA graph (f4) and report its time next to the eager one")
+    ap.add_argument("--e3", action="store_true",
+                    help="also run the f1 / f2 ablation on the paper's own E3 shape: 1 request, 5 x 4,096-token documents + a "
+                         "64-token query (PAPER.md L273), decode and the 64-row query prefill")
     ap.add_argument("--ablation", action="store_true",
                     help="also time the stored-position / absolute K layouts and the materialising re-encoding (f1/f2)")
     args = ap.parse_args()
@@ -1073,6 +1076,23 @@ def main():
                 side[name] = {"error": repr(e)}
             torch.cuda.empty_cache()
         out["configs"] = side
+
+    if args.e3 and rank == 0 and world == 1:
+        # PAPER.md L271-297 (Fig. 5): the rotation's overhead on the paper's own ablation shape, next to its +0.13 %
+        from paper_2606_04302_b200 import workloads as W
+        e3 = {}
+        for name, dec in (("decode", True), ("prefill_64_rows", False)):
+            b3 = W.e3_paper(decode=dec)
+            j3 = GpuJob(b3, device)
+            _, a3, _ = j3.time_steps(20, 3, barrier)
+            ab3 = run_ablation(j3, 20, 3)
+            e3[name] = {"seq_len": int(j3.timed[-1]["step"].seq_lens[0]), "lazy_ms": a3 / 20,
+                        **{k: ab3[k] for k in ("unrotated_ms", "stored_pos_ms", "absolute_ms", "rotation_overhead_pct",
+                                               "stored_pos_overhead_pct", "materialize_ms")}}
+            j3.dev.close()
+            del j3, b3
+            torch.cuda.empty_cache()
+        out["e3"] = e3
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         v, t, sample, cores = oracle_sample(args.workload, batch)

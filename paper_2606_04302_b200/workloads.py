@@ -269,6 +269,17 @@ def config4(scale: float = 1.0, **kw) -> LazyBatch:
                           prefill_question=False, **kw)
 
 
+def e3_paper(decode: bool, **kw) -> LazyBatch:
+    """The shape of the paper's overhead ablation (Fig. 5): ONE request over 5 cached documents of 4,096
+    tokens each plus a 64-token query, Llama-3-8B layer shape.  decode=True: one decode token over the 20,545-token
+    sequence; decode=False: the 64-row query prefill over the cached documents.  A measurement shape for
+    `bench.py --e3`, not one of BASELINE.json's configs."""
+    shape = LazyShape(32, 8, 128, 5.0e5)
+    return make_rag_batch("e3_decode" if decode else "e3_prefill", shape, seed=SEED0 + 6, pool_docs=5, doc_len=4096,
+                          num_reqs=1, docs_per_req=5, alpha=1.0, replace=False, question_len=64, decode=decode,
+                          prefill_question=not decode, **kw)
+
+
 def config5(scale: float = 1.0, q_scale: float = 1.0, noshare: bool = False) -> LazyBatch:
     """Mixed serving step (Hq=28, Hkv=4, theta 1e6): 16 decode requests over 20 cached docs x 512
     (pool 2000, Zipf 0.8) + 4 cache-miss docs x 1024 prefilled block-locally (positions from 0, causal)

@@ -82,3 +82,10 @@ def test_long_positions_128k():
     _run(b)
     b = W.config3(scale=0.07, pos_shift=131072 - 10496 - 16)
     _run(b)
+
+
+@pytest.mark.parametrize("decode", [True, False], ids=["decode", "prefill_64_rows"])
+def test_e3_paper_shape(decode):
+    """The paper's overhead-ablation shape (one request, 5 x 4,096-token documents + a 64-token query),
+    the batch `bench.py --e3` times: the decode token / every query row of the 64-row prefill against the oracle."""
+    _run(W.e3_paper(decode=decode))
